@@ -1,0 +1,133 @@
+"""ctypes wrapper around oracle/liboracle.so (argument marshalling only).
+
+TEST INFRASTRUCTURE: see the header of tpc_oracle.cpp for who may import this.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+_MAX_ROWS = 256
+
+
+class _Params(C.Structure):
+    _fields_ = [
+        ("n_sectors", C.c_int32), ("n_rows", C.c_int32),
+        ("row_x", C.c_float * _MAX_ROWS),
+        ("tan_half_sector", C.c_float), ("bz_tesla", C.c_float), ("err_y2", C.c_float), ("err_z2", C.c_float),
+        ("cell_y", C.c_float), ("cell_z", C.c_float),
+        ("link_ay", C.c_float), ("link_az", C.c_float), ("link_b", C.c_float), ("link_T", C.c_float),
+        ("min_chain_len", C.c_int32), ("max_gap", C.c_int32), ("min_tracklet_hits", C.c_int32),
+        ("min_track_hits", C.c_int32),
+        ("pick_chi2_cut", C.c_float), ("max_sinphi", C.c_float), ("y_margin", C.c_float),
+        ("init_c_ss", C.c_float), ("init_c_tt", C.c_float), ("init_c_qq", C.c_float),
+    ]
+
+
+_KINDS = {0: np.int32, 1: np.float32, 2: np.float64, 3: np.uint64, 4: np.int64}
+_lib = None
+
+
+def oracle_lib_path() -> str:
+    return _build.LIB
+
+
+def build_oracle(force: bool = False) -> str:
+    return _build.build(force)
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(_build.build())
+        lib.orc_create.restype = C.c_void_p
+        lib.orc_create.argtypes = [C.c_void_p]
+        lib.orc_destroy.argtypes = [C.c_void_p]
+        lib.orc_run.restype = C.c_int
+        lib.orc_run.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int]
+        lib.orc_get.restype = C.c_int
+        lib.orc_get.argtypes = [C.c_void_p, C.c_char_p, C.POINTER(C.c_void_p), C.POINTER(C.c_int64), C.POINTER(C.c_int)]
+        lib.orc_kf_propagate.restype = C.c_int
+        lib.orc_kf_propagate.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p]
+        lib.orc_kf_update.restype = None
+        lib.orc_kf_update.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_void_p]
+        lib.orc_kf_fit.restype = C.c_int
+        lib.orc_kf_fit.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                   C.c_void_p, C.c_void_p]
+        assert lib.orc_params_size() == C.sizeof(_Params)
+        _lib = lib
+    return _lib
+
+
+def _pack(params: dict) -> _Params:
+    p = _Params()
+    rx = np.asarray(params["row_x"], dtype=np.float32)
+    assert rx.shape[0] == params["n_rows"] <= _MAX_ROWS
+    for name, _ in _Params._fields_:
+        if name == "row_x":
+            for i, v in enumerate(rx):
+                p.row_x[i] = float(v)
+        else:
+            setattr(p, name, params[name].item() if hasattr(params[name], "item") else params[name])
+    return p
+
+
+class Oracle:
+    """One oracle instance = one parameter set.  ``run`` executes stages 1..last_stage."""
+
+    def __init__(self, params: dict):
+        self._lib = _load()
+        self._p = _pack(params)
+        self._h = self._lib.orc_create(C.byref(self._p))
+        self._keep = None
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            self._lib.orc_destroy(self._h)
+            self._h = None
+
+    def run(self, sector, row, y, z, precision: int = 32, last_stage: int = 5) -> "Oracle":
+        sector = np.ascontiguousarray(sector, dtype=np.uint8)
+        row = np.ascontiguousarray(row, dtype=np.uint8)
+        y = np.ascontiguousarray(y, dtype=np.float32)
+        z = np.ascontiguousarray(z, dtype=np.float32)
+        self._keep = (sector, row, y, z)
+        rc = self._lib.orc_run(self._h, sector.shape[0], sector.ctypes.data, row.ctypes.data, y.ctypes.data,
+                               z.ctypes.data, precision, last_stage)
+        if rc != 0:
+            raise ValueError(f"oracle rejected the input (rc={rc})")
+        return self
+
+    def get(self, name: str) -> np.ndarray:
+        ptr = C.c_void_p(); n = C.c_int64(); kind = C.c_int()
+        if self._lib.orc_get(self._h, name.encode(), C.byref(ptr), C.byref(n), C.byref(kind)) != 0:
+            raise KeyError(name)
+        dt = np.dtype(_KINDS[kind.value])
+        if n.value == 0:
+            return np.empty(0, dt)
+        buf = (C.c_char * (n.value * dt.itemsize)).from_address(ptr.value)
+        return np.frombuffer(buf, dtype=dt).copy()
+
+    # ---- single Kalman-filter steps, for the pins
+    def kf_propagate(self, par, cov15, x0, x1, precision=64):
+        par = np.array(par, dtype=np.float64); cov = np.array(cov15, dtype=np.float64); jac = np.zeros(25)
+        ok = self._lib.orc_kf_propagate(C.byref(self._p), precision, par.ctypes.data, cov.ctypes.data, float(x0),
+                                        float(x1), jac.ctypes.data)
+        return bool(ok), par, cov, jac.reshape(5, 5)
+
+    def kf_update(self, par, cov15, ym, zm_rel, chi2=0.0, precision=64):
+        par = np.array(par, dtype=np.float64); cov = np.array(cov15, dtype=np.float64); c2 = np.array([chi2], dtype=np.float64)
+        self._lib.orc_kf_update(C.byref(self._p), precision, par.ctypes.data, cov.ctypes.data, float(ym), float(zm_rel),
+                                c2.ctypes.data)
+        return par, cov, float(c2[0])
+
+    def kf_fit(self, x, y, z, precision=64):
+        x = np.ascontiguousarray(x, dtype=np.float64); y = np.ascontiguousarray(y, dtype=np.float64)
+        z = np.ascontiguousarray(z, dtype=np.float64)
+        par = np.zeros(5); cov = np.zeros(15); c2 = np.zeros(1)
+        ok = self._lib.orc_kf_fit(C.byref(self._p), precision, x.shape[0], x.ctypes.data, y.ctypes.data, z.ctypes.data,
+                                  par.ctypes.data, cov.ctypes.data, c2.ctypes.data)
+        return bool(ok), par, cov, float(c2[0])

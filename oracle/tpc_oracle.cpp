@@ -1,0 +1,682 @@
+// =============================================================================================
+// TEST INFRASTRUCTURE - NOT PART OF THE PRODUCT.
+//
+// Plain, slow, single-threaded CPU oracle for the TPC sector track finder ("Track Finding",
+// PAPER.md:137 Table 1; section 6).  The paper names the step but defers the algorithm
+// to references that are not available; the five steps come from BASELINE.json `north_star`
+// (sort+bin, neighbours finder, link cleaner, Kalman tracklet constructor, selector) and every
+// formula below is the reading fixed in DESIGN.md section 3 ("The method, step by step").  This file
+// follows that text in its order and notation; DESIGN.md is the authority when the two differ.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// build, load or call this.  It shares no code, header, table or constant generator with
+// paper_2009_07515_b200/csrc (the CUDA product) and neither includes the other.
+//
+// Arithmetic contract: fp32, round-to-nearest-even, one rounding per written
+// operation, evaluation order exactly as written, no FMA contraction (build with
+// -ffp-contract=off, no -ffast-math), only + - * / sqrt floor fabs.  Stage 4 is templated on the
+// scalar: the float instance is the parity reference, the double instance exists for the
+// analytic pins (tests/test_oracle_*.py) and to measure the fp32 error.
+//
+// Pins (tests/, -m "not gpu"): S1 vs numpy lexsort + independent bin recomputation; S2 vs
+// brute-force all-pairs search; S3 invariants + brute-force chain walk; helix step vs closed-form
+// circle, Jacobian vs finite differences; KF vs closed-form weighted line fit at Bz=0 and vs
+// generator truth (q/pT 1e-4 rel.) on noise-free helices, pulls on smeared input; S5 vs
+// brute-force ownership.  Unpinned beyond invariants + truth efficiency: the S4 pick-up /
+// phase logic (stated in DESIGN.md section 6, "parity unpinned").
+// =============================================================================================
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <map>
+#include <numeric>
+#include <string>
+#include <vector>
+
+namespace {
+
+constexpr int kMaxRows = 256;
+
+struct Params {             // mirrors the ctypes Structure in oracle/oracle.py (not the product header)
+  int32_t n_sectors, n_rows;
+  float row_x[kMaxRows];
+  float tan_half_sector, bz_tesla, err_y2, err_z2, cell_y, cell_z;
+  float link_ay, link_az, link_b, link_T;
+  int32_t min_chain_len, max_gap, min_tracklet_hits, min_track_hits;
+  float pick_chi2_cut, max_sinphi, y_margin, init_c_ss, init_c_tt, init_c_qq;
+};
+
+// floor(v) clamped to [0, hi]; defined for every v (NaN and negatives -> 0), DESIGN.md section 3.1 (3)
+inline int floor_clamp(float v, int hi) {
+  const float f = std::floor(v);
+  if (!(f >= 0.0f)) return 0;
+  if (f >= (float)hi) return hi;
+  return (int)f;
+}
+
+// ------------------------------------------------------------------------------------------
+// Kalman filter pieces.  State p = (y, z_rel, s=sin(phi), t=tan(lambda), q=q/pT) at a
+// pad-row plane x; C is the full symmetric 5x5 (lower triangle computed, upper mirrored).
+// ------------------------------------------------------------------------------------------
+template <class T>
+struct KF {
+  T p[5];
+  T C[5][5];
+  T chi2;
+};
+
+// Helix step x -> x+dx in a uniform Bz (exact circle in xy), DESIGN.md section 3.4.1.
+// Returns false and leaves (p, C) untouched if |s| or |s1| >= max_sinphi.
+template <class T>
+bool kf_propagate(KF<T>& k, T kb, T dx, T max_sinphi, T* jac_out /*25, row-major, may be null*/) {
+  const T y = k.p[0], z = k.p[1], s = k.p[2], t = k.p[3], q = k.p[4];
+  const T c = kb * q;                                   // curvature
+  const T s1 = s + c * dx;
+  if (!(std::fabs(s) < max_sinphi) || !(std::fabs(s1) < max_sinphi)) return false;
+  const T c0 = std::sqrt(T(1) - s * s);
+  const T c1 = std::sqrt(T(1) - s1 * s1);
+  const T cc = c0 + c1;
+  const T ss = s + s1;
+  const T Tn = ss / cc;                                 // tan of the chord direction
+  const T y1 = y + dx * Tn;
+  const T dl = dx * std::sqrt(T(1) + Tn * Tn);          // signed chord length
+  const T u = (T(0.5) * c) * dl;
+  const T w = u * u;
+  // asin(u)/u = 1 + w/6 + 3w^2/40 + 5w^3/112 + 35w^4/1152 + ...   (no libm transcendental)
+  const T ser = T(1) + w * (T(1.0 / 6.0) + w * (T(3.0 / 40.0) + w * (T(5.0 / 112.0) + w * T(35.0 / 1152.0))));
+  const T arc = dl * ser;                               // signed xy arc length
+  const T z1 = z + t * arc;
+
+  // Jacobian d(p1)/d(p0); identity except the six entries below.
+  const T c0c1 = c0 * c1;
+  const T kdx = kb * dx;
+  const T j_ys = dx * (c0 + s * Tn) / c0c1;
+  const T j_yq = (kdx * dx) * (c1 * cc + s1 * ss) / (c1 * (cc * cc));
+  const T j_sq = kdx;
+  const T j_zt = arc;
+  const T j_zs = (t * dx) * Tn / c0c1;
+  const T sm = s + (T(0.5) * c) * dx;                   // sin(phi) at the step midpoint (Simpson)
+  const T cm = std::sqrt(T(1) - sm * sm);
+  const T j_zq = ((t * kdx) * dx) * T(1.0 / 6.0) * (T(2) * sm / (cm * cm * cm) + s1 / (c1 * c1 * c1));
+
+  T J[5][5];
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j < 5; ++j) J[i][j] = (i == j) ? T(1) : T(0);
+  J[0][2] = j_ys; J[0][4] = j_yq; J[1][2] = j_zs; J[1][3] = j_zt; J[1][4] = j_zq; J[2][4] = j_sq;
+
+  // C1 = J C J^T: M = J C (k ascending), C1[i][j] = sum_l M[i][l] J[j][l] (l ascending) for i >= j, mirrored.
+  T M[5][5];
+  for (int i = 0; i < 5; ++i)
+    for (int l = 0; l < 5; ++l) {
+      T acc = T(0);
+      for (int kk = 0; kk < 5; ++kk) acc = acc + J[i][kk] * k.C[kk][l];
+      M[i][l] = acc;
+    }
+  T C1[5][5];
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j <= i; ++j) {
+      T acc = T(0);
+      for (int l = 0; l < 5; ++l) acc = acc + M[i][l] * J[j][l];
+      C1[i][j] = acc;
+      C1[j][i] = acc;
+    }
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j < 5; ++j) k.C[i][j] = C1[i][j];
+  k.p[0] = y1; k.p[1] = z1; k.p[2] = s1;                // t, q unchanged
+  if (jac_out)
+    for (int i = 0; i < 5; ++i)
+      for (int j = 0; j < 5; ++j) jac_out[i * 5 + j] = J[i][j];
+  return true;
+}
+
+// Textbook Kalman update with the measurement m = (y_m, z_m - z_ref), V = diag(err_y2, err_z2), H = [I2 0]
+// (DESIGN.md section 3.4.2).  No gate here.
+template <class T>
+void kf_update(KF<T>& k, T ym, T zm, T err_y2, T err_z2) {
+  const T r0 = ym - k.p[0];
+  const T r1 = zm - k.p[1];
+  const T S00 = k.C[0][0] + err_y2;
+  const T S10 = k.C[1][0];
+  const T S11 = k.C[1][1] + err_z2;
+  const T det = S00 * S11 - S10 * S10;
+  const T idet = T(1) / det;
+  const T I00 = S11 * idet, I10 = (T(0) - S10) * idet, I11 = S00 * idet;   // S^-1 (symmetric)
+  k.chi2 = k.chi2 + ((r0 * r0) * I00 + (T(2) * (r0 * r1)) * I10 + (r1 * r1) * I11);
+  T K0[5], K1[5];                                       // gain K = C H^T S^-1   (5x2)
+  for (int i = 0; i < 5; ++i) {
+    K0[i] = k.C[i][0] * I00 + k.C[i][1] * I10;
+    K1[i] = k.C[i][0] * I10 + k.C[i][1] * I11;
+  }
+  T C1[5][5];
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j <= i; ++j) {                      // C -= K (H C), lower triangle then mirror
+      const T v = k.C[i][j] - (K0[i] * k.C[0][j] + K1[i] * k.C[1][j]);
+      C1[i][j] = v;
+      C1[j][i] = v;
+    }
+  for (int i = 0; i < 5; ++i) k.p[i] = k.p[i] + (K0[i] * r0 + K1[i] * r1);
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j < 5; ++j) k.C[i][j] = C1[i][j];
+}
+
+template <class T>
+void kf_reset_cov(KF<T>& k, const Params& P) {
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j < 5; ++j) k.C[i][j] = T(0);
+  k.C[0][0] = T(P.err_y2); k.C[1][1] = T(P.err_z2);
+  k.C[2][2] = T(P.init_c_ss); k.C[3][3] = T(P.init_c_tt); k.C[4][4] = T(P.init_c_qq);
+  k.chi2 = T(0);
+}
+
+// ------------------------------------------------------------------------------------------
+struct Oracle {
+  Params P;
+  int n_sr = 0;                        // n_sectors * n_rows
+  float kb = 0.f;                      // curvature constant
+  float inv_cy = 0.f, inv_cz = 0.f;
+  std::vector<float> ymax;             // [n_rows]
+  std::vector<int32_t> ny;             // [n_rows]
+  // link tables, index [row][k-1], k = row step 1 or 2
+  std::vector<float> up_dx, up_ratio, up_wy, up_wz, dn_dx, dn_ratio, dn_wy, dn_wz;
+
+  // input (borrowed for the duration of run())
+  int64_t n = 0;
+  const uint8_t* in_sector = nullptr; const uint8_t* in_row = nullptr;
+  const float* in_y = nullptr; const float* in_z = nullptr;
+
+  // S1
+  std::vector<float> zmin, zmax; std::vector<int32_t> nz;         // per sector
+  std::vector<int32_t> bin_base;                                  // [n_sr+1]
+  std::vector<int32_t> gbin;                                      // [n] global bin of input cluster
+  std::vector<int32_t> perm;                                      // [n] sorted position -> input index
+  std::vector<float> ys, zs;                                      // [n] sorted
+  std::vector<int32_t> s_sector, s_row;                           // [n] sorted (oracle convenience)
+  std::vector<int32_t> bin_start;                                 // [n_bins+1]
+  std::vector<int32_t> row_start;                                 // [n_sr+1]
+  // S2
+  std::vector<int32_t> link_up_raw, link_dn_raw;
+  // S3
+  std::vector<int32_t> link_up, link_dn, seed_head, seed_len;
+  // S4 (per seed; values held as double, exact for the float instance)
+  std::vector<int32_t> t_hit;                                     // [n_seeds * n_rows] sorted position or -1
+  std::vector<int32_t> t_first_row, t_last_row, t_n_hits, t_kept, t_ndf, t_sector;
+  std::vector<double> t_par, t_cov, t_x_ref, t_z_ref, t_chi2;     // par [n_seeds*5], cov [n_seeds*15]
+  std::vector<int64_t> t_kf_steps;                                // [1] total propagate calls (for bytes model)
+  // S5
+  std::vector<int32_t> tracklet_of_seed;                          // [n_seeds] rank among kept or -1
+  std::vector<uint64_t> owner;                                    // [n] by sorted position
+  std::vector<int32_t> k_owned;                                   // [n_seeds]
+  std::vector<int32_t> trk_seed, trk_sector, trk_first_row, trk_last_row, trk_n_clusters, trk_ndf;
+  std::vector<double> trk_par, trk_cov, trk_x_ref, trk_z_ref, trk_chi2;
+  std::vector<int32_t> trk_cl_start, trk_cl_idx, cluster_track;
+  std::vector<double> stage_seconds;                              // [5]
+
+  explicit Oracle(const Params& p) : P(p) { derive(); }
+
+  // ---- host-side derived tables, each one stated fp32 expression
+  void derive() {
+    n_sr = P.n_sectors * P.n_rows;
+    kb = -0.00299792458f * P.bz_tesla;
+    inv_cy = 1.0f / P.cell_y;
+    inv_cz = 1.0f / P.cell_z;
+    ymax.resize(P.n_rows); ny.resize(P.n_rows);
+    for (int r = 0; r < P.n_rows; ++r) {
+      ymax[r] = P.row_x[r] * P.tan_half_sector;
+      ny[r] = (int)std::floor((2.0f * ymax[r]) * inv_cy) + 1;
+    }
+    auto tab = [&](std::vector<float>& v) { v.assign(P.n_rows * 2, 0.f); };
+    tab(up_dx); tab(up_ratio); tab(up_wy); tab(up_wz); tab(dn_dx); tab(dn_ratio); tab(dn_wy); tab(dn_wz);
+    for (int r = 0; r < P.n_rows; ++r)
+      for (int k = 1; k <= 2; ++k) {
+        if (r + k < P.n_rows) {
+          const float dx = P.row_x[r + k] - P.row_x[r];
+          up_dx[r * 2 + k - 1] = dx;
+          up_ratio[r * 2 + k - 1] = P.row_x[r + k] / P.row_x[r];
+          up_wy[r * 2 + k - 1] = P.link_ay * dx + P.link_b;
+          up_wz[r * 2 + k - 1] = P.link_az * dx + P.link_b;
+        }
+        if (r - k >= 0) {
+          const float dx = P.row_x[r] - P.row_x[r - k];
+          dn_dx[r * 2 + k - 1] = dx;
+          dn_ratio[r * 2 + k - 1] = P.row_x[r - k] / P.row_x[r];
+          dn_wy[r * 2 + k - 1] = P.link_ay * dx + P.link_b;
+          dn_wz[r * 2 + k - 1] = P.link_az * dx + P.link_b;
+        }
+      }
+  }
+
+  // grid coordinates (DESIGN.md section 3.1 (3)); v already fp32
+  int bin_iy(float y, int r) const { return floor_clamp((y + ymax[r]) * inv_cy, ny[r] - 1); }
+  int bin_iz(float z, int s) const { return floor_clamp((z - zmin[s]) * inv_cz, nz[s] - 1); }
+
+  // ------------------------------------------------------------------------------ S1
+  int stage1() {
+    zmin.assign(P.n_sectors, INFINITY); zmax.assign(P.n_sectors, -INFINITY); nz.assign(P.n_sectors, 0);
+    for (int64_t i = 0; i < n; ++i) {
+      if (in_sector[i] >= P.n_sectors || in_row[i] >= P.n_rows) return -1;
+      const int s = in_sector[i];
+      zmin[s] = std::min(zmin[s], in_z[i]);
+      zmax[s] = std::max(zmax[s], in_z[i]);
+    }
+    for (int s = 0; s < P.n_sectors; ++s)
+      nz[s] = (zmin[s] <= zmax[s]) ? (int)std::floor((zmax[s] - zmin[s]) * inv_cz) + 1 : 0;
+    bin_base.assign(n_sr + 1, 0);
+    int64_t acc = 0;
+    for (int s = 0; s < P.n_sectors; ++s)
+      for (int r = 0; r < P.n_rows; ++r) {
+        bin_base[s * P.n_rows + r] = (int32_t)acc;
+        acc += (int64_t)ny[r] * nz[s];
+        if (acc > INT32_MAX) return -2;
+      }
+    bin_base[n_sr] = (int32_t)acc;
+    const int64_t n_bins = acc;
+    gbin.resize(n);
+    for (int64_t i = 0; i < n; ++i) {
+      const int s = in_sector[i], r = in_row[i];
+      gbin[i] = bin_base[s * P.n_rows + r] + bin_iz(in_z[i], s) * ny[r] + bin_iy(in_y[i], r);
+    }
+    // order = ascending (sector,row,bin) = ascending global bin, ties by input index: std::stable_sort
+    perm.resize(n);
+    std::iota(perm.begin(), perm.end(), 0);
+    std::stable_sort(perm.begin(), perm.end(), [&](int32_t a, int32_t b) { return gbin[a] < gbin[b]; });
+    ys.resize(n); zs.resize(n); s_sector.resize(n); s_row.resize(n);
+    bin_start.assign(n_bins + 1, 0);
+    for (int64_t pos = 0; pos < n; ++pos) {
+      const int32_t i = perm[pos];
+      ys[pos] = in_y[i]; zs[pos] = in_z[i]; s_sector[pos] = in_sector[i]; s_row[pos] = in_row[i];
+      bin_start[gbin[i] + 1]++;
+    }
+    for (int64_t b = 0; b < n_bins; ++b) bin_start[b + 1] += bin_start[b];   // CSR: bin b = [bin_start[b], bin_start[b+1])
+    row_start.resize(n_sr + 1);
+    for (int sr = 0; sr <= n_sr; ++sr) row_start[sr] = bin_start[bin_base[sr]];
+    return 0;
+  }
+
+  // positions of row t of sector s whose (y,z) lies in the closed rectangle, visited in ascending position
+  template <class F>
+  void for_each_in_rect(int s, int t, float ylo, float yhi, float zlo, float zhi, F&& f) const {
+    if (nz[s] == 0) return;
+    const int b0 = bin_base[s * P.n_rows + t];
+    const int iy0 = bin_iy(ylo, t), iy1 = bin_iy(yhi, t), iz0 = bin_iz(zlo, s), iz1 = bin_iz(zhi, s);
+    for (int iz = iz0; iz <= iz1; ++iz) {
+      const int jb = bin_start[b0 + iz * ny[t] + iy0], je = bin_start[b0 + iz * ny[t] + iy1 + 1];
+      for (int j = jb; j < je; ++j)
+        if (ys[j] >= ylo && ys[j] <= yhi && zs[j] >= zlo && zs[j] <= zhi) f(j);
+    }
+  }
+
+  // ------------------------------------------------------------------------------ S2
+  void stage2() {
+    link_up_raw.assign(n, -1); link_dn_raw.assign(n, -1);
+    std::vector<int32_t> U, D;
+    for (int64_t i = 0; i < n; ++i) {
+      const int s = s_sector[i], r = s_row[i];
+      const float y = ys[i], z = zs[i];
+      int ku = 0, kd = 0;
+      U.clear(); D.clear();
+      for (int k = 1; k <= 2 && U.empty(); ++k) {
+        if (r + k >= P.n_rows) break;
+        const float yc = y * up_ratio[r * 2 + k - 1], wy = up_wy[r * 2 + k - 1], wz = up_wz[r * 2 + k - 1];
+        for_each_in_rect(s, r + k, yc - wy, yc + wy, z - wz, z + wz, [&](int j) { U.push_back(j); });
+        ku = k;
+      }
+      for (int k = 1; k <= 2 && D.empty(); ++k) {
+        if (r - k < 0) break;
+        const float yc = y * dn_ratio[r * 2 + k - 1], wy = dn_wy[r * 2 + k - 1], wz = dn_wz[r * 2 + k - 1];
+        for_each_in_rect(s, r - k, yc - wy, yc + wy, z - wz, z + wz, [&](int j) { D.push_back(j); });
+        kd = k;
+      }
+      if (U.empty() || D.empty()) continue;
+      const float dxu = up_dx[r * 2 + ku - 1], dxd = dn_dx[r * 2 + kd - 1];
+      const float cut = P.link_T * ((dxu * dxd) * (dxu * dxd));
+      float best = INFINITY; int bu = -1, bd = -1;
+      for (int u : U)                       // ascending u, then ascending d; strict '<' keeps the first minimum
+        for (int d : D) {
+          const float Dy = dxd * (ys[u] - y) - dxu * (y - ys[d]);
+          const float Dz = dxd * (zs[u] - z) - dxu * (z - zs[d]);
+          const float Dv = Dy * Dy + Dz * Dz;
+          if (Dv < best) { best = Dv; bu = u; bd = d; }
+        }
+      if (best <= cut) { link_up_raw[i] = bu; link_dn_raw[i] = bd; }
+    }
+  }
+
+  // ------------------------------------------------------------------------------ S3
+  void stage3() {
+    link_up.assign(n, -1); link_dn.assign(n, -1);
+    for (int64_t i = 0; i < n; ++i) {
+      const int u = link_up_raw[i], d = link_dn_raw[i];
+      if (u >= 0 && link_dn_raw[u] == i) link_up[i] = u;
+      if (d >= 0 && link_up_raw[d] == i) link_dn[i] = d;
+    }
+    seed_head.clear(); seed_len.clear();
+    for (int64_t i = 0; i < n; ++i) {
+      if (!(link_up[i] >= 0 && link_dn[i] < 0)) continue;
+      int len = 0;
+      for (int c = (int)i; c >= 0; c = link_up[c]) ++len;
+      if (len >= P.min_chain_len) { seed_head.push_back((int32_t)i); seed_len.push_back(len); }
+    }
+  }
+
+  // ------------------------------------------------------------------------------ S4
+  // nearest gated cluster of row r; returns sorted position or -1
+  template <class T>
+  int search(int s, int r, const KF<T>& k, T zref) const {
+    const T cut = T(P.pick_chi2_cut);
+    const T sy2 = k.C[0][0] + T(P.err_y2), sz2 = k.C[1][1] + T(P.err_z2);
+    const T hy = std::sqrt(cut * sy2), hz = std::sqrt(cut * sz2);
+    const T zabs = zref + k.p[1];
+    const T ylo = k.p[0] - hy, yhi = k.p[0] + hy, zlo = zabs - hz, zhi = zabs + hz;
+    const T wy = T(1) / sy2, wz = T(1) / sz2;
+    T best = T(INFINITY); int arg = -1;
+    for_each_in_rect(s, r, (float)ylo, (float)yhi, (float)zlo, (float)zhi, [&](int j) {
+      if (T(ys[j]) < ylo || T(ys[j]) > yhi || T(zs[j]) < zlo || T(zs[j]) > zhi) return;
+      const T dy = T(ys[j]) - k.p[0];
+      const T dz = (T(zs[j]) - zref) - k.p[1];
+      const T d2 = (dy * dy) * wy + (dz * dz) * wz;
+      if (d2 <= cut && d2 < best) { best = d2; arg = j; }
+    });
+    return arg;
+  }
+
+  template <class T>
+  void tracklet(int sd) {
+    const int R = P.n_rows;
+    int32_t* hit = &t_hit[(size_t)sd * R];
+    std::fill(hit, hit + R, -1);
+    const int h = seed_head[sd], nx = link_up[h];
+    const int s = s_sector[h], r0 = s_row[h], r1 = s_row[nx];
+    const T kbT = T(kb), msp = T(P.max_sinphi), ey2 = T(P.err_y2), ez2 = T(P.err_z2);
+    const T zref = T(zs[h]);
+    int64_t steps = 0;
+
+    // seed: straight line through the first two chain clusters
+    KF<T> k;
+    {
+      const T dx = T(P.row_x[r1]) - T(P.row_x[r0]);
+      const T dy = T(ys[nx]) - T(ys[h]);
+      const T dz = T(zs[nx]) - T(zs[h]);
+      const T dl = std::sqrt(dx * dx + dy * dy);
+      k.p[0] = T(ys[h]); k.p[1] = T(0); k.p[2] = dy / dl; k.p[3] = dz / dl; k.p[4] = T(0);
+      kf_reset_cov(k, P);
+    }
+    hit[r0] = h;
+    int cur = r0;                               // row the state lives on
+    KF<T> last = k; int last_row = r0;          // "last updated" state (phase A/B)
+
+    // Phase A: follow the chain upward, update without gate
+    bool up_ok = true;
+    for (int c = nx; c >= 0; c = link_up[c]) {
+      const int rc = s_row[c];
+      ++steps;
+      if (!kf_propagate(k, kbT, T(P.row_x[rc]) - T(P.row_x[cur]), msp, (T*)nullptr)) { up_ok = false; break; }
+      cur = rc;
+      kf_update(k, T(ys[c]), T(zs[c]) - zref, ey2, ez2);
+      hit[rc] = c;
+      last = k; last_row = rc;
+    }
+    // Phase B: extrapolate upward, pick up gated nearest clusters
+    if (up_ok) {
+      int gap = 0;
+      for (int r = cur + 1; r < R; ++r) {
+        ++steps;
+        if (!kf_propagate(k, kbT, T(P.row_x[r]) - T(P.row_x[cur]), msp, (T*)nullptr)) break;
+        cur = r;
+        if (!(std::fabs(k.p[0]) <= T(ymax[r]) + T(P.y_margin))) break;   // left the sector (NaN-safe)
+        const int c = search<T>(s, r, k, zref);
+        if (c >= 0) {
+          kf_update(k, T(ys[c]), T(zs[c]) - zref, ey2, ez2);
+          hit[r] = c; gap = 0;
+          last = k; last_row = r;
+        } else if (++gap > P.max_gap) break;
+      }
+    }
+    // Phase C: turn round at the last updated cluster, reset C and chi2, refit downward with pick-up
+    k = last; cur = last_row;
+    kf_reset_cov(k, P);
+    KF<T> out = k; int low = last_row;
+    {
+      int gap = 0;
+      for (int r = cur - 1; r >= 0; --r) {
+        ++steps;
+        if (!kf_propagate(k, kbT, T(P.row_x[r]) - T(P.row_x[cur]), msp, (T*)nullptr)) break;
+        cur = r;
+        if (!(std::fabs(k.p[0]) <= T(ymax[r]) + T(P.y_margin))) break;   // left the sector (NaN-safe)
+        const int c = hit[r] >= 0 ? hit[r] : search<T>(s, r, k, zref);
+        if (c >= 0) {
+          kf_update(k, T(ys[c]), T(zs[c]) - zref, ey2, ez2);
+          hit[r] = c; gap = 0;
+          out = k; low = r;
+        } else if (++gap > P.max_gap) break;
+      }
+    }
+    for (int r = 0; r < low; ++r) hit[r] = -1;
+    int nh = 0;
+    for (int r = 0; r < R; ++r) nh += hit[r] >= 0;
+    t_first_row[sd] = low; t_last_row[sd] = last_row; t_n_hits[sd] = nh; t_sector[sd] = s;
+    t_ndf[sd] = 2 * nh - 5;
+    t_kept[sd] = nh >= P.min_tracklet_hits;
+    for (int i = 0; i < 5; ++i) t_par[(size_t)sd * 5 + i] = (double)out.p[i];
+    for (int i = 0, m = 0; i < 5; ++i)
+      for (int j = 0; j <= i; ++j, ++m) t_cov[(size_t)sd * 15 + m] = (double)out.C[i][j];
+    t_x_ref[sd] = (double)P.row_x[low]; t_z_ref[sd] = (double)zref; t_chi2[sd] = (double)out.chi2;
+    t_kf_steps[0] += steps;
+  }
+
+  template <class T>
+  void stage4() {
+    const size_t K = seed_head.size();
+    t_hit.assign(K * P.n_rows, -1);
+    t_first_row.assign(K, 0); t_last_row.assign(K, 0); t_n_hits.assign(K, 0); t_kept.assign(K, 0);
+    t_ndf.assign(K, 0); t_sector.assign(K, 0);
+    t_par.assign(K * 5, 0.0); t_cov.assign(K * 15, 0.0);
+    t_x_ref.assign(K, 0.0); t_z_ref.assign(K, 0.0); t_chi2.assign(K, 0.0);
+    t_kf_steps.assign(1, 0);
+    for (size_t sd = 0; sd < K; ++sd) tracklet<T>((int)sd);
+  }
+
+  // ------------------------------------------------------------------------------ S5
+  void stage5() {
+    const size_t K = seed_head.size();
+    const int R = P.n_rows;
+    tracklet_of_seed.assign(K, -1);
+    int32_t nk = 0;
+    for (size_t sd = 0; sd < K; ++sd)
+      if (t_kept[sd]) tracklet_of_seed[sd] = nk++;
+    auto key = [&](size_t sd) {
+      return ((uint64_t)(uint32_t)t_n_hits[sd] << 32) | (uint64_t)(0xFFFFFFFFu - (uint32_t)tracklet_of_seed[sd]);
+    };
+    owner.assign(n, 0);
+    for (size_t sd = 0; sd < K; ++sd) {
+      if (!t_kept[sd]) continue;
+      const uint64_t kk = key(sd);
+      for (int r = 0; r < R; ++r) {
+        const int c = t_hit[sd * R + r];
+        if (c >= 0) owner[c] = std::max(owner[c], kk);
+      }
+    }
+    k_owned.assign(K, 0);
+    for (size_t sd = 0; sd < K; ++sd) {
+      if (!t_kept[sd]) continue;
+      const uint64_t kk = key(sd);
+      for (int r = 0; r < R; ++r) {
+        const int c = t_hit[sd * R + r];
+        if (c >= 0 && owner[c] == kk) k_owned[sd]++;
+      }
+    }
+    trk_seed.clear(); trk_sector.clear(); trk_first_row.clear(); trk_last_row.clear(); trk_n_clusters.clear();
+    trk_ndf.clear(); trk_par.clear(); trk_cov.clear(); trk_x_ref.clear(); trk_z_ref.clear(); trk_chi2.clear();
+    trk_cl_start.assign(1, 0); trk_cl_idx.clear();
+    cluster_track.assign(n, -1);
+    for (size_t sd = 0; sd < K; ++sd) {
+      if (!t_kept[sd] || k_owned[sd] < P.min_track_hits) continue;
+      const int32_t id = (int32_t)trk_seed.size();
+      const uint64_t kk = key(sd);
+      int first = -1, lastr = -1;
+      for (int r = 0; r < R; ++r) {
+        const int c = t_hit[sd * R + r];
+        if (c >= 0 && owner[c] == kk) {
+          if (first < 0) first = r;
+          lastr = r;
+          trk_cl_idx.push_back(perm[c]);
+          cluster_track[perm[c]] = id;
+        }
+      }
+      trk_cl_start.push_back((int32_t)trk_cl_idx.size());
+      trk_seed.push_back((int32_t)sd); trk_sector.push_back(t_sector[sd]);
+      trk_first_row.push_back(first); trk_last_row.push_back(lastr); trk_n_clusters.push_back(k_owned[sd]);
+      trk_ndf.push_back(t_ndf[sd]);
+      for (int i = 0; i < 5; ++i) trk_par.push_back(t_par[sd * 5 + i]);
+      for (int i = 0; i < 15; ++i) trk_cov.push_back(t_cov[sd * 15 + i]);
+      trk_x_ref.push_back(t_x_ref[sd]); trk_z_ref.push_back(t_z_ref[sd]); trk_chi2.push_back(t_chi2[sd]);
+    }
+  }
+
+  int run(int64_t n_, const uint8_t* sec, const uint8_t* row, const float* y, const float* z, int prec, int last_stage) {
+    n = n_; in_sector = sec; in_row = row; in_y = y; in_z = z;
+    stage_seconds.assign(5, 0.0);
+    auto now = [] { return std::chrono::steady_clock::now(); };
+    auto secs = [](auto a, auto b) { return std::chrono::duration<double>(b - a).count(); };
+    auto t0 = now();
+    int rc = stage1();
+    auto t1 = now(); stage_seconds[0] = secs(t0, t1);
+    if (rc != 0 || last_stage < 2) return rc;
+    stage2();
+    auto t2 = now(); stage_seconds[1] = secs(t1, t2);
+    if (last_stage < 3) return 0;
+    stage3();
+    auto t3 = now(); stage_seconds[2] = secs(t2, t3);
+    if (last_stage < 4) return 0;
+    if (prec == 64) stage4<double>(); else stage4<float>();
+    auto t4 = now(); stage_seconds[3] = secs(t3, t4);
+    if (last_stage < 5) return 0;
+    stage5();
+    auto t5 = now(); stage_seconds[4] = secs(t4, t5);
+    return 0;
+  }
+};
+
+template <class V>
+int give(const V& v, const void** ptr, int64_t* n, int* kind, int k) {
+  *ptr = v.data(); *n = (int64_t)v.size(); *kind = k;
+  return 0;
+}
+
+template <class T>
+void load_kf(KF<T>& k, const double* par, const double* cov15, double chi2) {
+  for (int i = 0; i < 5; ++i) k.p[i] = (T)par[i];
+  for (int i = 0, m = 0; i < 5; ++i)
+    for (int j = 0; j <= i; ++j, ++m) { k.C[i][j] = (T)cov15[m]; k.C[j][i] = (T)cov15[m]; }
+  k.chi2 = (T)chi2;
+}
+template <class T>
+void store_kf(const KF<T>& k, double* par, double* cov15, double* chi2) {
+  for (int i = 0; i < 5; ++i) par[i] = (double)k.p[i];
+  for (int i = 0, m = 0; i < 5; ++i)
+    for (int j = 0; j <= i; ++j, ++m) cov15[m] = (double)k.C[i][j];
+  if (chi2) *chi2 = (double)k.chi2;
+}
+
+template <class T>
+int kf_propagate_entry(const Params& P, double* par, double* cov15, double x0, double x1, double* jac25) {
+  KF<T> k; load_kf(k, par, cov15, 0.0);
+  T J[25];
+  const T kbT = T(-0.00299792458f * P.bz_tesla);
+  const bool ok = kf_propagate<T>(k, kbT, T(x1) - T(x0), T(P.max_sinphi), J);
+  if (!ok) return 0;
+  store_kf(k, par, cov15, nullptr);
+  if (jac25) for (int i = 0; i < 25; ++i) jac25[i] = (double)J[i];
+  return 1;
+}
+
+// KF over an explicit point list with the S4 seed rule + phase-A updates (no search), ending on the last point.
+template <class T>
+int kf_fit_entry(const Params& P, int npt, const double* x, const double* y, const double* z, double* par, double* cov15,
+                 double* chi2) {
+  if (npt < 2) return 0;
+  KF<T> k;
+  const T zref = T(z[0]);
+  const T dx = T(x[1]) - T(x[0]), dy = T(y[1]) - T(y[0]), dz = T(z[1]) - T(z[0]);
+  const T dl = std::sqrt(dx * dx + dy * dy);
+  k.p[0] = T(y[0]); k.p[1] = T(0); k.p[2] = dy / dl; k.p[3] = dz / dl; k.p[4] = T(0);
+  kf_reset_cov(k, P);
+  const T kbT = T(-0.00299792458f * P.bz_tesla);
+  for (int i = 1; i < npt; ++i) {
+    if (!kf_propagate<T>(k, kbT, T(x[i]) - T(x[i - 1]), T(P.max_sinphi), (T*)nullptr)) return 0;
+    kf_update<T>(k, T(y[i]), T(z[i]) - zref, T(P.err_y2), T(P.err_z2));
+  }
+  store_kf(k, par, cov15, chi2);
+  return 1;
+}
+
+}  // namespace
+
+// =============================================================================================
+extern "C" {
+
+void* orc_create(const void* params) { return new Oracle(*reinterpret_cast<const Params*>(params)); }
+void orc_destroy(void* h) { delete reinterpret_cast<Oracle*>(h); }
+int orc_params_size() { return (int)sizeof(Params); }
+
+// prec: 32 (parity reference) or 64; last_stage: 1..5
+int orc_run(void* h, int64_t n, const uint8_t* sector, const uint8_t* row, const float* y, const float* z, int prec,
+            int last_stage) {
+  return reinterpret_cast<Oracle*>(h)->run(n, sector, row, y, z, prec, last_stage);
+}
+
+// kind: 0 int32, 1 float32, 2 float64, 3 uint64, 4 int64
+int orc_get(void* h, const char* name, const void** ptr, int64_t* n, int* kind) {
+  Oracle& o = *reinterpret_cast<Oracle*>(h);
+  const std::string s(name);
+#define I32(f) if (s == #f) return give(o.f, ptr, n, kind, 0)
+#define F32(f) if (s == #f) return give(o.f, ptr, n, kind, 1)
+#define F64(f) if (s == #f) return give(o.f, ptr, n, kind, 2)
+#define U64(f) if (s == #f) return give(o.f, ptr, n, kind, 3)
+#define I64(f) if (s == #f) return give(o.f, ptr, n, kind, 4)
+  F32(ymax); I32(ny); F32(zmin); F32(zmax); I32(nz); I32(bin_base); I32(gbin); I32(perm); F32(ys); F32(zs);
+  I32(s_sector); I32(s_row); I32(bin_start); I32(row_start);
+  I32(link_up_raw); I32(link_dn_raw); I32(link_up); I32(link_dn); I32(seed_head); I32(seed_len);
+  I32(t_hit); I32(t_first_row); I32(t_last_row); I32(t_n_hits); I32(t_kept); I32(t_ndf); I32(t_sector);
+  F64(t_par); F64(t_cov); F64(t_x_ref); F64(t_z_ref); F64(t_chi2); I64(t_kf_steps);
+  I32(tracklet_of_seed); U64(owner); I32(k_owned);
+  I32(trk_seed); I32(trk_sector); I32(trk_first_row); I32(trk_last_row); I32(trk_n_clusters); I32(trk_ndf);
+  F64(trk_par); F64(trk_cov); F64(trk_x_ref); F64(trk_z_ref); F64(trk_chi2);
+  I32(trk_cl_start); I32(trk_cl_idx); I32(cluster_track); F64(stage_seconds);
+  F32(up_dx); F32(up_ratio); F32(up_wy); F32(up_wz); F32(dn_dx); F32(dn_ratio); F32(dn_wy); F32(dn_wz);
+#undef I32
+#undef F32
+#undef F64
+#undef U64
+#undef I64
+  return -1;
+}
+
+int orc_kf_propagate(const void* params, int prec, double* par, double* cov15, double x0, double x1, double* jac25) {
+  const Params& P = *reinterpret_cast<const Params*>(params);
+  return prec == 64 ? kf_propagate_entry<double>(P, par, cov15, x0, x1, jac25)
+                    : kf_propagate_entry<float>(P, par, cov15, x0, x1, jac25);
+}
+
+void orc_kf_update(const void* params, int prec, double* par, double* cov15, double ym, double zm_rel, double* chi2) {
+  const Params& P = *reinterpret_cast<const Params*>(params);
+  if (prec == 64) {
+    KF<double> k; load_kf(k, par, cov15, *chi2);
+    kf_update<double>(k, ym, zm_rel, (double)P.err_y2, (double)P.err_z2);
+    store_kf(k, par, cov15, chi2);
+  } else {
+    KF<float> k; load_kf(k, par, cov15, *chi2);
+    kf_update<float>(k, (float)ym, (float)zm_rel, P.err_y2, P.err_z2);
+    store_kf(k, par, cov15, chi2);
+  }
+}
+
+int orc_kf_fit(const void* params, int prec, int npt, const double* x, const double* y, const double* z, double* par,
+               double* cov15, double* chi2) {
+  const Params& P = *reinterpret_cast<const Params*>(params);
+  return prec == 64 ? kf_fit_entry<double>(P, npt, x, y, z, par, cov15, chi2)
+                    : kf_fit_entry<float>(P, npt, x, y, z, par, cov15, chi2);
+}
+
+}  // extern "C"
