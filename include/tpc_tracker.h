@@ -1,0 +1,222 @@
+/*
+ * tpc_tracker.h - C ABI of the B200-native TPC sector track finder.
+ *
+ * The operation: "Track Finding" of the ALICE Run 3 synchronous TPC chain (Table 1;
+ * PAPER.md:99, section 6: "the TPC tracking runs first standalone without such corrections"), on a
+ * whole time frame resident in GPU memory.  The paper names the step and defers
+ * the algorithm to references that are not available; the five stages (sort+bin, neighbours finder,
+ * link cleaner, Kalman tracklet constructor, selector) are those of BASELINE.json `north_star`, and
+ * every formula is the reading fixed in DESIGN.md section 3.
+ *
+ * Plain pointers and sizes only.  Every pointer below says HOST or DEVICE.  The library allocates no
+ * device memory: inputs, outputs and one workspace arena are the caller's (PyTorch tensors in this
+ * repository).  All work is enqueued on the caller's CUDA stream; unless stated, calls do not
+ * synchronise.  There is no CPU fallback: every stage runs in the library's sm_100a kernels.
+ *
+ * Error behaviour: functions return 0 (TPC_OK) or a negative tpc_error code; device-detected
+ * conditions (bad sector/row value, capacity overflow) are reported through the 32-bit status word
+ * (tpc_tracks_t.status, tpc_counters_t.status) as a bit set of TPC_STATUS_*; when a status bit is
+ * set the run is aborted on the device and n_tracks = 0 - outputs are never silently truncated.
+ */
+#ifndef TPC_TRACKER_H_
+#define TPC_TRACKER_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define TPC_API __attribute__((visibility("default")))
+#else
+#define TPC_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum tpc_error {
+  TPC_OK = 0,
+  TPC_ERR_INVALID_ARG = -1, /* null pointer, negative size, unsupported geometry (n_rows > 256, ...) */
+  TPC_ERR_CAPACITY = -2,    /* workspace too small for the requested capacities, n > max_clusters */
+  TPC_ERR_CUDA = -3         /* a CUDA runtime call or kernel launch failed (cudaGetLastError) */
+};
+
+enum tpc_status_bits {
+  TPC_STATUS_BAD_CLUSTER = 1,      /* a cluster had sector >= n_sectors or row >= n_rows */
+  TPC_STATUS_BINS_OVERFLOW = 2,    /* the (y,z) grids need more than max_bins bins (or > INT32_MAX) */
+  TPC_STATUS_SEEDS_OVERFLOW = 4,   /* more than max_seeds chain heads qualified as seeds */
+  TPC_STATUS_TRACKS_OVERFLOW = 8,  /* more than max_tracks tracks or max_track_clusters attached clusters */
+  TPC_STATUS_CHAIN_CYCLE = 16      /* internal consistency: a link chain longer than n_rows (cannot happen) */
+};
+
+typedef struct tpc_tracker tpc_tracker_t; /* opaque; owned by the library, freed by tpc_tracker_destroy */
+
+/*
+ * Geometry, field and cuts.  POD, copied at create.  The per-row derived
+ * tables (ymax_r, ny_r, link windows) are computed by the library on the host in fp32 from these
+ * values, each with the one expression stated in DESIGN.md section 3.0.
+ */
+typedef struct {
+  int32_t n_sectors;        /* <= 256 (sector ids are uint8); 36 for the ALICE TPC */
+  int32_t n_rows;           /* <= 256 (row ids are uint8); n_sectors*n_rows <= 65535; 152 */
+  const float* row_x;       /* HOST, n_rows values, strictly increasing, cm: pad-row radius x_r */
+  float tan_half_sector;    /* tan(10 deg) */
+  float bz_tesla;           /* solenoid field; curvature = -0.00299792458 * bz * (q/pT) [1/cm] */
+  float err_y2, err_z2;     /* cluster variances, cm^2 */
+  float cell_y, cell_z;     /* (y,z) grid cell, cm (> 0) */
+  float link_ay, link_az, link_b, link_T; /* S2 window slopes / offset and the link cut (section 3.2) */
+  int32_t min_chain_len;    /* S3: seeds are chains of at least this many clusters (>= 2) */
+  int32_t max_gap;          /* S4: rows without a cluster before a tracklet stops */
+  int32_t min_tracklet_hits;/* S4: tracklets with fewer hits are dropped */
+  int32_t min_track_hits;   /* S5: tracks must own at least this many clusters */
+  float pick_chi2_cut;      /* S4 pick-up gate */
+  float max_sinphi;         /* S4 propagation limit */
+  float y_margin;           /* S4 sector-exit margin, cm */
+  float init_c_ss, init_c_tt, init_c_qq; /* S4 initial variances of sin(phi), tan(lambda), q/pT */
+} tpc_params_t;
+
+/* Input clusters of one time frame, SoA.  DEVICE pointers for tpc_track_timeframe, HOST pointers
+ * (ideally pinned) for tpc_track_timeframe_host.  Read-only; must stay valid until the stream has
+ * finished the call.  `x` may be NULL and is not read: the tracker uses row_x[row] (pad-row centre).
+ * `z` is the pseudo-z in cm computed with vertex time 0 (continuous readout).
+ * Preconditions: coordinates finite; 0 <= n <= max_clusters; DEVICE arrays aligned like fresh
+ * allocations (sector to 4 bytes, z to 16 bytes - the kernels use vector loads), else INVALID_ARG. */
+typedef struct {
+  int64_t n;
+  const uint8_t* sector; /* [n] */
+  const uint8_t* row;    /* [n] */
+  const float* x;        /* [n] or NULL (unused) */
+  const float* y;        /* [n] sector-local y, cm */
+  const float* z;        /* [n] pseudo-z, cm */
+} tpc_clusters_t;
+
+/* Output tracks, SoA, caller-allocated with the stated capacities.  DEVICE pointers for
+ * tpc_track_timeframe, HOST pointers for tpc_track_timeframe_host.  Track ids are 0..n_tracks-1 in
+ * ascending order of the seed's sorted position (deterministic).
+ * par  : [5][max_tracks]  (y, z - z_ref, sin(phi), tan(lambda), q/pT) at x_ref; par[i*max_tracks + t]
+ * cov  : [15][max_tracks] lower triangle, row-major (c00,c10,c11,c20,...,c44); cov[m*max_tracks + t]
+ * trk_cl_start : [max_tracks+1] CSR offsets into trk_cl_idx
+ * trk_cl_idx   : [max_track_clusters] INPUT indices of the track's clusters, ascending row
+ * cluster_track: [clusters.n] track id of every input cluster, -1 if unassigned */
+typedef struct {
+  int64_t max_tracks;
+  int64_t max_track_clusters;
+  int32_t* n_tracks;      /* [1] */
+  int32_t* status;        /* [1] bit set of tpc_status_bits, 0 = fine */
+  int32_t* sector;        /* [max_tracks] */
+  int32_t* first_row;     /* [max_tracks] lowest owned row */
+  int32_t* last_row;      /* [max_tracks] highest owned row */
+  int32_t* n_clusters;    /* [max_tracks] owned clusters */
+  float* par;
+  float* cov;
+  float* x_ref;           /* [max_tracks] x of the plane the parameters are given at */
+  float* z_ref;           /* [max_tracks] z offset: absolute z = par[1] + z_ref */
+  float* chi2;            /* [max_tracks] */
+  int32_t* ndf;           /* [max_tracks] 2*n_hits(tracklet) - 5 */
+  int32_t* trk_cl_start;
+  int32_t* trk_cl_idx;
+  int32_t* cluster_track;
+} tpc_tracks_t;
+
+/* Small counter block read back by tpc_tracker_counters (sizes of the last run). */
+typedef struct {
+  int64_t n_clusters;
+  int64_t n_bins;        /* N_b: grid bins over all (sector,row) */
+  int64_t n_seeds;       /* K_s: chains that qualified as seeds */
+  int64_t n_tracklets;   /* K: tracklets kept by S4 */
+  int64_t n_tracks;      /* T_k */
+  int64_t n_track_clusters; /* clusters attached to tracks */
+  int64_t n_linked;      /* clusters with a cleaned up-link (chain edges) */
+  int64_t kf_steps;      /* S: Kalman propagate calls */
+  int64_t n_hits;        /* H: hits over all kept tracklets */
+  int32_t status;
+  int32_t reserved;
+} tpc_counters_t;
+
+/* Debug views into the workspace, valid until the next track call on the handle (DEVICE pointers).
+ * All positions are indices into the sorted order of S1. */
+enum tpc_stage_array {
+  TPC_VIEW_PERM = 0,        /* int32 [n]      sorted position -> input index (S1) */
+  TPC_VIEW_YS = 1,          /* float [n]      sorted y */
+  TPC_VIEW_ZS = 2,          /* float [n]      sorted z */
+  TPC_VIEW_SROW = 3,        /* uint16 [n]     sector*n_rows + row of the sorted cluster */
+  TPC_VIEW_BIN_START = 4,   /* int32 [n_bins+1] CSR over global bins */
+  TPC_VIEW_ROW_START = 5,   /* int32 [n_sectors*n_rows+1] */
+  TPC_VIEW_BIN_BASE = 6,    /* int32 [n_sectors*n_rows+1] first global bin of each (sector,row) */
+  TPC_VIEW_ZMIN = 7,        /* float [n_sectors] */
+  TPC_VIEW_ZMAX = 8,        /* float [n_sectors] */
+  TPC_VIEW_NZ = 9,          /* int32 [n_sectors] */
+  TPC_VIEW_LINK_UP_RAW = 10,/* int32 [n] (S2) */
+  TPC_VIEW_LINK_DN_RAW = 11,
+  TPC_VIEW_LINK_UP = 12,    /* int32 [n] cleaned (S3) */
+  TPC_VIEW_LINK_DN = 13,
+  TPC_VIEW_SEED_HEAD = 14,  /* int32 [n_seeds] */
+  TPC_VIEW_SEED_LEN = 15,   /* int32 [n_seeds] */
+  TPC_VIEW_T_HIT = 16,      /* int32 [n_seeds][n_rows] sorted position or -1 (S4) */
+  TPC_VIEW_T_FIRST_ROW = 17,/* int32 [n_seeds] */
+  TPC_VIEW_T_LAST_ROW = 18, /* int32 [n_seeds] */
+  TPC_VIEW_T_N_HITS = 19,   /* int32 [n_seeds] */
+  TPC_VIEW_T_PAR = 20,      /* float [n_seeds][5] */
+  TPC_VIEW_T_COV = 21,      /* float [n_seeds][15] */
+  TPC_VIEW_T_CHI2 = 22,     /* float [n_seeds] */
+  TPC_VIEW_T_ZREF = 23,     /* float [n_seeds] */
+  TPC_VIEW_TRACKLET_OF_SEED = 24, /* int32 [n_seeds] rank among kept tracklets or -1 (S5) */
+  TPC_VIEW_OWNED = 25,      /* int32 [n_seeds] clusters owned (S5) */
+  TPC_VIEW_COUNT_ = 26
+};
+
+typedef struct {
+  const void* ptr;     /* DEVICE */
+  int64_t n;           /* elements (synchronises the stream of the last call to read device counters) */
+  int32_t elem_bytes;
+  int32_t is_float;
+} tpc_stage_view_t;
+
+/* Bytes of DEVICE workspace the tracker needs for the given capacities.  `host_io` != 0 adds the
+ * staging buffers tpc_track_timeframe_host uses (inputs for max_clusters, outputs for max_tracks /
+ * max_track_clusters).  Returns 0 on invalid arguments. */
+TPC_API size_t tpc_tracker_workspace_bytes(const tpc_params_t* params, int64_t max_clusters, int64_t max_bins,
+                                   int64_t max_seeds, int64_t max_tracks, int64_t max_track_clusters,
+                                   int32_t host_io);
+
+/* Creates a tracker on the current CUDA device.  `d_workspace` (DEVICE, 256-byte aligned, at least
+ * workspace_bytes long) stays owned by the caller and must outlive the handle.  Uploads the derived
+ * tables (synchronous).  `host_io` as above. */
+TPC_API int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t max_bins, int64_t max_seeds,
+                       int64_t max_tracks, int64_t max_track_clusters, int32_t host_io, void* d_workspace,
+                       size_t workspace_bytes, tpc_tracker_t** out);
+
+/* Enqueues stages S1..S5 for one time frame on `cuda_stream` (a cudaStream_t; NULL = default
+ * stream).  DEVICE pointers in `in` and `out`.  Does not synchronise; counts and status stay on
+ * the device (out->n_tracks, out->status).  out->max_tracks / max_track_clusters must not exceed
+ * the capacities given at create. */
+TPC_API int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tracks_t* out, void* cuda_stream);
+
+/* Same from/to HOST buffers (tracker created with host_io != 0): copies the SoA input to the device,
+ * runs S1..S5, copies n_tracks, status, the track list, the CSR and cluster_track back, all on
+ * `cuda_stream`, then synchronises that stream.  Copy sizes of the outputs are bounded by the
+ * capacities; the per-track arrays are copied for the n_tracks tracks found. */
+TPC_API int tpc_track_timeframe_host(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tracks_t* out, void* cuda_stream);
+
+/* Synchronises the stream of the last call and reads the counter block (HOST out). */
+TPC_API int tpc_tracker_counters(tpc_tracker_t* t, tpc_counters_t* out);
+
+/* Per-stage device times of the next calls: when enabled, tpc_track_timeframe records CUDA events
+ * between the stages; tpc_tracker_stage_ms synchronises and returns ms for S1..S5 (HOST out[5]). */
+TPC_API int tpc_tracker_enable_stage_timing(tpc_tracker_t* t, int32_t enable);
+TPC_API int tpc_tracker_stage_ms(tpc_tracker_t* t, float* out_ms5);
+
+/* Debug view of one workspace array (enum tpc_stage_array).  Synchronises. */
+TPC_API int tpc_tracker_stage_view(tpc_tracker_t* t, int32_t which, tpc_stage_view_t* out);
+
+/* Number of kernel launches tpc_track_timeframe enqueues per call (for bench.py's gpu_launches). */
+TPC_API int tpc_tracker_launches_per_call(const tpc_tracker_t* t);
+
+TPC_API int tpc_tracker_destroy(tpc_tracker_t* t);
+
+TPC_API const char* tpc_error_string(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPC_TRACKER_H_ */

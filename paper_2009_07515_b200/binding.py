@@ -1,0 +1,304 @@
+"""ctypes binding of libtpc_tracker.so - same names as include/tpc_tracker.h, argument marshalling only.
+
+PyTorch supplies device memory and streams; every step of the path runs in the library's CUDA
+kernels.  There is NO CPU fallback: importing works without a GPU (so the ABI can be checked), but
+creating a tracker needs a CUDA device and a missing library raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+# ------------------------------------------------------------------ C structs (include/tpc_tracker.h)
+c_f32p = C.POINTER(C.c_float)
+
+
+class tpc_params_t(C.Structure):
+    _fields_ = [
+        ("n_sectors", C.c_int32), ("n_rows", C.c_int32), ("row_x", C.c_void_p),
+        ("tan_half_sector", C.c_float), ("bz_tesla", C.c_float), ("err_y2", C.c_float), ("err_z2", C.c_float),
+        ("cell_y", C.c_float), ("cell_z", C.c_float),
+        ("link_ay", C.c_float), ("link_az", C.c_float), ("link_b", C.c_float), ("link_T", C.c_float),
+        ("min_chain_len", C.c_int32), ("max_gap", C.c_int32), ("min_tracklet_hits", C.c_int32),
+        ("min_track_hits", C.c_int32),
+        ("pick_chi2_cut", C.c_float), ("max_sinphi", C.c_float), ("y_margin", C.c_float),
+        ("init_c_ss", C.c_float), ("init_c_tt", C.c_float), ("init_c_qq", C.c_float),
+    ]
+
+
+class tpc_clusters_t(C.Structure):
+    _fields_ = [("n", C.c_int64), ("sector", C.c_void_p), ("row", C.c_void_p), ("x", C.c_void_p), ("y", C.c_void_p),
+                ("z", C.c_void_p)]
+
+
+_TRACK_FIELDS = ["n_tracks", "status", "sector", "first_row", "last_row", "n_clusters", "par", "cov", "x_ref", "z_ref",
+                 "chi2", "ndf", "trk_cl_start", "trk_cl_idx", "cluster_track"]
+
+
+class tpc_tracks_t(C.Structure):
+    _fields_ = [("max_tracks", C.c_int64), ("max_track_clusters", C.c_int64)] + [(f, C.c_void_p) for f in _TRACK_FIELDS]
+
+
+class tpc_counters_t(C.Structure):
+    _fields_ = [("n_clusters", C.c_int64), ("n_bins", C.c_int64), ("n_seeds", C.c_int64), ("n_tracklets", C.c_int64),
+                ("n_tracks", C.c_int64), ("n_track_clusters", C.c_int64), ("n_linked", C.c_int64),
+                ("kf_steps", C.c_int64), ("n_hits", C.c_int64), ("status", C.c_int32), ("reserved", C.c_int32)]
+
+
+class tpc_stage_view_t(C.Structure):
+    _fields_ = [("ptr", C.c_void_p), ("n", C.c_int64), ("elem_bytes", C.c_int32), ("is_float", C.c_int32)]
+
+
+VIEWS = {name: i for i, name in enumerate([
+    "perm", "ys", "zs", "srow", "bin_start", "row_start", "bin_base", "zmin", "zmax", "nz",
+    "link_up_raw", "link_dn_raw", "link_up", "link_dn", "seed_head", "seed_len",
+    "t_hit", "t_first_row", "t_last_row", "t_n_hits", "t_par", "t_cov", "t_chi2", "t_zref",
+    "tracklet_of_seed", "k_owned"])}
+
+STATUS_BITS = {1: "BAD_CLUSTER", 2: "BINS_OVERFLOW", 4: "SEEDS_OVERFLOW", 8: "TRACKS_OVERFLOW", 16: "CHAIN_CYCLE"}
+
+EXPORTS = [
+    "tpc_tracker_workspace_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
+    "tpc_tracker_counters", "tpc_tracker_enable_stage_timing", "tpc_tracker_stage_ms", "tpc_tracker_stage_view",
+    "tpc_tracker_launches_per_call", "tpc_tracker_destroy", "tpc_error_string",
+]
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load_library(build: bool = True) -> C.CDLL:
+    """Loads (building first if stale and nvcc is there) libtpc_tracker.so.  Raises if unavailable."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if build:
+        try:
+            path = _build.build()
+        except Exception as e:  # nvcc missing on the box: use the shipped .so if it is there
+            if not os.path.exists(path):
+                raise RuntimeError(f"libtpc_tracker.so is missing and could not be built: {e}") from e
+    if not os.path.exists(path):
+        raise RuntimeError("libtpc_tracker.so is missing: run `python -m paper_2009_07515_b200.build` (no CPU fallback)")
+    lib = C.CDLL(path)
+    P = C.POINTER
+    lib.tpc_tracker_workspace_bytes.restype = C.c_size_t
+    lib.tpc_tracker_workspace_bytes.argtypes = [P(tpc_params_t), C.c_int64, C.c_int64, C.c_int64, C.c_int64, C.c_int64, C.c_int32]
+    lib.tpc_tracker_create.restype = C.c_int
+    lib.tpc_tracker_create.argtypes = [P(tpc_params_t), C.c_int64, C.c_int64, C.c_int64, C.c_int64, C.c_int64, C.c_int32,
+                                       C.c_void_p, C.c_size_t, P(C.c_void_p)]
+    for name in ("tpc_track_timeframe", "tpc_track_timeframe_host"):
+        f = getattr(lib, name)
+        f.restype = C.c_int
+        f.argtypes = [C.c_void_p, P(tpc_clusters_t), P(tpc_tracks_t), C.c_void_p]
+    lib.tpc_tracker_counters.restype = C.c_int
+    lib.tpc_tracker_counters.argtypes = [C.c_void_p, P(tpc_counters_t)]
+    lib.tpc_tracker_enable_stage_timing.restype = C.c_int
+    lib.tpc_tracker_enable_stage_timing.argtypes = [C.c_void_p, C.c_int32]
+    lib.tpc_tracker_stage_ms.restype = C.c_int
+    lib.tpc_tracker_stage_ms.argtypes = [C.c_void_p, P(C.c_float)]
+    lib.tpc_tracker_stage_view.restype = C.c_int
+    lib.tpc_tracker_stage_view.argtypes = [C.c_void_p, C.c_int32, P(tpc_stage_view_t)]
+    lib.tpc_tracker_launches_per_call.restype = C.c_int
+    lib.tpc_tracker_launches_per_call.argtypes = [C.c_void_p]
+    lib.tpc_tracker_destroy.restype = C.c_int
+    lib.tpc_tracker_destroy.argtypes = [C.c_void_p]
+    lib.tpc_error_string.restype = C.c_char_p
+    lib.tpc_error_string.argtypes = [C.c_int]
+    _lib = lib
+    return lib
+
+
+def _check(lib, rc: int, what: str):
+    if rc != 0:
+        raise RuntimeError(f"{what}: {lib.tpc_error_string(rc).decode()} ({rc})")
+
+
+def pack_params(params: dict):
+    """dict (tpc_synth.default_params) -> (tpc_params_t, keep-alive row_x array)."""
+    rx = np.ascontiguousarray(params["row_x"], dtype=np.float32)
+    p = tpc_params_t()
+    for name, _ in tpc_params_t._fields_:
+        if name == "row_x":
+            p.row_x = rx.ctypes.data
+        else:
+            v = params[name]
+            setattr(p, name, v.item() if hasattr(v, "item") else v)
+    return p, rx
+
+
+class Tracks:
+    """Output buffers (torch tensors on `device`, or pinned host tensors) laid out as tpc_tracks_t wants."""
+
+    def __init__(self, n_clusters: int, max_tracks: int, max_track_clusters: int, device):
+        host = torch.device(device).type == "cpu"
+        kw = dict(device=device, pin_memory=True) if host else dict(device=device)
+        i32 = lambda *s: torch.empty(*s, dtype=torch.int32, **kw)   # noqa: E731
+        f32 = lambda *s: torch.empty(*s, dtype=torch.float32, **kw)  # noqa: E731
+        self.max_tracks, self.max_track_clusters = int(max_tracks), int(max_track_clusters)
+        self.n_tracks = i32(1); self.status = i32(1)
+        self.sector = i32(max_tracks); self.first_row = i32(max_tracks); self.last_row = i32(max_tracks)
+        self.n_clusters = i32(max_tracks)
+        self.par = f32(5, max_tracks); self.cov = f32(15, max_tracks)
+        self.x_ref = f32(max_tracks); self.z_ref = f32(max_tracks); self.chi2 = f32(max_tracks); self.ndf = i32(max_tracks)
+        self.trk_cl_start = i32(max_tracks + 1); self.trk_cl_idx = i32(max_track_clusters)
+        self.cluster_track = i32(max(1, n_clusters))
+        self.n_in = int(n_clusters)
+
+    def struct(self) -> tpc_tracks_t:
+        s = tpc_tracks_t()
+        s.max_tracks = self.max_tracks; s.max_track_clusters = self.max_track_clusters
+        for f in _TRACK_FIELDS:
+            setattr(s, f, getattr(self, f).data_ptr())
+        return s
+
+    def bytes_out(self) -> int:
+        """Bytes a host run copies back for the tracks found (d2h_bytes_per_step)."""
+        T = int(self.n_tracks.item())
+        ntc = int(self.trk_cl_start[T].item()) if T else 0
+        return 8 + T * 4 * (8 + 5 + 15) + (T + 1) * 4 + ntc * 4 + self.n_in * 4
+
+    def numpy(self) -> dict:
+        """Host copies trimmed to the tracks found."""
+        T = int(self.n_tracks.item())
+        g = lambda t: t.detach().cpu().numpy()  # noqa: E731
+        st = g(self.trk_cl_start)[: T + 1].copy()
+        if T == 0:
+            st = np.zeros(1, np.int32)
+        return dict(
+            n_tracks=T, status=int(self.status.item()),
+            sector=g(self.sector)[:T].copy(), first_row=g(self.first_row)[:T].copy(), last_row=g(self.last_row)[:T].copy(),
+            n_clusters=g(self.n_clusters)[:T].copy(), par=g(self.par)[:, :T].T.copy(), cov=g(self.cov)[:, :T].T.copy(),
+            x_ref=g(self.x_ref)[:T].copy(), z_ref=g(self.z_ref)[:T].copy(), chi2=g(self.chi2)[:T].copy(),
+            ndf=g(self.ndf)[:T].copy(), trk_cl_start=st, trk_cl_idx=g(self.trk_cl_idx)[: int(st[-1])].copy(),
+            cluster_track=g(self.cluster_track)[: self.n_in].copy())
+
+
+class Tracker:
+    """tpc_tracker_create / tpc_track_timeframe / tpc_tracker_destroy with torch-owned memory."""
+
+    def __init__(self, params: dict, max_clusters: int, max_bins: int, max_seeds: int, max_tracks: int,
+                 max_track_clusters: int, host_io: bool = False, device="cuda:0"):
+        if not torch.cuda.is_available():
+            raise RuntimeError("tpc tracker needs a CUDA device: there is no CPU fallback")
+        self.lib = load_library()
+        self.device = torch.device(device)
+        self._p, self._rx = pack_params(params)
+        self.params = params
+        caps = [int(max_clusters), int(max_bins), int(max_seeds), int(max_tracks), int(max_track_clusters)]
+        self.caps = caps
+        nbytes = self.lib.tpc_tracker_workspace_bytes(C.byref(self._p), *caps, int(host_io))
+        if nbytes == 0:
+            raise ValueError("tpc_tracker_workspace_bytes rejected the parameters / capacities")
+        self.workspace_bytes = int(nbytes)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            h = C.c_void_p()
+            _check(self.lib, self.lib.tpc_tracker_create(C.byref(self._p), *caps, int(host_io), self.workspace.data_ptr(),
+                                                         nbytes, C.byref(h)), "tpc_tracker_create")
+        self._h = h
+
+    # -- lifetime
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self.lib.tpc_tracker_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    # -- calls
+    @staticmethod
+    def _clusters(sector, row, y, z) -> tpc_clusters_t:
+        c = tpc_clusters_t()
+        c.n = int(sector.shape[0])
+        c.sector = sector.data_ptr(); c.row = row.data_ptr(); c.x = None; c.y = y.data_ptr(); c.z = z.data_ptr()
+        return c
+
+    def new_tracks(self, n_clusters: int, host: bool = False) -> Tracks:
+        return Tracks(n_clusters, self.caps[3], self.caps[4], "cpu" if host else self.device)
+
+    def track_timeframe(self, sector, row, y, z, out: Tracks, stream=None):
+        """Device tensors in, device tensors out; enqueues on `stream` (default: torch's current stream)."""
+        for t in (sector, row, y, z):
+            assert t.is_cuda and t.is_contiguous()
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        c = self._clusters(sector, row, y, z)
+        s = out.struct()
+        _check(self.lib, self.lib.tpc_track_timeframe(self._h, C.byref(c), C.byref(s), C.c_void_p(st.cuda_stream)),
+               "tpc_track_timeframe")
+
+    def track_timeframe_host(self, sector, row, y, z, out: Tracks, stream=None):
+        """Pinned host tensors in/out; H2D, S1..S5 and D2H inside the call; synchronises."""
+        for t in (sector, row, y, z):
+            assert (not t.is_cuda) and t.is_contiguous()
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        c = self._clusters(sector, row, y, z)
+        s = out.struct()
+        _check(self.lib, self.lib.tpc_track_timeframe_host(self._h, C.byref(c), C.byref(s), C.c_void_p(st.cuda_stream)),
+               "tpc_track_timeframe_host")
+
+    def counters(self) -> dict:
+        k = tpc_counters_t()
+        _check(self.lib, self.lib.tpc_tracker_counters(self._h, C.byref(k)), "tpc_tracker_counters")
+        return {f: getattr(k, f) for f, _ in tpc_counters_t._fields_ if f != "reserved"}
+
+    def enable_stage_timing(self, on: bool = True):
+        _check(self.lib, self.lib.tpc_tracker_enable_stage_timing(self._h, int(on)), "tpc_tracker_enable_stage_timing")
+
+    def stage_ms(self) -> list[float]:
+        ms = (C.c_float * 5)()
+        _check(self.lib, self.lib.tpc_tracker_stage_ms(self._h, ms), "tpc_tracker_stage_ms")
+        return [float(v) for v in ms]
+
+    def launches_per_call(self) -> int:
+        return int(self.lib.tpc_tracker_launches_per_call(self._h))
+
+    def stage_view(self, name: str) -> np.ndarray:
+        """Host copy of one workspace array (debug / parity tests)."""
+        v = tpc_stage_view_t()
+        _check(self.lib, self.lib.tpc_tracker_stage_view(self._h, VIEWS[name], C.byref(v)), "tpc_tracker_stage_view")
+        dt = {(4, 0): np.int32, (4, 1): np.float32, (2, 0): np.uint16}[(v.elem_bytes, v.is_float)]
+        out = np.empty(v.n, dtype=dt)
+        if v.n:
+            # plain byte copy device -> host of a workspace slice
+            off = v.ptr - self.workspace.data_ptr()
+            src = self.workspace[off: off + v.n * v.elem_bytes]
+            out.view(np.uint8)[:] = src.cpu().numpy()
+        return out
+
+
+def max_bins_bound(sector, z, params: dict) -> int:
+    """Upper bound of N_b for sizing the workspace (host-side helper, numpy float64, +2 rows of slack per
+    sector; the tracker computes the exact grids itself on the device)."""
+    sector = np.asarray(sector); z = np.asarray(z, dtype=np.float64)
+    S = int(params["n_sectors"])
+    if sector.size == 0:
+        return 1
+    zmin = np.full(S, np.inf); zmax = np.full(S, -np.inf)
+    np.minimum.at(zmin, sector, z); np.maximum.at(zmax, sector, z)
+    span = np.where(np.isfinite(zmin), zmax - zmin, 0.0)
+    nz = np.where(np.isfinite(zmin), np.floor(span / float(params["cell_z"])) + 3, 0)
+    rx = np.asarray(params["row_x"], dtype=np.float64)
+    ny = np.floor(2.0 * rx * float(params["tan_half_sector"]) / float(params["cell_y"])) + 2
+    return int(nz.sum() * ny.sum()) + 1
+
+
+def suggest_capacities(n_clusters: int, params: dict) -> dict:
+    """Loose capacities for a workload of n clusters (host-side sizing helper, no tracker arithmetic):
+    seeds <= n / min_chain_len, tracks <= n / min_track_hits, attached clusters <= n."""
+    n = max(1, int(n_clusters))
+    return dict(max_clusters=n, max_seeds=max(1024, n // max(2, int(params["min_chain_len"])) + 1),
+                max_tracks=max(1024, n // max(1, int(params["min_track_hits"])) + 1), max_track_clusters=n)

@@ -1,0 +1,387 @@
+// C-ABI boundary of libtpc_tracker.so (include/tpc_tracker.h): argument checks, host-side derived
+// tables, workspace carving, stage orchestration on the caller's stream.  No device allocation.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/tpc_tracker.h"
+#include "tpc_internal.cuh"
+
+using namespace tpc;
+
+struct tpc_tracker {
+  tpc_params_t params;            // row_x pointer is NOT kept (copied into rowtab)
+  Ctx ctx;                        // pointers into the workspace; input fields set per call
+  int64_t max_clusters, max_bins, max_seeds, max_tracks, max_track_clusters;
+  int host_io;
+  // staging for the host variant (device)
+  uint8_t* st_sector; uint8_t* st_row; float* st_y; float* st_z;
+  OutPtrs st_out;
+  cudaStream_t last_stream;
+  bool timing;
+  cudaEvent_t ev[6];
+  int64_t last_n;
+};
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+// Walks the workspace layout; with base == nullptr only sizes it.
+struct Carver {
+  char* base; size_t off;
+  template <class T> T* take(size_t count) {
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += up(count * sizeof(T));
+    return p;
+  }
+};
+
+bool params_ok(const tpc_params_t* p) {
+  if (!p || !p->row_x) return false;
+  if (p->n_sectors < 1 || p->n_sectors > 256 || p->n_rows < 3 || p->n_rows > kMaxRows) return false;
+  if ((int64_t)p->n_sectors * p->n_rows > 65535) return false;
+  if (!(p->cell_y > 0.f) || !(p->cell_z > 0.f) || !(p->tan_half_sector > 0.f)) return false;
+  if (p->min_chain_len < 2 || p->max_gap < 0) return false;
+  for (int r = 0; r < p->n_rows; ++r) {
+    if (!(p->row_x[r] > 0.f)) return false;
+    if (r && !(p->row_x[r] > p->row_x[r - 1])) return false;
+  }
+  return true;
+}
+
+void layout(tpc_tracker* t, char* base, size_t* total) {
+  Carver cv{base, 0};
+  Ctx& c = t->ctx;
+  const size_t N = (size_t)t->max_clusters, NB = (size_t)t->max_bins, K = (size_t)t->max_seeds;
+  const int S = t->params.n_sectors, R = t->params.n_rows, SR = S * R;
+  c.cnt = cv.take<Counters>(1);
+  c.rowtab = cv.take<RowTab>(R);
+  c.zmin_key = cv.take<int>(S); c.zmax_key = cv.take<int>(S);
+  c.zmin = cv.take<float>(S); c.zmax = cv.take<float>(S); c.nz = cv.take<int>(S);
+  c.bin_base = cv.take<int>(SR + 1); c.row_start = cv.take<int>(SR + 1);
+  c.gbin = cv.take<int>(N); c.tmp_idx = cv.take<int>(N);
+  c.bins = cv.take<int>(NB + 2 + 8);
+  c.perm = cv.take<int>(N); c.ys = cv.take<float>(N); c.zs = cv.take<float>(N); c.srow = cv.take<uint16_t>(N);
+  size_t max_scan = N > NB + 2 ? N : NB + 2;
+  if (K > max_scan) max_scan = K;
+  c.tile_sums = cv.take<int>(max_scan / kScanTile + 2);
+  c.link_up_raw = cv.take<int>(N); c.link_dn_raw = cv.take<int>(N);
+  c.link_up = cv.take<int>(N); c.link_dn = cv.take<int>(N);
+  c.flag = cv.take<int>(N); c.flag_scan = cv.take<int>(N);
+  c.seed_head = cv.take<int>(K); c.seed_len = cv.take<int>(K);
+  c.t_hit = cv.take<int>(K * R);
+  c.t_first_row = cv.take<int>(K); c.t_last_row = cv.take<int>(K); c.t_n_hits = cv.take<int>(K);
+  c.t_par = cv.take<float>(K * 5); c.t_cov = cv.take<float>(K * 15); c.t_chi2 = cv.take<float>(K); c.t_zref = cv.take<float>(K);
+  c.kept_scan = cv.take<int>(K); c.tracklet_of_seed = cv.take<int>(K);
+  c.owner = cv.take<unsigned long long>(N);
+  c.k_owned = cv.take<int>(K); c.k_first = cv.take<int>(K); c.k_last = cv.take<int>(K);
+  c.surv_scan = cv.take<int>(K); c.owned_scan = cv.take<int>(K);
+  if (t->host_io) {
+    const size_t T = (size_t)t->max_tracks, TC = (size_t)t->max_track_clusters;
+    t->st_sector = cv.take<uint8_t>(N); t->st_row = cv.take<uint8_t>(N);
+    t->st_y = cv.take<float>(N); t->st_z = cv.take<float>(N);
+    OutPtrs& o = t->st_out;
+    o.n_tracks = cv.take<int>(1); o.status = cv.take<int>(1);
+    o.sector = cv.take<int>(T); o.first_row = cv.take<int>(T); o.last_row = cv.take<int>(T); o.n_clusters = cv.take<int>(T);
+    o.par = cv.take<float>(T * 5); o.cov = cv.take<float>(T * 15);
+    o.x_ref = cv.take<float>(T); o.z_ref = cv.take<float>(T); o.chi2 = cv.take<float>(T); o.ndf = cv.take<int>(T);
+    o.trk_cl_start = cv.take<int>(T + 1); o.trk_cl_idx = cv.take<int>(TC); o.cluster_track = cv.take<int>(N);
+    o.max_tracks = (int)T; o.max_track_clusters = (int)TC;
+  }
+  *total = cv.off;
+}
+
+bool caps_ok(int64_t max_clusters, int64_t max_bins, int64_t max_seeds, int64_t max_tracks, int64_t max_track_clusters) {
+  const int64_t lim = 2147483647LL - 16;
+  return max_clusters >= 1 && max_clusters <= lim && max_bins >= 1 && max_bins <= lim && max_seeds >= 1 &&
+         max_seeds <= lim && max_tracks >= 1 && max_tracks <= lim && max_track_clusters >= 1 && max_track_clusters <= lim;
+}
+
+void fill_ctx_constants(tpc_tracker* t, std::vector<RowTab>& tab) {
+  const tpc_params_t& p = t->params;
+  Ctx& c = t->ctx;
+  const int R = p.n_rows;
+  c.S = p.n_sectors; c.R = R; c.SR = p.n_sectors * R;
+  // each a single fp32 expression, DESIGN.md section 3.0
+  c.kb = -0.00299792458f * p.bz_tesla;
+  c.inv_cy = 1.0f / p.cell_y;
+  c.inv_cz = 1.0f / p.cell_z;
+  c.err_y2 = p.err_y2; c.err_z2 = p.err_z2; c.link_T = p.link_T;
+  c.min_chain_len = p.min_chain_len; c.max_gap = p.max_gap;
+  c.min_tracklet_hits = p.min_tracklet_hits; c.min_track_hits = p.min_track_hits;
+  c.pick_chi2_cut = p.pick_chi2_cut; c.max_sinphi = p.max_sinphi; c.y_margin = p.y_margin;
+  c.init_c_ss = p.init_c_ss; c.init_c_tt = p.init_c_tt; c.init_c_qq = p.init_c_qq;
+  tab.assign(R, RowTab{});
+  int acc = 0;
+  for (int r = 0; r < R; ++r) {
+    RowTab& e = tab[r];
+    e.x = p.row_x[r];
+    e.ymax = p.row_x[r] * p.tan_half_sector;
+    e.ny = (int)std::floor((2.0f * e.ymax) * c.inv_cy) + 1;
+    e.ny_prefix = acc;
+    acc += e.ny;
+    for (int k = 1; k <= 2; ++k) {
+      if (r + k < R) {
+        const float dx = p.row_x[r + k] - p.row_x[r];
+        e.up_dx[k - 1] = dx;
+        e.up_ratio[k - 1] = p.row_x[r + k] / p.row_x[r];
+        e.up_wy[k - 1] = p.link_ay * dx + p.link_b;
+        e.up_wz[k - 1] = p.link_az * dx + p.link_b;
+      }
+      if (r - k >= 0) {
+        const float dx = p.row_x[r] - p.row_x[r - k];
+        e.dn_dx[k - 1] = dx;
+        e.dn_ratio[k - 1] = p.row_x[r - k] / p.row_x[r];
+        e.dn_wy[k - 1] = p.link_ay * dx + p.link_b;
+        e.dn_wz[k - 1] = p.link_az * dx + p.link_b;
+      }
+    }
+  }
+  c.ny_total = acc;
+}
+
+bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+int run_device(tpc_tracker* t, const tpc_clusters_t* in, const OutPtrs& o, cudaStream_t st) {
+  Ctx& c = t->ctx;
+  c.n = (int)in->n;
+  c.in_sector = in->sector; c.in_row = in->row; c.in_y = in->y; c.in_z = in->z;
+  t->last_stream = st;
+  t->last_n = in->n;
+  const bool tm = t->timing;
+  if (tm) cudaEventRecord(t->ev[0], st);
+  if (launch_reset(c, st)) return TPC_ERR_CUDA;
+  if (launch_s1(c, st)) return TPC_ERR_CUDA;
+  if (tm) cudaEventRecord(t->ev[1], st);
+  if (launch_s2(c, st)) return TPC_ERR_CUDA;
+  if (tm) cudaEventRecord(t->ev[2], st);
+  if (launch_s3(c, st)) return TPC_ERR_CUDA;
+  if (tm) cudaEventRecord(t->ev[3], st);
+  if (launch_s4(c, st)) return TPC_ERR_CUDA;
+  if (tm) cudaEventRecord(t->ev[4], st);
+  if (launch_s5(c, o, st)) return TPC_ERR_CUDA;
+  if (tm) cudaEventRecord(t->ev[5], st);
+  return cudaGetLastError() == cudaSuccess ? TPC_OK : TPC_ERR_CUDA;
+}
+
+bool out_ok(const tpc_tracks_t* o) {
+  return o && o->n_tracks && o->status && o->sector && o->first_row && o->last_row && o->n_clusters && o->par && o->cov &&
+         o->x_ref && o->z_ref && o->chi2 && o->ndf && o->trk_cl_start && o->trk_cl_idx && o->cluster_track &&
+         o->max_tracks >= 1 && o->max_track_clusters >= 1;
+}
+
+OutPtrs to_out(const tpc_tracks_t* o) {
+  OutPtrs r;
+  r.n_tracks = o->n_tracks; r.status = o->status; r.sector = o->sector; r.first_row = o->first_row;
+  r.last_row = o->last_row; r.n_clusters = o->n_clusters; r.par = o->par; r.cov = o->cov; r.x_ref = o->x_ref;
+  r.z_ref = o->z_ref; r.chi2 = o->chi2; r.ndf = o->ndf; r.trk_cl_start = o->trk_cl_start; r.trk_cl_idx = o->trk_cl_idx;
+  r.cluster_track = o->cluster_track; r.max_tracks = (int)o->max_tracks; r.max_track_clusters = (int)o->max_track_clusters;
+  return r;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t tpc_tracker_workspace_bytes(const tpc_params_t* params, int64_t max_clusters, int64_t max_bins, int64_t max_seeds,
+                                   int64_t max_tracks, int64_t max_track_clusters, int32_t host_io) {
+  if (!params_ok(params) || !caps_ok(max_clusters, max_bins, max_seeds, max_tracks, max_track_clusters)) return 0;
+  tpc_tracker tmp{};
+  tmp.params = *params;
+  tmp.max_clusters = max_clusters; tmp.max_bins = max_bins; tmp.max_seeds = max_seeds;
+  tmp.max_tracks = max_tracks; tmp.max_track_clusters = max_track_clusters; tmp.host_io = host_io;
+  size_t total = 0;
+  layout(&tmp, nullptr, &total);
+  return total;
+}
+
+int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t max_bins, int64_t max_seeds,
+                       int64_t max_tracks, int64_t max_track_clusters, int32_t host_io, void* d_workspace,
+                       size_t workspace_bytes, tpc_tracker_t** out) {
+  if (!out) return TPC_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!params_ok(params) || !caps_ok(max_clusters, max_bins, max_seeds, max_tracks, max_track_clusters)) return TPC_ERR_INVALID_ARG;
+  if (!d_workspace || !aligned(d_workspace, kAlign)) return TPC_ERR_INVALID_ARG;
+  tpc_tracker* t = new (std::nothrow) tpc_tracker{};
+  if (!t) return TPC_ERR_INVALID_ARG;
+  t->params = *params;
+  t->max_clusters = max_clusters; t->max_bins = max_bins; t->max_seeds = max_seeds;
+  t->max_tracks = max_tracks; t->max_track_clusters = max_track_clusters; t->host_io = host_io;
+  size_t total = 0;
+  layout(t, static_cast<char*>(d_workspace), &total);
+  if (total > workspace_bytes) { delete t; return TPC_ERR_CAPACITY; }
+  std::vector<RowTab> tab;
+  fill_ctx_constants(t, tab);
+  t->params.row_x = nullptr;
+  Ctx& c = t->ctx;
+  c.max_clusters = (int)max_clusters; c.max_bins = (int)max_bins; c.max_seeds = (int)max_seeds;
+  c.max_tracks = (int)max_tracks; c.max_track_clusters = (int)max_track_clusters;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+    delete t; return TPC_ERR_CUDA;
+  }
+  c.n_sms = sms;
+  if (cudaMemcpy(const_cast<RowTab*>(c.rowtab), tab.data(), tab.size() * sizeof(RowTab), cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemset(c.cnt, 0, sizeof(Counters)) != cudaSuccess) {
+    delete t; return TPC_ERR_CUDA;
+  }
+  for (auto& e : t->ev)
+    if (cudaEventCreate(&e) != cudaSuccess) { delete t; return TPC_ERR_CUDA; }
+  *out = t;
+  return TPC_OK;
+}
+
+int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tracks_t* out, void* cuda_stream) {
+  if (!t || !in || !out_ok(out)) return TPC_ERR_INVALID_ARG;
+  if (in->n < 0 || (in->n > 0 && (!in->sector || !in->row || !in->y || !in->z))) return TPC_ERR_INVALID_ARG;
+  if (in->n > t->max_clusters || out->max_tracks > t->max_tracks || out->max_track_clusters > t->max_track_clusters)
+    return TPC_ERR_CAPACITY;
+  if (!aligned(in->sector, 4) || !aligned(in->z, 16) || !aligned(in->y, 4)) return TPC_ERR_INVALID_ARG;
+  return run_device(t, in, to_out(out), static_cast<cudaStream_t>(cuda_stream));
+}
+
+int tpc_track_timeframe_host(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tracks_t* out, void* cuda_stream) {
+  if (!t || !in || !out_ok(out) || !t->host_io) return TPC_ERR_INVALID_ARG;
+  if (in->n < 0 || (in->n > 0 && (!in->sector || !in->row || !in->y || !in->z))) return TPC_ERR_INVALID_ARG;
+  if (in->n > t->max_clusters || out->max_tracks > t->max_tracks || out->max_track_clusters > t->max_track_clusters)
+    return TPC_ERR_CAPACITY;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const size_t n = (size_t)in->n;
+  tpc_clusters_t d = *in;
+  d.sector = t->st_sector; d.row = t->st_row; d.y = t->st_y; d.z = t->st_z; d.x = nullptr;
+  if (n) {
+    if (cudaMemcpyAsync(t->st_sector, in->sector, n, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(t->st_row, in->row, n, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(t->st_y, in->y, n * 4, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(t->st_z, in->z, n * 4, cudaMemcpyHostToDevice, st) != cudaSuccess)
+      return TPC_ERR_CUDA;
+  }
+  OutPtrs o = t->st_out;
+  o.max_tracks = (int)out->max_tracks; o.max_track_clusters = (int)out->max_track_clusters;
+  const int rc = run_device(t, &d, o, st);
+  if (rc != TPC_OK) return rc;
+  // counts first, then exactly the tracks found
+  int head[2] = {0, 0};
+  if (cudaMemcpyAsync(&head[0], o.n_tracks, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+      cudaMemcpyAsync(&head[1], o.status, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+      cudaStreamSynchronize(st) != cudaSuccess)
+    return TPC_ERR_CUDA;
+  *out->n_tracks = head[0]; *out->status = head[1];
+  const size_t T = (size_t)head[0], mt = (size_t)out->max_tracks;
+  auto d2h = [&](void* dst, const void* src, size_t bytes) {
+    return bytes == 0 || cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  };
+  bool ok = true;
+  int n_tc = 0;
+  if (T) {
+    ok = ok && d2h(out->sector, o.sector, T * 4) && d2h(out->first_row, o.first_row, T * 4) &&
+         d2h(out->last_row, o.last_row, T * 4) && d2h(out->n_clusters, o.n_clusters, T * 4) &&
+         d2h(out->x_ref, o.x_ref, T * 4) && d2h(out->z_ref, o.z_ref, T * 4) && d2h(out->chi2, o.chi2, T * 4) &&
+         d2h(out->ndf, o.ndf, T * 4) && d2h(out->trk_cl_start, o.trk_cl_start, (T + 1) * 4);
+    for (int i = 0; i < 5 && ok; ++i) ok = d2h(out->par + i * mt, o.par + i * mt, T * 4);
+    for (int i = 0; i < 15 && ok; ++i) ok = d2h(out->cov + i * mt, o.cov + i * mt, T * 4);
+    ok = ok && d2h(&n_tc, &t->ctx.cnt->n_track_clusters, 4) && cudaStreamSynchronize(st) == cudaSuccess;
+    ok = ok && d2h(out->trk_cl_idx, o.trk_cl_idx, (size_t)n_tc * 4);
+  } else {
+    out->trk_cl_start[0] = 0;
+  }
+  ok = ok && d2h(out->cluster_track, o.cluster_track, n * 4);
+  if (!ok || cudaStreamSynchronize(st) != cudaSuccess) return TPC_ERR_CUDA;
+  return TPC_OK;
+}
+
+int tpc_tracker_counters(tpc_tracker_t* t, tpc_counters_t* out) {
+  if (!t || !out) return TPC_ERR_INVALID_ARG;
+  Counters k;
+  if (cudaStreamSynchronize(t->last_stream) != cudaSuccess ||
+      cudaMemcpy(&k, t->ctx.cnt, sizeof(k), cudaMemcpyDeviceToHost) != cudaSuccess)
+    return TPC_ERR_CUDA;
+  out->n_clusters = t->last_n; out->n_bins = k.n_bins; out->n_seeds = k.n_seeds; out->n_tracklets = k.n_tracklets;
+  out->n_tracks = k.n_tracks; out->n_track_clusters = k.n_track_clusters; out->n_linked = k.n_linked;
+  out->kf_steps = (int64_t)k.kf_steps; out->n_hits = (int64_t)k.n_hits; out->status = k.status; out->reserved = 0;
+  return TPC_OK;
+}
+
+int tpc_tracker_enable_stage_timing(tpc_tracker_t* t, int32_t enable) {
+  if (!t) return TPC_ERR_INVALID_ARG;
+  t->timing = enable != 0;
+  return TPC_OK;
+}
+
+int tpc_tracker_stage_ms(tpc_tracker_t* t, float* out_ms5) {
+  if (!t || !out_ms5 || !t->timing) return TPC_ERR_INVALID_ARG;
+  if (cudaEventSynchronize(t->ev[5]) != cudaSuccess) return TPC_ERR_CUDA;
+  for (int i = 0; i < 5; ++i)
+    if (cudaEventElapsedTime(&out_ms5[i], t->ev[i], t->ev[i + 1]) != cudaSuccess) return TPC_ERR_CUDA;
+  return TPC_OK;
+}
+
+int tpc_tracker_stage_view(tpc_tracker_t* t, int32_t which, tpc_stage_view_t* out) {
+  if (!t || !out || which < 0 || which >= TPC_VIEW_COUNT_) return TPC_ERR_INVALID_ARG;
+  Counters k;
+  if (cudaStreamSynchronize(t->last_stream) != cudaSuccess ||
+      cudaMemcpy(&k, t->ctx.cnt, sizeof(k), cudaMemcpyDeviceToHost) != cudaSuccess)
+    return TPC_ERR_CUDA;
+  const Ctx& c = t->ctx;
+  const int64_t n = t->last_n, ns = k.n_seeds, SR1 = c.SR + 1;
+  auto set = [&](const void* p, int64_t cnt, int eb, int fl) { out->ptr = p; out->n = cnt; out->elem_bytes = eb; out->is_float = fl; };
+  switch (which) {
+    case TPC_VIEW_PERM: set(c.perm, n, 4, 0); break;
+    case TPC_VIEW_YS: set(c.ys, n, 4, 1); break;
+    case TPC_VIEW_ZS: set(c.zs, n, 4, 1); break;
+    case TPC_VIEW_SROW: set(c.srow, n, 2, 0); break;
+    case TPC_VIEW_BIN_START: set(c.bins, (int64_t)k.n_bins + 1, 4, 0); break;
+    case TPC_VIEW_ROW_START: set(c.row_start, SR1, 4, 0); break;
+    case TPC_VIEW_BIN_BASE: set(c.bin_base, SR1, 4, 0); break;
+    case TPC_VIEW_ZMIN: set(c.zmin, c.S, 4, 1); break;
+    case TPC_VIEW_ZMAX: set(c.zmax, c.S, 4, 1); break;
+    case TPC_VIEW_NZ: set(c.nz, c.S, 4, 0); break;
+    case TPC_VIEW_LINK_UP_RAW: set(c.link_up_raw, n, 4, 0); break;
+    case TPC_VIEW_LINK_DN_RAW: set(c.link_dn_raw, n, 4, 0); break;
+    case TPC_VIEW_LINK_UP: set(c.link_up, n, 4, 0); break;
+    case TPC_VIEW_LINK_DN: set(c.link_dn, n, 4, 0); break;
+    case TPC_VIEW_SEED_HEAD: set(c.seed_head, ns, 4, 0); break;
+    case TPC_VIEW_SEED_LEN: set(c.seed_len, ns, 4, 0); break;
+    case TPC_VIEW_T_HIT: set(c.t_hit, ns * c.R, 4, 0); break;
+    case TPC_VIEW_T_FIRST_ROW: set(c.t_first_row, ns, 4, 0); break;
+    case TPC_VIEW_T_LAST_ROW: set(c.t_last_row, ns, 4, 0); break;
+    case TPC_VIEW_T_N_HITS: set(c.t_n_hits, ns, 4, 0); break;
+    case TPC_VIEW_T_PAR: set(c.t_par, ns * 5, 4, 1); break;
+    case TPC_VIEW_T_COV: set(c.t_cov, ns * 15, 4, 1); break;
+    case TPC_VIEW_T_CHI2: set(c.t_chi2, ns, 4, 1); break;
+    case TPC_VIEW_T_ZREF: set(c.t_zref, ns, 4, 1); break;
+    case TPC_VIEW_TRACKLET_OF_SEED: set(c.tracklet_of_seed, ns, 4, 0); break;
+    case TPC_VIEW_OWNED: set(c.k_owned, ns, 4, 0); break;
+    default: return TPC_ERR_INVALID_ARG;
+  }
+  return TPC_OK;
+}
+
+int tpc_tracker_launches_per_call(const tpc_tracker_t* t) {
+  if (!t) return TPC_ERR_INVALID_ARG;
+  return launches_reset() + launches_s1() + launches_s2() + launches_s3() + launches_s4() + launches_s5();
+}
+
+int tpc_tracker_destroy(tpc_tracker_t* t) {
+  if (!t) return TPC_ERR_INVALID_ARG;
+  for (auto& e : t->ev)
+    if (e) cudaEventDestroy(e);
+  delete t;
+  return TPC_OK;
+}
+
+const char* tpc_error_string(int code) {
+  switch (code) {
+    case TPC_OK: return "ok";
+    case TPC_ERR_INVALID_ARG: return "invalid argument";
+    case TPC_ERR_CAPACITY: return "capacity exceeded";
+    case TPC_ERR_CUDA: return "CUDA error";
+    default: return "unknown error";
+  }
+}
+
+}  // extern "C"

@@ -1,0 +1,116 @@
+// S2 - neighbours finder (BASELINE.json north_star (2)): for every cluster of row
+// r the best (up, down) link pair in rows r+-1 (widening to r+-2) by minimal straight-line deviation
+// inside a search window.  One thread per sorted position; consecutive positions are neighbours in
+// (z, y) of the same row, so a warp's rectangle queries hit the same few cache lines of the rows
+// above and below.  The per-row tables sit in shared memory.  Division-free, no candidate cap:
+// up to kCap candidates per side are kept in registers/local memory, beyond that the thread
+// re-walks the rectangles (same visiting order, same result).
+#include "tpc_internal.cuh"
+
+namespace tpc {
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kCap = 8;
+
+struct Cand {
+  int pos[kCap];
+  float y[kCap], z[kCap];
+  int n;
+};
+
+__device__ __forceinline__ RowGrid make_grid(const Ctx& c, const RowTab* tab, int s, int t) {
+  RowGrid g;
+  g.b0 = __ldg(c.bin_base + s * c.R + t);
+  g.ny = tab[t].ny;
+  g.nz = __ldg(c.nz + s);
+  g.ymax = tab[t].ymax;
+  g.zmin = __ldg(c.zmin + s);
+  return g;
+}
+
+__global__ void __launch_bounds__(kThreads) k_neighbours(Ctx c) {
+  extern __shared__ RowTab tab[];
+  for (int i = threadIdx.x; i < c.R * (int)(sizeof(RowTab) / 4); i += blockDim.x)
+    reinterpret_cast<int*>(tab)[i] = __ldg(reinterpret_cast<const int*>(c.rowtab) + i);
+  __syncthreads();
+  if (c.cnt->status) return;
+  const float* __restrict__ ys = c.ys;
+  const float* __restrict__ zs = c.zs;
+  const int* __restrict__ bin_start = c.bins;
+  const long long n = c.n;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const int sr = c.srow[i];
+    const int s = sr / c.R, r = sr - s * c.R;
+    const float y = ys[i], z = zs[i];
+    int lu = -1, ld = -1;
+
+    Cand U, D;
+    U.n = 0; D.n = 0;
+    int ku = 0, kd = 0;
+    float uylo = 0, uyhi = 0, uzlo = 0, uzhi = 0, dylo = 0, dyhi = 0, dzlo = 0, dzhi = 0;
+    RowGrid gu = {}, gd = {};
+    for (int k = 1; k <= 2 && U.n == 0; ++k) {
+      if (r + k >= c.R) break;
+      const float yc = y * tab[r].up_ratio[k - 1], wy = tab[r].up_wy[k - 1], wz = tab[r].up_wz[k - 1];
+      uylo = yc - wy; uyhi = yc + wy; uzlo = z - wz; uzhi = z + wz;
+      gu = make_grid(c, tab, s, r + k);
+      for_each_in_rect(gu, c.inv_cy, c.inv_cz, bin_start, ys, zs, uylo, uyhi, uzlo, uzhi, [&](int j, float yj, float zj) {
+        if (U.n < kCap) { U.pos[U.n] = j; U.y[U.n] = yj; U.z[U.n] = zj; }
+        ++U.n;
+      });
+      ku = k;
+    }
+    if (U.n > 0) {
+      for (int k = 1; k <= 2 && D.n == 0; ++k) {
+        if (r - k < 0) break;
+        const float yc = y * tab[r].dn_ratio[k - 1], wy = tab[r].dn_wy[k - 1], wz = tab[r].dn_wz[k - 1];
+        dylo = yc - wy; dyhi = yc + wy; dzlo = z - wz; dzhi = z + wz;
+        gd = make_grid(c, tab, s, r - k);
+        for_each_in_rect(gd, c.inv_cy, c.inv_cz, bin_start, ys, zs, dylo, dyhi, dzlo, dzhi, [&](int j, float yj, float zj) {
+          if (D.n < kCap) { D.pos[D.n] = j; D.y[D.n] = yj; D.z[D.n] = zj; }
+          ++D.n;
+        });
+        kd = k;
+      }
+    }
+    if (U.n > 0 && D.n > 0) {
+      const float dxu = tab[r].up_dx[ku - 1], dxd = tab[r].dn_dx[kd - 1];
+      const float cut = c.link_T * ((dxu * dxd) * (dxu * dxd));
+      float best = INFINITY;
+      int bu = -1, bd = -1;
+      auto score = [&](int u, float yu, float zu, int d, float yd, float zd) {
+        const float Dy = dxd * (yu - y) - dxu * (y - yd);
+        const float Dz = dxd * (zu - z) - dxu * (z - zd);
+        const float Dv = Dy * Dy + Dz * Dz;
+        if (Dv < best) { best = Dv; bu = u; bd = d; }
+      };
+      if (U.n <= kCap && D.n <= kCap) {
+        for (int a = 0; a < U.n; ++a)
+          for (int b = 0; b < D.n; ++b) score(U.pos[a], U.y[a], U.z[a], D.pos[b], D.y[b], D.z[b]);
+      } else {   // rare: crowded window, walk the rectangles again
+        for_each_in_rect(gu, c.inv_cy, c.inv_cz, bin_start, ys, zs, uylo, uyhi, uzlo, uzhi, [&](int u, float yu, float zu) {
+          for_each_in_rect(gd, c.inv_cy, c.inv_cz, bin_start, ys, zs, dylo, dyhi, dzlo, dzhi,
+                           [&](int d, float yd, float zd) { score(u, yu, zu, d, yd, zd); });
+        });
+      }
+      if (best <= cut) { lu = bu; ld = bd; }
+    }
+    c.link_up_raw[i] = lu;
+    c.link_dn_raw[i] = ld;
+  }
+}
+
+}  // namespace
+
+int launches_s2() { return 1; }
+int launch_s2(const Ctx& c, cudaStream_t st) {
+  long long g = ((long long)c.n + kThreads - 1) / kThreads;
+  const long long cap = (long long)c.n_sms * 32;
+  if (g > cap) g = cap;
+  if (g < 1) g = 1;
+  k_neighbours<<<(unsigned)g, kThreads, c.R * sizeof(RowTab), st>>>(c);
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+}  // namespace tpc

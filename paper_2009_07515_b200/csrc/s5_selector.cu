@@ -1,0 +1,171 @@
+// S5 - track selector (BASELINE.json north_star (5)): deduplicates tracklets by shared
+// clusters.  Every cluster goes to the tracklet with the largest key = (n_hits << 32 | ~tracklet id)
+// among those holding it (u64 atomicMax); a tracklet survives if it still owns min_track_hits
+// clusters.  Tracklet ids, track ids and the CSR offsets are ranks from scans (deterministic).
+//   k_kept       kept flag per seed                      -> scan -> tracklet ids, n_tracklets
+//   k_owner      owner[cluster] = max key                 (one warp per tracklet, coalesced hit rows)
+//   k_owned      owned count, first/last owned row        -> scans -> track ids, CSR starts
+//   k_finalize   capacity checks, n_tracks
+//   k_write      tracks SoA, trk_cl_idx (input indices, ascending row), cluster_track
+#include "tpc_internal.cuh"
+#include "../../include/tpc_tracker.h"
+
+namespace tpc {
+namespace {
+
+constexpr int kThreads = 256;
+
+__device__ __forceinline__ unsigned long long make_key(int n_hits, int tracklet_id) {
+  return ((unsigned long long)(unsigned)n_hits << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)tracklet_id);
+}
+
+__global__ void __launch_bounds__(kThreads) k_init_out(Ctx c, OutPtrs o) {
+  // owner = 0, cluster_track = -1 (vectorised where aligned; n is host-known)
+  const long long n = c.n;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    c.owner[i] = 0ull;
+    o.cluster_track[i] = -1;
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_kept(Ctx c) {
+  if (c.cnt->status) return;
+  const int ns = c.cnt->n_seeds;
+  for (int sd = blockIdx.x * blockDim.x + threadIdx.x; sd < ns; sd += gridDim.x * blockDim.x)
+    c.kept_scan[sd] = c.t_n_hits[sd] >= c.min_tracklet_hits;
+}
+
+__global__ void __launch_bounds__(kThreads) k_owner(Ctx c) {
+  if (c.cnt->status) return;
+  const int ns = c.cnt->n_seeds, R = c.R;
+  const int lane = threadIdx.x & 31;
+  const int warps = (gridDim.x * blockDim.x) >> 5;
+  for (int sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < ns; sd += warps) {
+    const int inc = c.kept_scan[sd], prev = sd ? c.kept_scan[sd - 1] : 0;
+    const bool kept = inc != prev;
+    if (lane == 0) c.tracklet_of_seed[sd] = kept ? inc - 1 : -1;
+    if (!kept) continue;
+    const unsigned long long key = make_key(c.t_n_hits[sd], inc - 1);
+    const int* hit = c.t_hit + (size_t)sd * R;
+    for (int r = lane; r < R; r += 32) {
+      const int cl = hit[r];
+      if (cl >= 0) atomicMax(c.owner + cl, key);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_owned(Ctx c) {
+  if (c.cnt->status) return;
+  const int ns = c.cnt->n_seeds, R = c.R;
+  const int lane = threadIdx.x & 31;
+  const int warps = (gridDim.x * blockDim.x) >> 5;
+  for (int sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < ns; sd += warps) {
+    const int tid = c.tracklet_of_seed[sd];
+    int owned = 0, first = 0x7FFFFFFF, last = -1;
+    if (tid >= 0) {
+      const unsigned long long key = make_key(c.t_n_hits[sd], tid);
+      const int* hit = c.t_hit + (size_t)sd * R;
+      for (int r = lane; r < R; r += 32) {
+        const int cl = hit[r];
+        if (cl >= 0 && c.owner[cl] == key) { ++owned; first = min(first, r); last = max(last, r); }
+      }
+    }
+    for (int o = 16; o; o >>= 1) {
+      owned += __shfl_xor_sync(0xffffffffu, owned, o);
+      first = min(first, __shfl_xor_sync(0xffffffffu, first, o));
+      last = max(last, __shfl_xor_sync(0xffffffffu, last, o));
+    }
+    if (lane == 0) {
+      const bool surv = tid >= 0 && owned >= c.min_track_hits;
+      c.k_owned[sd] = owned; c.k_first[sd] = first; c.k_last[sd] = last;
+      c.surv_scan[sd] = surv;
+      c.owned_scan[sd] = surv ? owned : 0;
+    }
+  }
+}
+
+__global__ void k_finalize(Ctx c, OutPtrs o) {
+  Counters& k = *c.cnt;
+  if (!k.status && (k.n_tracks > o.max_tracks || k.n_track_clusters > o.max_track_clusters))
+    k.status |= TPC_STATUS_TRACKS_OVERFLOW;
+  if (k.status) { k.n_tracks = 0; k.n_track_clusters = 0; k.n_tracklets = 0; }
+  *o.n_tracks = k.n_tracks;
+  *o.status = k.status;
+  if (k.status) o.trk_cl_start[0] = 0;
+}
+
+__global__ void __launch_bounds__(kThreads) k_write(Ctx c, OutPtrs o) {
+  if (c.cnt->status) return;
+  const int ns = c.cnt->n_seeds, R = c.R;
+  const int lane = threadIdx.x & 31;
+  const int warps = (gridDim.x * blockDim.x) >> 5;
+  const size_t mt = (size_t)o.max_tracks;
+  if (blockIdx.x == 0 && threadIdx.x == 0) o.trk_cl_start[0] = 0;
+  for (int sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < ns; sd += warps) {
+    const int inc = c.surv_scan[sd], prev = sd ? c.surv_scan[sd - 1] : 0;
+    if (inc == prev) continue;
+    const int id = inc - 1;
+    const int end = c.owned_scan[sd];
+    int off = end - c.k_owned[sd];
+    const unsigned long long key = make_key(c.t_n_hits[sd], c.tracklet_of_seed[sd]);
+    const int* hit = c.t_hit + (size_t)sd * R;
+    for (int rb = 0; rb < R; rb += 32) {
+      const int r = rb + lane;
+      int cl = -1;
+      if (r < R) {
+        cl = hit[r];
+        if (cl >= 0 && c.owner[cl] != key) cl = -1;
+      }
+      const unsigned m = __ballot_sync(0xffffffffu, cl >= 0);
+      if (cl >= 0) {
+        const int in_idx = c.perm[cl];
+        o.trk_cl_idx[off + __popc(m & ((1u << lane) - 1))] = in_idx;
+        o.cluster_track[in_idx] = id;
+      }
+      off += __popc(m);
+    }
+    if (lane < 5) o.par[lane * mt + id] = c.t_par[(size_t)sd * 5 + lane];
+    if (lane < 15) o.cov[lane * mt + id] = c.t_cov[(size_t)sd * 15 + lane];
+    if (lane == 0) {
+      const int low = c.t_first_row[sd];
+      o.sector[id] = (int)c.srow[c.seed_head[sd]] / R;
+      o.first_row[id] = c.k_first[sd];
+      o.last_row[id] = c.k_last[sd];
+      o.n_clusters[id] = c.k_owned[sd];
+      o.x_ref[id] = c.rowtab[low].x;
+      o.z_ref[id] = c.t_zref[sd];
+      o.chi2[id] = c.t_chi2[sd];
+      o.ndf[id] = 2 * c.t_n_hits[sd] - 5;
+      o.trk_cl_start[id + 1] = end;
+    }
+  }
+}
+
+inline unsigned grid_for(long long n, int per_block, int n_sms, int waves) {
+  long long g = (n + per_block - 1) / per_block;
+  const long long cap = (long long)n_sms * waves;
+  if (g > cap) g = cap;
+  if (g < 1) g = 1;
+  return (unsigned)g;
+}
+
+}  // namespace
+
+int launches_s5() { return 6 + 9; }
+int launch_s5(const Ctx& c, const OutPtrs& o, cudaStream_t st) {
+  const unsigned gn = grid_for(c.n, kThreads, c.n_sms, 8);
+  const unsigned gs = grid_for(c.max_seeds, kThreads, c.n_sms, 8);          // thread per seed
+  const unsigned gw = grid_for((long long)c.max_seeds * 32, kThreads, c.n_sms, 8);   // warp per seed
+  k_init_out<<<gn, kThreads, 0, st>>>(c, o);
+  k_kept<<<gs, kThreads, 0, st>>>(c);
+  if (launch_scan_inclusive(c.kept_scan, &c.cnt->n_seeds, 0, c.max_seeds, c.tile_sums, &c.cnt->n_tracklets, c.n_sms, st)) return -1;
+  k_owner<<<gw, kThreads, 0, st>>>(c);
+  k_owned<<<gw, kThreads, 0, st>>>(c);
+  if (launch_scan_inclusive(c.surv_scan, &c.cnt->n_seeds, 0, c.max_seeds, c.tile_sums, &c.cnt->n_tracks, c.n_sms, st)) return -1;
+  if (launch_scan_inclusive(c.owned_scan, &c.cnt->n_seeds, 0, c.max_seeds, c.tile_sums, &c.cnt->n_track_clusters, c.n_sms, st)) return -1;
+  k_finalize<<<1, 1, 0, st>>>(c, o);
+  k_write<<<gw, kThreads, 0, st>>>(c, o);
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+}  // namespace tpc

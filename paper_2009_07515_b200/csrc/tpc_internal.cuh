@@ -1,0 +1,157 @@
+// Internal declarations shared by the CUDA translation units of libtpc_tracker.so (sm_100a only).
+// Nothing here is visible across the C ABI (include/tpc_tracker.h) and nothing is shared with oracle/.
+//
+// Arithmetic contract: fp32, one rounding per written operation, no FMA
+// contraction - every .cu file is compiled with `nvcc -fmad=false` and without --use_fast_math, so
+// + - * / sqrtf floorf are IEEE-correctly rounded and the decisions (bins, windows, link choice,
+// gates) come out bit-identical to any other IEEE implementation of DESIGN.md section 3.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tpc {
+
+constexpr int kMaxRows = 256;      // row ids are uint8
+constexpr int kScanTile = 2048;    // items per scan tile (256 threads x 8)
+
+// Per-row derived tables, one stated fp32 expression each; built on the host at create.
+struct RowTab {
+  float x;            // row_x[r]
+  float ymax;         // row_x[r] * tan_half_sector
+  int ny;             // (int)floor((2*ymax)*inv_cy) + 1
+  int ny_prefix;      // sum of ny over rows < r
+  float up_dx[2], up_ratio[2], up_wy[2], up_wz[2];   // index k-1, k = row step 1 or 2
+  float dn_dx[2], dn_ratio[2], dn_wy[2], dn_wz[2];
+};
+static_assert(sizeof(RowTab) == 80, "RowTab layout");
+
+// Device counter block (lives in the workspace).  All written by kernels.
+struct Counters {
+  int n_bins;             // N_b
+  int n_seeds;
+  int n_tracklets;
+  int n_tracks;
+  int n_track_clusters;
+  int n_linked;
+  int status;             // tpc_status_bits
+  int zero;               // always 0 (a device-resident "n = 0" for scans of host-known length)
+  unsigned long long kf_steps;
+  unsigned long long n_hits;
+  int s4_ticket;          // dynamic work counter of the S4 persistent kernel
+  int pad[3];
+};
+
+// Everything a kernel needs, passed by value (a few hundred bytes).
+struct Ctx {
+  // geometry / cuts
+  int S, R, SR;
+  int ny_total;                       // sum over rows of ny
+  float inv_cy, inv_cz, kb;
+  float err_y2, err_z2, link_T;
+  int min_chain_len, max_gap, min_tracklet_hits, min_track_hits;
+  float pick_chi2_cut, max_sinphi, y_margin, init_c_ss, init_c_tt, init_c_qq;
+  const RowTab* rowtab;               // [R]
+  // capacities
+  int max_clusters; int max_bins; int max_seeds; int max_tracks; int max_track_clusters;
+  // input of the current call
+  int n;
+  const uint8_t* in_sector; const uint8_t* in_row; const float* in_y; const float* in_z;
+  // S1
+  int* zmin_key; int* zmax_key;       // [S] order-preserving integer keys of the floats during the reduction
+  float* zmin; float* zmax; int* nz;  // [S]
+  int* bin_base;                      // [SR+1]
+  int* row_start;                     // [SR+1]
+  int* gbin;                          // [n] global bin of the input cluster
+  int* tmp_idx;                       // [n] input indices grouped by bin, arrival order
+  int* bins;                          // [max_bins+2]; after S1 bins[0..N_b] is the CSR bin_start
+  int* perm; float* ys; float* zs; uint16_t* srow;   // [n] sorted
+  int* tile_sums;                     // scan scratch
+  // S2 / S3
+  int* link_up_raw; int* link_dn_raw; int* link_up; int* link_dn;
+  int* flag;                          // [n] S3: chain length at qualifying heads else 0; reused by scans
+  int* flag_scan;                     // [n] inclusive scan of (flag != 0)
+  int* seed_head; int* seed_len;      // [max_seeds]
+  // S4
+  int* t_hit;                         // [max_seeds][R]
+  int* t_first_row; int* t_last_row; int* t_n_hits;   // [max_seeds]
+  float* t_par; float* t_cov; float* t_chi2; float* t_zref;   // [max_seeds][5], [max_seeds][15], ...
+  // S5
+  int* kept_scan;                     // [max_seeds] inclusive scan of kept flags
+  int* tracklet_of_seed;              // [max_seeds]
+  unsigned long long* owner;          // [n]
+  int* k_owned; int* k_first; int* k_last;   // [max_seeds]
+  int* surv_scan; int* owned_scan;    // [max_seeds] inclusive scans
+  Counters* cnt;
+  int n_sms;
+};
+
+// ---- host launchers, one per stage (each only enqueues kernels on `st`)
+int launch_s1(const Ctx& c, cudaStream_t st);
+int launch_s2(const Ctx& c, cudaStream_t st);
+int launch_s3(const Ctx& c, cudaStream_t st);
+int launch_s4(const Ctx& c, cudaStream_t st);
+struct OutPtrs {
+  int* n_tracks; int* status; int* sector; int* first_row; int* last_row; int* n_clusters; float* par; float* cov;
+  float* x_ref; float* z_ref; float* chi2; int* ndf; int* trk_cl_start; int* trk_cl_idx; int* cluster_track;
+  int max_tracks; int max_track_clusters;
+};
+int launch_s5(const Ctx& c, const OutPtrs& o, cudaStream_t st);
+int launch_reset(const Ctx& c, cudaStream_t st);
+
+// In-place inclusive scan of data[0 .. *n_ptr + n_add) (int32), length known only on the device.
+// max_n bounds the grid; tile_sums needs ceil(max_n / kScanTile) + 1 ints.  total_out (nullable)
+// receives the grand total.  3 launches.
+int launch_scan_inclusive(int* data, const int* n_ptr, int n_add, long long max_n, int* tile_sums, int* total_out,
+                          int n_sms, cudaStream_t st);
+
+// number of kernel launches per call of each launcher (kept next to the launch code)
+int launches_reset(); int launches_s1(); int launches_s2(); int launches_s3(); int launches_s4(); int launches_s5();
+
+// ---------------------------------------------------------------------------- device helpers
+#ifdef __CUDACC__
+// floor(v) clamped to [0, hi]; NaN and negatives -> 0
+__device__ __forceinline__ int floor_clamp(float v, int hi) {
+  const float f = floorf(v);
+  if (!(f >= 0.0f)) return 0;
+  if (f >= (float)hi) return hi;
+  return (int)f;
+}
+
+// order-preserving float <-> int key (signed compare)
+__device__ __forceinline__ int float_key(float f) {
+  const int i = __float_as_int(f);
+  return i >= 0 ? i : i ^ 0x7FFFFFFF;
+}
+__device__ __forceinline__ float key_float(int k) { return __int_as_float(k >= 0 ? k : k ^ 0x7FFFFFFF); }
+
+// The (y,z) grid of one (sector,row): what a rectangle query needs.
+struct RowGrid {
+  int b0;        // bin_base[s*R + t]
+  int ny;        // bins along y
+  int nz;        // bins along z (sector-wide)
+  float ymax, zmin;
+};
+
+// Visits the sorted positions of one row whose (y,z) lies in the closed rectangle, in ascending
+// position (iz ascending, then position) - the "rectangle query" of DESIGN.md section 3.1.
+template <class F>
+__device__ __forceinline__ void for_each_in_rect(const RowGrid& g, float inv_cy, float inv_cz,
+                                                 const int* __restrict__ bin_start, const float* __restrict__ ys,
+                                                 const float* __restrict__ zs, float ylo, float yhi, float zlo,
+                                                 float zhi, F&& f) {
+  const int iy0 = floor_clamp((ylo + g.ymax) * inv_cy, g.ny - 1);
+  const int iy1 = floor_clamp((yhi + g.ymax) * inv_cy, g.ny - 1);
+  const int iz0 = floor_clamp((zlo - g.zmin) * inv_cz, g.nz - 1);
+  const int iz1 = floor_clamp((zhi - g.zmin) * inv_cz, g.nz - 1);
+  for (int iz = iz0; iz <= iz1; ++iz) {
+    const int b = g.b0 + iz * g.ny;
+    const int jb = __ldg(bin_start + b + iy0), je = __ldg(bin_start + b + iy1 + 1);
+    for (int j = jb; j < je; ++j) {
+      const float yj = __ldg(ys + j), zj = __ldg(zs + j);
+      if (yj >= ylo && yj <= yhi && zj >= zlo && zj <= zhi) f(j, yj, zj);
+    }
+  }
+}
+#endif
+
+}  // namespace tpc
