@@ -1,0 +1,356 @@
+#!/usr/bin/env python
+"""bench.py - TPC clusters/s tracked per B200 on a synthetic time frame (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5] [--impl ours|reference]
+
+A step = one pass of the whole hot path (S1..S5, tpc_track_timeframe) over one time frame.
+`value`  : clusters/s, device-timed (CUDA events), inputs resident in HBM.
+`e2e`    : the same through tpc_track_timeframe_host (pinned HOST buffers in and out).
+`roofline`: the dominant kernel against the measured HBM peak (MEASURED_PEAKS.json), algorithmic
+            bytes per DESIGN.md section 6, duration from CUDA events recorded inside the library.
+`cpu_baseline`: the oracle, as it stands, single-threaded, on a bounded sample (whole sectors).
+N > 1: replicas only - every rank tracks its own time frame, no collective on the
+data path; value = clusters of all ranks / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "TPC clusters/sec tracked per B200 (time frame, device-timed)"
+UNIT = "clusters/s"
+FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg5", help="cfg1..cfg5 (BASELINE.json configs[0..4]); cfg5 = the metric's")
+    ap.add_argument("--collisions", type=int, default=0, help="override n_collisions (debug; 0 = the config's own)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.lines = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_timeframe(args, rank: int):
+    from tpc_synth import generate_config
+    import torch
+    over = {}
+    if args.collisions:
+        over["n_collisions"] = args.collisions
+    if rank:
+        from tpc_synth import CONFIGS
+        over["seed"] = CONFIGS[args.workload]["seed"] + 1000 * rank     # replicas track different time frames
+    dev = "cuda" if torch.cuda.is_available() and args.impl == "ours" else "cpu"
+    return generate_config(args.workload, device=dev, **over)
+
+
+def algorithmic_bytes(k: dict) -> dict:
+    """what the method itself must move, ideal caching."""
+    N, Nb, S, H, K, T = k["n_clusters"], k["n_bins"], k["kf_steps"], k["n_hits"], k["n_seeds"], k["n_tracks"]
+    L = k["n_linked"]
+    Ho = k["n_track_clusters"]
+    b = {
+        "S1": 53 * N + 8 * Nb,
+        "S2": 20 * N + 4 * Nb,
+        "S3": 24 * N + 4 * L + 8 * K,
+        "S4": 20 * S + 8 * H + 120 * K,
+        "S5": 12 * N + 32 * H + 4 * Ho + 100 * T,
+    }
+    b["total"] = sum(b.values())
+    return b
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the same workload."""
+    from oracle import Oracle
+    from tpc_synth import default_params, select_sectors
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    tf = make_timeframe(args, 0)
+    P = default_params(tf)           # cell chosen on the full workload, as for the CUDA arm
+    # calibrate on one sector, then take as many whole sectors as fit ~100 s / (K+W) per step
+    sub, _ = select_sectors(tf, [0])
+    t0 = time.perf_counter()
+    Oracle(P).run(sub.sector, sub.row, sub.y, sub.z)
+    rate = sub.n / max(1e-9, time.perf_counter() - t0)
+    budget = 100.0 / max(1, args.steps + args.warmup)
+    order = list(range(tf.geometry.n_sectors))
+    counts = np.bincount(tf.sector, minlength=tf.geometry.n_sectors)
+    take, tot = [], 0
+    for s in order:
+        if take and (tot + counts[s]) / rate > budget:
+            break
+        take.append(s); tot += int(counts[s])
+    sub, _ = select_sectors(tf, take)
+    o = Oracle(P)
+    times = []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        o.run(sub.sector, sub.row, sub.y, sub.z)
+        if i >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    dt = float(np.mean(times))
+    val = sub.n / dt
+    sample = f"sectors {take[0]}..{take[-1]} of {tf.name} ({sub.n} of {tf.n} clusters), all five stages, fp32"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": tf.name, "n_clusters": tf.n, "sample_clusters": sub.n},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2009_07515_b200 as tpc
+    from tpc_synth import default_params, select_sectors
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    t_gen = time.perf_counter()
+    tf = make_timeframe(args, rank)
+    t_gen = time.perf_counter() - t_gen
+    P = default_params(tf)
+    caps = tpc.suggest_capacities(tf.n, P)
+    caps["max_bins"] = tpc.max_bins_bound(tf.sector, tf.z, P)
+
+    # sizing run with loose capacities, then a tracker with capacities fitted to this workload
+    # (x1.25): the workspace the timed runs use is what a deployment would allocate.
+    th = lambda a: torch.from_numpy(np.ascontiguousarray(a))  # noqa: E731
+    d_in = [th(a).to(dev) for a in (tf.sector, tf.row, tf.y, tf.z)]
+    trk = tpc.Tracker(P, caps["max_clusters"], caps["max_bins"], caps["max_seeds"], caps["max_tracks"],
+                      caps["max_track_clusters"], device=dev)
+    out = trk.new_tracks(tf.n)
+    trk.track_timeframe(*d_in, out)
+    k0 = trk.counters()
+    if k0["status"] != 0:
+        raise RuntimeError(f"tracker status {k0['status']}")
+    trk.destroy(); del trk, out
+    torch.cuda.empty_cache()
+    fit = lambda v, lo=1024: int(max(lo, v * 1.25 + 1))  # noqa: E731
+    caps.update(max_bins=fit(k0["n_bins"]), max_seeds=fit(k0["n_seeds"]), max_tracks=fit(k0["n_tracks"]),
+                max_track_clusters=fit(k0["n_track_clusters"]))
+    trk = tpc.Tracker(P, caps["max_clusters"], caps["max_bins"], caps["max_seeds"], caps["max_tracks"],
+                      caps["max_track_clusters"], host_io=not args.no_e2e, device=dev)
+    out = trk.new_tracks(tf.n)
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-timed: K steps back to back, inputs resident
+    for _ in range(args.warmup):
+        trk.track_timeframe(*d_in, out)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        trk.track_timeframe(*d_in, out)
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else None
+    k = trk.counters()
+
+    # ---- per-stage device times (events recorded inside the library, separate untimed-by-value runs)
+    trk.enable_stage_timing(True)
+    stage = np.zeros(5)
+    for _ in range(args.steps):
+        trk.track_timeframe(*d_in, out)
+        stage += np.array(trk.stage_ms())
+    stage /= args.steps
+    trk.enable_stage_timing(False)
+
+    # ---- end to end through the host entry point (pinned host buffers in and out)
+    e2e = None
+    if not args.no_e2e:
+        h_in = [th(a).pin_memory() for a in (tf.sector, tf.row, tf.y, tf.z)]
+        h_out = trk.new_tracks(tf.n, host=True)
+        for _ in range(min(2, args.warmup)):
+            trk.track_timeframe_host(*h_in, h_out)
+        barrier()
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for _ in range(args.steps):
+            trk.track_timeframe_host(*h_in, h_out)
+        e1.record(stream)
+        barrier()
+        ms_e2e = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3)
+        e2e = {"ms": ms_e2e / args.steps, "h2d": int(sum(t.numel() * t.element_size() for t in h_in)), "d2h": h_out.bytes_out()}
+
+    # ---- max over ranks
+    n_total = tf.n
+    if world > 1:
+        t = torch.tensor([ms_total, e2e["ms"] if e2e else 0.0], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t[0]); ms_e2e_max = float(t[1])
+        if e2e:
+            e2e["ms"] = ms_e2e_max
+        nn = torch.tensor([tf.n], device=dev, dtype=torch.int64)
+        dist.all_reduce(nn)
+        n_total = int(nn[0])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    ms_step = ms_total / args.steps
+    value = n_total / (ms_step * 1e-3)
+    peak, peak_src = hbm_peak()
+    bytes_ = algorithmic_bytes(k)
+    names = ["S1", "S2", "S3", "S4", "S5"]
+    dom = int(np.argmax(stage))
+    dom_kernel = {"S1": "S1 (sort+bin, 10 launches)", "S2": "k_neighbours", "S3": "S3 (cleaner, 7 launches)",
+                  "S4": "k_tracklets", "S5": "S5 (selector, 15 launches)"}[names[dom]]
+    achieved = bytes_[names[dom]] / (stage[dom] * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom_kernel, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_[names[dom]],
+                "kernel_ms": float(stage[dom]),
+                "whole_path": {"algorithmic_bytes": bytes_["total"], "achieved": bytes_["total"] / (ms_step * 1e-3) / 1e9,
+                               "frac_of_measured": bytes_["total"] / (ms_step * 1e-3) / 1e9 / peak,
+                               "frac_of_8TBs": bytes_["total"] / (ms_step * 1e-3) / 1e9 / 8000.0},
+                "stage_ms": {n: float(v) for n, v in zip(names, stage)},
+                "stage_bytes": {n: int(bytes_[n]) for n in names}}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import Oracle
+        # bounded sample: whole sectors, ~15 s of single-threaded oracle work
+        counts = np.bincount(tf.sector, minlength=tf.geometry.n_sectors)
+        take, tot = [], 0
+        for s in range(tf.geometry.n_sectors):
+            if take and tot + counts[s] > 8_000_000:
+                break
+            take.append(s); tot += int(counts[s])
+        sub, _ = select_sectors(tf, take)
+        t0 = time.perf_counter()
+        o = Oracle(P).run(sub.sector, sub.row, sub.y, sub.z)
+        dt = time.perf_counter() - t0
+        cpu = {"value": sub.n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"sectors {take[0]}..{take[-1]} of {tf.name} ({sub.n} of {tf.n} clusters), all five stages, fp32, {dt:.1f} s",
+               "stage_seconds": [float(v) for v in o.get("stage_seconds")]}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": tf.name, "n_clusters_per_gpu": tf.n, "n_clusters_total": n_total,
+                   "parallelism": "replicas (one time frame per GPU, no collective)" if world > 1 else "single GPU",
+                   "l2": "inputs larger than L2" if tf.n * 10 > 126e6 else "inputs fit L2 (small config)",
+                   "cell_cm": float(P["cell_y"]), "generate_s": round(t_gen, 1),
+                   "workspace_GB": round(trk.workspace_bytes / 1e9, 2)},
+        "counters": {kk: int(v) for kk, v in k.items()},
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+        "gpu_launches": trk.launches_per_call() * args.steps,
+        "clocks": clocks,
+    }
+    if e2e:
+        line["e2e"] = {"value": n_total / (e2e["ms"] * 1e-3), "unit": UNIT, "ms_per_step": e2e["ms"],
+                       "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"]}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
