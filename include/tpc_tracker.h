@@ -137,32 +137,32 @@ typedef struct {
  * All positions are indices into the sorted order of S1. */
 enum tpc_stage_array {
   TPC_VIEW_PERM = 0,        /* int32 [n]      sorted position -> input index (S1) */
-  TPC_VIEW_YS = 1,          /* float [n]      sorted y */
-  TPC_VIEW_ZS = 2,          /* float [n]      sorted z */
-  TPC_VIEW_SROW = 3,        /* uint16 [n]     sector*n_rows + row of the sorted cluster */
-  TPC_VIEW_BIN_START = 4,   /* int32 [n_bins+1] CSR over global bins */
-  TPC_VIEW_ROW_START = 5,   /* int32 [n_sectors*n_rows+1] */
-  TPC_VIEW_BIN_BASE = 6,    /* int32 [n_sectors*n_rows+1] first global bin of each (sector,row) */
-  TPC_VIEW_ZMIN = 7,        /* float [n_sectors] */
-  TPC_VIEW_ZMAX = 8,        /* float [n_sectors] */
-  TPC_VIEW_NZ = 9,          /* int32 [n_sectors] */
-  TPC_VIEW_LINK_UP_RAW = 10,/* int32 [n] (S2) */
-  TPC_VIEW_LINK_DN_RAW = 11,
-  TPC_VIEW_LINK_UP = 12,    /* int32 [n] cleaned (S3) */
-  TPC_VIEW_LINK_DN = 13,
-  TPC_VIEW_SEED_HEAD = 14,  /* int32 [n_seeds] */
-  TPC_VIEW_SEED_LEN = 15,   /* int32 [n_seeds] */
-  TPC_VIEW_T_HIT = 16,      /* int32 [n_seeds][n_rows] sorted position or -1 (S4) */
-  TPC_VIEW_T_FIRST_ROW = 17,/* int32 [n_seeds] */
-  TPC_VIEW_T_LAST_ROW = 18, /* int32 [n_seeds] */
-  TPC_VIEW_T_N_HITS = 19,   /* int32 [n_seeds] */
-  TPC_VIEW_T_PAR = 20,      /* float [n_seeds][5] */
-  TPC_VIEW_T_COV = 21,      /* float [n_seeds][15] */
-  TPC_VIEW_T_CHI2 = 22,     /* float [n_seeds] */
-  TPC_VIEW_T_ZREF = 23,     /* float [n_seeds] */
-  TPC_VIEW_TRACKLET_OF_SEED = 24, /* int32 [n_seeds] rank among kept tracklets or -1 (S5) */
-  TPC_VIEW_OWNED = 25,      /* int32 [n_seeds] clusters owned (S5) */
-  TPC_VIEW_COUNT_ = 26
+  TPC_VIEW_YZ = 1,          /* float [n][2]   sorted (y, z) pairs */
+  TPC_VIEW_SROW = 2,        /* uint16 [n]     sector*n_rows + row of the sorted cluster */
+  TPC_VIEW_BIN_START = 3,   /* int32 [n_bins+1] CSR over global bins */
+  TPC_VIEW_ROW_START = 4,   /* int32 [n_sectors*n_rows+1] */
+  TPC_VIEW_BIN_BASE = 5,    /* int32 [n_sectors*n_rows+1] first global bin of each (sector,row) */
+  TPC_VIEW_ZMIN = 6,        /* float [n_sectors] */
+  TPC_VIEW_ZMAX = 7,        /* float [n_sectors] */
+  TPC_VIEW_NZ = 8,          /* int32 [n_sectors] */
+  TPC_VIEW_LINK_UP_RAW = 9, /* int32 [n] (S2) */
+  TPC_VIEW_LINK_DN_RAW = 10,
+  TPC_VIEW_LINK_UP = 11,    /* int32 [n] cleaned (S3) */
+  TPC_VIEW_LINK_DN = 12,
+  TPC_VIEW_SEED_HEAD = 13,  /* int32 [n_seeds] */
+  TPC_VIEW_SEED_LEN = 14,   /* int32 [n_seeds] */
+  TPC_VIEW_T_HIT = 15,      /* int32 [n_seeds][n_rows] sorted position or -1 (S4); row r of seed k is
+                               defined only for t_first_row[k] <= r <= t_last_row[k] (no hits outside) */
+  TPC_VIEW_T_FIRST_ROW = 16,/* int32 [n_seeds] */
+  TPC_VIEW_T_LAST_ROW = 17, /* int32 [n_seeds] */
+  TPC_VIEW_T_N_HITS = 18,   /* int32 [n_seeds] */
+  TPC_VIEW_T_PAR = 19,      /* float [n_seeds][5] */
+  TPC_VIEW_T_COV = 20,      /* float [n_seeds][15] */
+  TPC_VIEW_T_CHI2 = 21,     /* float [n_seeds] */
+  TPC_VIEW_T_ZREF = 22,     /* float [n_seeds] */
+  TPC_VIEW_TRACKLET_OF_SEED = 23, /* int32 [n_seeds] rank among kept tracklets or -1 (S5) */
+  TPC_VIEW_OWNED = 24,      /* int32 [n_seeds] clusters owned (S5) */
+  TPC_VIEW_COUNT_ = 25
 };
 
 typedef struct {

@@ -55,7 +55,7 @@ class tpc_stage_view_t(C.Structure):
 
 
 VIEWS = {name: i for i, name in enumerate([
-    "perm", "ys", "zs", "srow", "bin_start", "row_start", "bin_base", "zmin", "zmax", "nz",
+    "perm", "yz", "srow", "bin_start", "row_start", "bin_base", "zmin", "zmax", "nz",
     "link_up_raw", "link_dn_raw", "link_up", "link_dn", "seed_head", "seed_len",
     "t_hit", "t_first_row", "t_last_row", "t_n_hits", "t_par", "t_cov", "t_chi2", "t_zref",
     "tracklet_of_seed", "k_owned"])}

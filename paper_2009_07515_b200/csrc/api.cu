@@ -65,7 +65,7 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   c.bin_base = cv.take<int>(SR + 1); c.row_start = cv.take<int>(SR + 1);
   c.gbin = cv.take<int>(N); c.tmp_idx = cv.take<int>(N);
   c.bins = cv.take<int>(NB + 2 + 8);
-  c.perm = cv.take<int>(N); c.ys = cv.take<float>(N); c.zs = cv.take<float>(N); c.srow = cv.take<uint16_t>(N);
+  c.perm = cv.take<int>(N); c.yz = cv.take<float2>(N); c.srow = cv.take<uint16_t>(N);
   size_t max_scan = N > NB + 2 ? N : NB + 2;
   if (K > max_scan) max_scan = K;
   c.tile_sums = cv.take<int>(max_scan / kScanTile + 2);
@@ -331,8 +331,7 @@ int tpc_tracker_stage_view(tpc_tracker_t* t, int32_t which, tpc_stage_view_t* ou
   auto set = [&](const void* p, int64_t cnt, int eb, int fl) { out->ptr = p; out->n = cnt; out->elem_bytes = eb; out->is_float = fl; };
   switch (which) {
     case TPC_VIEW_PERM: set(c.perm, n, 4, 0); break;
-    case TPC_VIEW_YS: set(c.ys, n, 4, 1); break;
-    case TPC_VIEW_ZS: set(c.zs, n, 4, 1); break;
+    case TPC_VIEW_YZ: set(c.yz, 2 * n, 4, 1); break;
     case TPC_VIEW_SROW: set(c.srow, n, 2, 0); break;
     case TPC_VIEW_BIN_START: set(c.bins, (int64_t)k.n_bins + 1, 4, 0); break;
     case TPC_VIEW_ROW_START: set(c.row_start, SR1, 4, 0); break;

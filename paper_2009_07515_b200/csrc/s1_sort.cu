@@ -164,8 +164,7 @@ __global__ void __launch_bounds__(kThreads) k_place(Ctx c) {
     for (int j = bs; j < be; ++j) rank += (__ldg(c.tmp_idx + j) < i);
     const int fp = bs + rank;
     c.perm[fp] = i;
-    c.ys[fp] = __ldg(c.in_y + i);
-    c.zs[fp] = __ldg(c.in_z + i);
+    c.yz[fp] = make_float2(__ldg(c.in_y + i), __ldg(c.in_z + i));
     c.srow[fp] = (uint16_t)((int)__ldg(c.in_sector + i) * c.R + (int)__ldg(c.in_row + i));
   }
 }

@@ -35,14 +35,14 @@ __global__ void __launch_bounds__(kThreads) k_neighbours(Ctx c) {
     reinterpret_cast<int*>(tab)[i] = __ldg(reinterpret_cast<const int*>(c.rowtab) + i);
   __syncthreads();
   if (c.cnt->status) return;
-  const float* __restrict__ ys = c.ys;
-  const float* __restrict__ zs = c.zs;
+  const float2* __restrict__ yz = c.yz;
   const int* __restrict__ bin_start = c.bins;
   const long long n = c.n;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
     const int sr = c.srow[i];
     const int s = sr / c.R, r = sr - s * c.R;
-    const float y = ys[i], z = zs[i];
+    const float2 me = yz[i];
+    const float y = me.x, z = me.y;
     int lu = -1, ld = -1;
 
     Cand U, D;
@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(kThreads) k_neighbours(Ctx c) {
       const float yc = y * tab[r].up_ratio[k - 1], wy = tab[r].up_wy[k - 1], wz = tab[r].up_wz[k - 1];
       uylo = yc - wy; uyhi = yc + wy; uzlo = z - wz; uzhi = z + wz;
       gu = make_grid(c, tab, s, r + k);
-      for_each_in_rect(gu, c.inv_cy, c.inv_cz, bin_start, ys, zs, uylo, uyhi, uzlo, uzhi, [&](int j, float yj, float zj) {
+      for_each_in_rect(gu, c.inv_cy, c.inv_cz, bin_start, yz, uylo, uyhi, uzlo, uzhi, [&](int j, float yj, float zj) {
         if (U.n < kCap) { U.pos[U.n] = j; U.y[U.n] = yj; U.z[U.n] = zj; }
         ++U.n;
       });
@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(kThreads) k_neighbours(Ctx c) {
         const float yc = y * tab[r].dn_ratio[k - 1], wy = tab[r].dn_wy[k - 1], wz = tab[r].dn_wz[k - 1];
         dylo = yc - wy; dyhi = yc + wy; dzlo = z - wz; dzhi = z + wz;
         gd = make_grid(c, tab, s, r - k);
-        for_each_in_rect(gd, c.inv_cy, c.inv_cz, bin_start, ys, zs, dylo, dyhi, dzlo, dzhi, [&](int j, float yj, float zj) {
+        for_each_in_rect(gd, c.inv_cy, c.inv_cz, bin_start, yz, dylo, dyhi, dzlo, dzhi, [&](int j, float yj, float zj) {
           if (D.n < kCap) { D.pos[D.n] = j; D.y[D.n] = yj; D.z[D.n] = zj; }
           ++D.n;
         });
@@ -89,8 +89,8 @@ __global__ void __launch_bounds__(kThreads) k_neighbours(Ctx c) {
         for (int a = 0; a < U.n; ++a)
           for (int b = 0; b < D.n; ++b) score(U.pos[a], U.y[a], U.z[a], D.pos[b], D.y[b], D.z[b]);
       } else {   // rare: crowded window, walk the rectangles again
-        for_each_in_rect(gu, c.inv_cy, c.inv_cz, bin_start, ys, zs, uylo, uyhi, uzlo, uzhi, [&](int u, float yu, float zu) {
-          for_each_in_rect(gd, c.inv_cy, c.inv_cz, bin_start, ys, zs, dylo, dyhi, dzlo, dzhi,
+        for_each_in_rect(gu, c.inv_cy, c.inv_cz, bin_start, yz, uylo, uyhi, uzlo, uzhi, [&](int u, float yu, float zu) {
+          for_each_in_rect(gd, c.inv_cy, c.inv_cz, bin_start, yz, dylo, dyhi, dzlo, dzhi,
                            [&](int d, float yd, float zd) { score(u, yu, zu, d, yd, zd); });
         });
       }

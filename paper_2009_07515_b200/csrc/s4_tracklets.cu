@@ -5,10 +5,18 @@
 // circle propagation in a uniform Bz, full 5x5 symmetric covariance (15 unique entries) in
 // registers, textbook update.
 //
-// Persistent kernel: one thread per tracklet, warps fetch 32 consecutive seeds from a global
-// ticket counter (one atomic per warp), so SMs stay busy whatever the chain-length mix.  The hit
-// table [seed][row] of a warp's 32 seeds is one contiguous 32*R*4-byte block and is cleared
-// cooperatively with coalesced stores.
+// Persistent kernel, one thread per tracklet, ONE uniform step loop for all three phases: every
+// iteration each lane resolves its next row (chain cluster, row above, row below), then all lanes run
+// the same propagate -> candidate (known cluster or grid search) -> update code together, whatever
+// phase they are in.  A lane that finishes writes its tracklet and takes the next seed from a global
+// ticket (idle lanes of a warp are served by one atomic: ballot + popc), so lanes never wait for the
+// longest chain of a batch.  (Round 1a ran the three phases as three loops per 32-seed batch and
+// measured 3.7 active lanes per instruction; see profiles/.)
+//
+// Hit table t_hit[seed][row]: no clearing pass.  A lane writes every row it visits between the lowest
+// updated row and the turning row (a position, or -1 for a skipped / empty row), so the entries in
+// [first_row, last_row] are all defined and nothing outside that range is ever read (S5 and the debug
+// view honour the range).
 //
 // Arithmetic is written operation by operation in the order of DESIGN.md section 3.4 (compiled with
 // -fmad=false): the transport J C J^T skips only the terms that are structurally 0*x or 1*x.
@@ -18,6 +26,7 @@ namespace tpc {
 namespace {
 
 constexpr int kThreads = 128;
+constexpr int kCtasPerSm = 4;
 
 // symmetric 5x5, lower triangle row-major: index(i,j) = i*(i+1)/2 + j for i >= j
 #define CI(i, j) ((i) >= (j) ? ((i) * ((i) + 1) / 2 + (j)) : ((j) * ((j) + 1) / 2 + (i)))
@@ -124,18 +133,9 @@ __device__ __forceinline__ void kf_update(KF& k, float ym, float zm, float err_y
   for (int i = 0; i < 15; ++i) k.c[i] = n[i];
 }
 
-struct Grid {
-  const int* __restrict__ bin_start;
-  const float* __restrict__ ys;
-  const float* __restrict__ zs;
-  const int* __restrict__ bin_base_s;   // bin_base + s*R
-  int nz;
-  float zmin;
-};
-
-// nearest gated cluster of row r, or -1
-__device__ __forceinline__ int kf_search(const Ctx& c, const RowTab* tab, const Grid& G, int r, const KF& k, float zref,
-                                         float* ym, float* zm) {
+// nearest gated cluster of row r of sector s, or -1
+__device__ __forceinline__ int kf_search(const Ctx& c, int b0, int ny, float ymax, int nz, float zmin, const KF& k,
+                                         float zref, float* ym, float* zm) {
   const float cut = c.pick_chi2_cut;
   const float sy2 = k.c[CI(0, 0)] + c.err_y2, sz2 = k.c[CI(1, 1)] + c.err_z2;
   const float hy = sqrtf(cut * sy2), hz = sqrtf(cut * sz2);
@@ -145,8 +145,8 @@ __device__ __forceinline__ int kf_search(const Ctx& c, const RowTab* tab, const 
   float best = INFINITY;
   int arg = -1;
   RowGrid g;
-  g.b0 = __ldg(G.bin_base_s + r); g.ny = tab[r].ny; g.nz = G.nz; g.ymax = tab[r].ymax; g.zmin = G.zmin;
-  for_each_in_rect(g, c.inv_cy, c.inv_cz, G.bin_start, G.ys, G.zs, ylo, yhi, zlo, zhi, [&](int j, float yj, float zj) {
+  g.b0 = b0; g.ny = ny; g.nz = nz; g.ymax = ymax; g.zmin = zmin;
+  for_each_in_rect(g, c.inv_cy, c.inv_cz, c.bins, c.yz, ylo, yhi, zlo, zhi, [&](int j, float yj, float zj) {
     const float dy = yj - k.p[0];
     const float dz = (zj - zref) - k.p[1];
     const float d2 = (dy * dy) * wy + (dz * dz) * wz;
@@ -155,133 +155,172 @@ __device__ __forceinline__ int kf_search(const Ctx& c, const RowTab* tab, const 
   return arg;
 }
 
-__global__ void __launch_bounds__(kThreads) k_tracklets(Ctx c) {
-  extern __shared__ RowTab tab[];
-  for (int i = threadIdx.x; i < c.R * (int)(sizeof(RowTab) / 4); i += blockDim.x)
-    reinterpret_cast<int*>(tab)[i] = __ldg(reinterpret_cast<const int*>(c.rowtab) + i);
+enum : int { kIdle = 0, kPhaseA = 1, kPhaseB = 2, kPhaseC = 3 };
+
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_tracklets(Ctx c) {
+  extern __shared__ float smem[];
+  const int R = c.R;
+  float* tx = smem;                               // row_x[r]
+  float* tymax = smem + R;                        // ymax_r
+  int* tny = reinterpret_cast<int*>(smem + 2 * R);   // ny_r
+  for (int i = threadIdx.x; i < R; i += blockDim.x) {
+    tx[i] = c.rowtab[i].x; tymax[i] = c.rowtab[i].ymax; tny[i] = c.rowtab[i].ny;
+  }
   __syncthreads();
   if (c.cnt->status) return;
   const int n_seeds = c.cnt->n_seeds;
-  const int R = c.R;
   const int lane = threadIdx.x & 31;
-  const float* __restrict__ ys = c.ys;
-  const float* __restrict__ zs = c.zs;
+  const float2* __restrict__ yz = c.yz;
   const int* __restrict__ link_up = c.link_up;
+  const float ey2 = c.err_y2, ez2 = c.err_z2, kb = c.kb, msp = c.max_sinphi, ymargin = c.y_margin;
+  const int max_gap = c.max_gap;
+
   unsigned long long steps = 0, hits_kept = 0;
-  int kept_cnt = 0;
+  bool exhausted = false;                         // warp-uniform: the ticket ran out
+
+  // per-lane tracklet state
+  int phase = kIdle;
+  int sd = 0, sR = 0, r0 = 0, cur = 0, gap = 0, nh = 0, last_row = 0, low = 0, nextcl = -1, nz = 0;
+  float zref = 0.f, zmin = 0.f;
+  int* hit = nullptr;
+  KF k, sv;                                       // sv: state at the last update (A/B: parameters only; C: the output)
+#pragma unroll
+  for (int i = 0; i < 5; ++i) { k.p[i] = 0.f; sv.p[i] = 0.f; }
+#pragma unroll
+  for (int i = 0; i < 15; ++i) { k.c[i] = 0.f; sv.c[i] = 0.f; }
+  k.chi2 = 0.f; sv.chi2 = 0.f;
 
   for (;;) {
-    int base = 0;
-    if (lane == 0) base = atomicAdd(&c.cnt->s4_ticket, 32);
-    base = __shfl_sync(0xffffffffu, base, 0);
-    if (base >= n_seeds) break;
-    const int cnt = min(32, n_seeds - base);
-    {   // clear the warp's hit tables (contiguous cnt*R ints)
-      int* h0 = c.t_hit + (size_t)base * R;
-      for (int i = lane; i < cnt * R; i += 32) h0[i] = -1;
-    }
-    __syncwarp();
-    const int sd = base + lane;
-    if (sd < n_seeds) {
-      int* __restrict__ hit = c.t_hit + (size_t)sd * R;
-      const int h = __ldg(c.seed_head + sd), nx = __ldg(link_up + h);
-      const int srh = c.srow[h];
-      const int s = srh / R, r0 = srh - s * R;
-      const int r1 = (int)c.srow[nx] - s * R;
-      Grid G;
-      G.bin_start = c.bins; G.ys = ys; G.zs = zs; G.bin_base_s = c.bin_base + s * R;
-      G.nz = __ldg(c.nz + s); G.zmin = __ldg(c.zmin + s);
-      const float zref = __ldg(zs + h);
-      const float ey2 = c.err_y2, ez2 = c.err_z2, kb = c.kb, msp = c.max_sinphi;
-
-      KF k;
-      {
-        const float dx = tab[r1].x - tab[r0].x;
-        const float dy = __ldg(ys + nx) - __ldg(ys + h);
-        const float dz = __ldg(zs + nx) - zref;
-        const float dl = sqrtf(dx * dx + dy * dy);
-        k.p[0] = __ldg(ys + h); k.p[1] = 0.0f; k.p[2] = dy / dl; k.p[3] = dz / dl; k.p[4] = 0.0f;
-        kf_reset_cov(k, c);
-      }
-      hit[r0] = h;
-      int cur = r0;
-      float lp[5];
+    // ---- refill idle lanes from the ticket
+    const unsigned idle = __ballot_sync(0xffffffffu, phase == kIdle);
+    if (idle && !exhausted) {
+      const int leader = __ffs(idle) - 1;
+      int base = 0;
+      if (lane == leader) base = atomicAdd(&c.cnt->s4_ticket, __popc(idle));
+      base = __shfl_sync(0xffffffffu, base, leader);
+      if (base + __popc(idle) >= n_seeds) exhausted = true;
+      if (phase == kIdle) {
+        const int mine = base + __popc(idle & ((1u << lane) - 1u));
+        if (mine < n_seeds) {
+          sd = mine;
+          hit = c.t_hit + (size_t)sd * R;
+          const int h = __ldg(c.seed_head + sd), nx = __ldg(link_up + h);
+          const int srh = c.srow[h];
+          const int s = srh / R;
+          sR = s * R; r0 = srh - sR;
+          nz = __ldg(c.nz + s); zmin = __ldg(c.zmin + s);
+          const float2 ph = __ldg(yz + h), pn = __ldg(yz + nx);
+          zref = ph.y;
+          const int r1 = r0 + 1 + (nx >= __ldg(c.row_start + sR + r0 + 2));
+          const float dx = tx[r1] - tx[r0];
+          const float dy = pn.x - ph.x;
+          const float dz = pn.y - zref;
+          const float dl = sqrtf(dx * dx + dy * dy);
+          k.p[0] = ph.x; k.p[1] = 0.0f; k.p[2] = dy / dl; k.p[3] = dz / dl; k.p[4] = 0.0f;
+          kf_reset_cov(k, c);
 #pragma unroll
-      for (int i = 0; i < 5; ++i) lp[i] = k.p[i];
-      int last_row = r0;
-
-      // Phase A
-      bool up_ok = true;
-      for (int cl = nx; cl >= 0; cl = __ldg(link_up + cl)) {
-        const int rc = (int)c.srow[cl] - s * R;
-        ++steps;
-        if (!kf_propagate(k, kb, tab[rc].x - tab[cur].x, msp)) { up_ok = false; break; }
-        cur = rc;
-        kf_update(k, __ldg(ys + cl), __ldg(zs + cl) - zref, ey2, ez2);
-        hit[rc] = cl;
-#pragma unroll
-        for (int i = 0; i < 5; ++i) lp[i] = k.p[i];
-        last_row = rc;
-      }
-      // Phase B
-      if (up_ok) {
-        int gap = 0;
-        for (int r = cur + 1; r < R; ++r) {
-          ++steps;
-          if (!kf_propagate(k, kb, tab[r].x - tab[cur].x, msp)) break;
-          cur = r;
-          if (!(fabsf(k.p[0]) <= tab[r].ymax + c.y_margin)) break;
-          float ym, zm;
-          const int cl = kf_search(c, tab, G, r, k, zref, &ym, &zm);
-          if (cl >= 0) {
-            kf_update(k, ym, zm - zref, ey2, ez2);
-            hit[r] = cl; gap = 0;
-#pragma unroll
-            for (int i = 0; i < 5; ++i) lp[i] = k.p[i];
-            last_row = r;
-          } else if (++gap > c.max_gap) break;
+          for (int i = 0; i < 5; ++i) sv.p[i] = k.p[i];
+          hit[r0] = h;
+          cur = r0; last_row = r0; low = r0; nh = 1; gap = 0; nextcl = nx;
+          phase = kPhaseA;
         }
       }
-      // Phase C
+    }
+    if (!__any_sync(0xffffffffu, phase != kIdle)) break;
+
+    // ---- resolve this lane's next row r and its known cluster cl (or -1: search)
+    bool act = false, go_c = false, done = false;
+    int r = 0, cl = -1;
+    if (phase == kPhaseA) {
+      if (nextcl >= 0) {
+        cl = nextcl;
+        r = cur + 1 + (cl >= __ldg(c.row_start + sR + cur + 2));   // links go up one row or two
+        act = true;
+      } else {
+        phase = kPhaseB; gap = 0;
+      }
+    }
+    if (phase == kPhaseB) {
+      if (cur + 1 < R) { r = cur + 1; act = true; }
+      else go_c = true;
+    } else if (phase == kPhaseC) {
+      if (cur >= 1) { r = cur - 1; cl = (r >= r0) ? hit[r] : -1; act = true; }
+      else done = true;
+    }
+
+    // ---- one Kalman step, the same code for every phase
+    if (act) {
+      ++steps;
+      bool stop = false;
+      if (!kf_propagate(k, kb, tx[r] - tx[cur], msp)) stop = true;
+      else {
+        const int prev = cur;
+        cur = r;
+        if (phase != kPhaseA && !(fabsf(k.p[0]) <= tymax[r] + ymargin)) stop = true;
+        else {
+          float ym, zm;
+          const bool known = cl >= 0;
+          if (known) { const float2 v = __ldg(yz + cl); ym = v.x; zm = v.y; }
+          else cl = kf_search(c, __ldg(c.bin_base + sR + r), tny[r], tymax[r], nz, zmin, k, zref, &ym, &zm);
+          if (cl >= 0) {
+            kf_update(k, ym, zm - zref, ey2, ez2);
+            gap = 0;
+            if (!known) { hit[r] = cl; ++nh; }
 #pragma unroll
-      for (int i = 0; i < 5; ++i) k.p[i] = lp[i];
-      cur = last_row;
+            for (int i = 0; i < 5; ++i) sv.p[i] = k.p[i];
+            if (phase == kPhaseC) {
+#pragma unroll
+              for (int i = 0; i < 15; ++i) sv.c[i] = k.c[i];
+              sv.chi2 = k.chi2;
+              low = r;
+            } else {
+              last_row = r;
+              if (phase == kPhaseA) {
+                hit[r] = cl; ++nh;
+                if (r == prev + 2) hit[prev + 1] = -1;
+                nextcl = __ldg(link_up + cl);
+              }
+            }
+          } else {
+            if (phase == kPhaseB || r < r0) hit[r] = -1;
+            if (++gap > max_gap) stop = true;
+          }
+        }
+      }
+      if (stop) {
+        if (phase == kPhaseC) done = true;
+        else go_c = true;                         // a failed step of A skips B
+      }
+    }
+
+    // ---- turn round: back to the last updated state, covariance and chi2 reset
+    if (go_c) {
+#pragma unroll
+      for (int i = 0; i < 5; ++i) k.p[i] = sv.p[i];
       kf_reset_cov(k, c);
-      KF out = k;
-      int low = last_row;
-      {
-        int gap = 0;
-        for (int r = cur - 1; r >= 0; --r) {
-          ++steps;
-          if (!kf_propagate(k, kb, tab[r].x - tab[cur].x, msp)) break;
-          cur = r;
-          if (!(fabsf(k.p[0]) <= tab[r].ymax + c.y_margin)) break;
-          int cl = hit[r];
-          float ym, zm;
-          if (cl >= 0) { ym = __ldg(ys + cl); zm = __ldg(zs + cl); }
-          else cl = kf_search(c, tab, G, r, k, zref, &ym, &zm);
-          if (cl >= 0) {
-            kf_update(k, ym, zm - zref, ey2, ez2);
-            hit[r] = cl; gap = 0;
-            out = k; low = r;
-          } else if (++gap > c.max_gap) break;
-        }
-      }
-      int nh = 0;
-      for (int r = 0; r < R; ++r) {
-        if (r < low) hit[r] = -1;
-        else nh += hit[r] >= 0;
-      }
-      c.t_first_row[sd] = low; c.t_last_row[sd] = last_row; c.t_n_hits[sd] = nh;
 #pragma unroll
-      for (int i = 0; i < 5; ++i) c.t_par[(size_t)sd * 5 + i] = out.p[i];
-#pragma unroll
-      for (int i = 0; i < 15; ++i) c.t_cov[(size_t)sd * 15 + i] = out.c[i];
-      c.t_chi2[sd] = out.chi2; c.t_zref[sd] = zref;
-      if (nh >= c.min_tracklet_hits) { hits_kept += nh; ++kept_cnt; }
+      for (int i = 0; i < 15; ++i) sv.c[i] = k.c[i];
+      sv.chi2 = 0.0f;
+      cur = last_row; low = last_row; gap = 0;
+      phase = kPhaseC;
     }
-    __syncwarp();
+
+    // ---- finished: write the tracklet, become idle
+    if (done) {
+      for (int rr = r0; rr < low; ++rr) nh -= (hit[rr] >= 0);   // only if phase C stopped above the head
+      c.t_first_row[sd] = low; c.t_last_row[sd] = last_row; c.t_n_hits[sd] = nh;
+      float* op = c.t_par + (size_t)sd * 5;
+      float* oc = c.t_cov + (size_t)sd * 15;
+#pragma unroll
+      for (int i = 0; i < 5; ++i) op[i] = sv.p[i];
+#pragma unroll
+      for (int i = 0; i < 15; ++i) oc[i] = sv.c[i];
+      c.t_chi2[sd] = sv.chi2; c.t_zref[sd] = zref;
+      if (nh >= c.min_tracklet_hits) hits_kept += nh;
+      phase = kIdle;
+    }
   }
+
   for (int o = 16; o; o >>= 1) {
     steps += __shfl_xor_sync(0xffffffffu, steps, o);
     hits_kept += __shfl_xor_sync(0xffffffffu, hits_kept, o);
@@ -290,16 +329,14 @@ __global__ void __launch_bounds__(kThreads) k_tracklets(Ctx c) {
     if (steps) atomicAdd(&c.cnt->kf_steps, steps);
     if (hits_kept) atomicAdd(&c.cnt->n_hits, hits_kept);
   }
-  (void)kept_cnt;
 }
 
 }  // namespace
 
 int launches_s4() { return 1; }
 int launch_s4(const Ctx& c, cudaStream_t st) {
-  // persistent: enough CTAs to fill every SM; each warp pulls work until the ticket runs out
-  const int per_sm = 4;
-  k_tracklets<<<c.n_sms * per_sm, kThreads, c.R * sizeof(RowTab), st>>>(c);
+  // persistent: every SM filled with resident CTAs; lanes pull seeds until the ticket runs out
+  k_tracklets<<<c.n_sms * kCtasPerSm, kThreads, 3 * c.R * sizeof(float), st>>>(c);
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 

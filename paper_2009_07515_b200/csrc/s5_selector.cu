@@ -47,7 +47,8 @@ __global__ void __launch_bounds__(kThreads) k_owner(Ctx c) {
     if (!kept) continue;
     const unsigned long long key = make_key(c.t_n_hits[sd], inc - 1);
     const int* hit = c.t_hit + (size_t)sd * R;
-    for (int r = lane; r < R; r += 32) {
+    const int last = c.t_last_row[sd];
+    for (int r = c.t_first_row[sd] + lane; r <= last; r += 32) {   // the table is defined on [first_row, last_row] only
       const int cl = hit[r];
       if (cl >= 0) atomicMax(c.owner + cl, key);
     }
@@ -65,7 +66,8 @@ __global__ void __launch_bounds__(kThreads) k_owned(Ctx c) {
     if (tid >= 0) {
       const unsigned long long key = make_key(c.t_n_hits[sd], tid);
       const int* hit = c.t_hit + (size_t)sd * R;
-      for (int r = lane; r < R; r += 32) {
+      const int hi = c.t_last_row[sd];
+      for (int r = c.t_first_row[sd] + lane; r <= hi; r += 32) {
         const int cl = hit[r];
         if (cl >= 0 && c.owner[cl] == key) { ++owned; first = min(first, r); last = max(last, r); }
       }
@@ -109,10 +111,11 @@ __global__ void __launch_bounds__(kThreads) k_write(Ctx c, OutPtrs o) {
     int off = end - c.k_owned[sd];
     const unsigned long long key = make_key(c.t_n_hits[sd], c.tracklet_of_seed[sd]);
     const int* hit = c.t_hit + (size_t)sd * R;
-    for (int rb = 0; rb < R; rb += 32) {
+    const int hi = c.t_last_row[sd];
+    for (int rb = c.t_first_row[sd]; rb <= hi; rb += 32) {
       const int r = rb + lane;
       int cl = -1;
-      if (r < R) {
+      if (r <= hi) {
         cl = hit[r];
         if (cl >= 0 && c.owner[cl] != key) cl = -1;
       }

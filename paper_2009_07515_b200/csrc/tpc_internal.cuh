@@ -64,7 +64,7 @@ struct Ctx {
   int* gbin;                          // [n] global bin of the input cluster
   int* tmp_idx;                       // [n] input indices grouped by bin, arrival order
   int* bins;                          // [max_bins+2]; after S1 bins[0..N_b] is the CSR bin_start
-  int* perm; float* ys; float* zs; uint16_t* srow;   // [n] sorted
+  int* perm; float2* yz; uint16_t* srow;              // [n] sorted: input index, (y,z) pair, sector*R+row
   int* tile_sums;                     // scan scratch
   // S2 / S3
   int* link_up_raw; int* link_dn_raw; int* link_up; int* link_dn;
@@ -136,9 +136,8 @@ struct RowGrid {
 // position (iz ascending, then position) - the "rectangle query" of DESIGN.md section 3.1.
 template <class F>
 __device__ __forceinline__ void for_each_in_rect(const RowGrid& g, float inv_cy, float inv_cz,
-                                                 const int* __restrict__ bin_start, const float* __restrict__ ys,
-                                                 const float* __restrict__ zs, float ylo, float yhi, float zlo,
-                                                 float zhi, F&& f) {
+                                                 const int* __restrict__ bin_start, const float2* __restrict__ yz,
+                                                 float ylo, float yhi, float zlo, float zhi, F&& f) {
   const int iy0 = floor_clamp((ylo + g.ymax) * inv_cy, g.ny - 1);
   const int iy1 = floor_clamp((yhi + g.ymax) * inv_cy, g.ny - 1);
   const int iz0 = floor_clamp((zlo - g.zmin) * inv_cz, g.nz - 1);
@@ -147,8 +146,8 @@ __device__ __forceinline__ void for_each_in_rect(const RowGrid& g, float inv_cy,
     const int b = g.b0 + iz * g.ny;
     const int jb = __ldg(bin_start + b + iy0), je = __ldg(bin_start + b + iy1 + 1);
     for (int j = jb; j < je; ++j) {
-      const float yj = __ldg(ys + j), zj = __ldg(zs + j);
-      if (yj >= ylo && yj <= yhi && zj >= zlo && zj <= zhi) f(j, yj, zj);
+      const float2 v = __ldg(yz + j);
+      if (v.x >= ylo && v.x <= yhi && v.y >= zlo && v.y <= zhi) f(j, v.x, v.y);
     }
   }
 }

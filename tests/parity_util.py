@@ -54,8 +54,10 @@ def compare_integer_stages(trk, o, upto=3):
             bad[name] = f"shape {a.shape} vs {b.shape}"
         elif not np.array_equal(a, b):
             bad[name] = int((a != b).sum())
-    for name in ("ys", "zs", "zmin", "zmax"):
-        a = trk.stage_view(name); b = o.get(name)
+    yz = trk.stage_view("yz").reshape(-1, 2)
+    for name, a in (("ys", yz[:, 0]), ("zs", yz[:, 1]), ("zmin", None), ("zmax", None)):
+        a = trk.stage_view(name) if a is None else a
+        b = o.get(name)
         if name in ("zmin", "zmax"):
             keep = o.get("nz") > 0
             a, b = a[keep], b[keep]
@@ -80,7 +82,11 @@ def compare_tracklets(trk, o):
     """S4 per seed: hit tables bit-exact?  parameters / covariance relative error."""
     R = trk.params["n_rows"]
     res = {}
-    hit_g = trk.stage_view("t_hit").reshape(-1, R); hit_o = o.get("t_hit").reshape(-1, R)
+    hit_g = trk.stage_view("t_hit").reshape(-1, R).copy(); hit_o = o.get("t_hit").reshape(-1, R)
+    # the CUDA table is defined on [t_first_row, t_last_row] only (tpc_tracker.h); the oracle's holds -1 outside
+    rows = np.arange(R)[None, :]
+    outside = (rows < trk.stage_view("t_first_row")[:, None]) | (rows > trk.stage_view("t_last_row")[:, None])
+    hit_g[outside] = -1
     res["n_seeds"] = (hit_g.shape[0], hit_o.shape[0])
     if hit_g.shape != hit_o.shape:
         res["hit_mismatch_seeds"] = -1
