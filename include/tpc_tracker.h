@@ -80,7 +80,8 @@ typedef struct {
  * finished the call.  `x` may be NULL and is not read: the tracker uses row_x[row] (pad-row centre).
  * `z` is the pseudo-z in cm computed with vertex time 0 (continuous readout).
  * Preconditions: coordinates finite; 0 <= n <= max_clusters; DEVICE arrays aligned like fresh
- * allocations (sector to 4 bytes, z to 16 bytes - the kernels use vector loads), else INVALID_ARG. */
+ * allocations (sector and row to 4 bytes, y and z to 16 bytes - the kernels use vector loads), else
+ * INVALID_ARG. */
 typedef struct {
   int64_t n;
   const uint8_t* sector; /* [n] */

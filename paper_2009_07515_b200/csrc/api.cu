@@ -63,7 +63,8 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   c.zmin_key = cv.take<int>(S); c.zmax_key = cv.take<int>(S);
   c.zmin = cv.take<float>(S); c.zmax = cv.take<float>(S); c.nz = cv.take<int>(S);
   c.bin_base = cv.take<int>(SR + 1); c.row_start = cv.take<int>(SR + 1);
-  c.gbin = cv.take<int>(N); c.tmp_idx = cv.take<int>(N);
+  c.sr_count = cv.take<int>(SR); c.sr_cursor = cv.take<int>(SR);
+  c.rec = cv.take<float4>(N);
   c.bins = cv.take<int>(NB + 2 + 8);
   c.perm = cv.take<int>(N); c.yz = cv.take<float2>(N); c.srow = cv.take<uint16_t>(N);
   size_t max_scan = N > NB + 2 ? N : NB + 2;
@@ -240,7 +241,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tr
   if (in->n < 0 || (in->n > 0 && (!in->sector || !in->row || !in->y || !in->z))) return TPC_ERR_INVALID_ARG;
   if (in->n > t->max_clusters || out->max_tracks > t->max_tracks || out->max_track_clusters > t->max_track_clusters)
     return TPC_ERR_CAPACITY;
-  if (!aligned(in->sector, 4) || !aligned(in->z, 16) || !aligned(in->y, 4)) return TPC_ERR_INVALID_ARG;
+  if (!aligned(in->sector, 4) || !aligned(in->row, 4) || !aligned(in->z, 16) || !aligned(in->y, 16)) return TPC_ERR_INVALID_ARG;
   return run_device(t, in, to_out(out), static_cast<cudaStream_t>(cuda_stream));
 }
 

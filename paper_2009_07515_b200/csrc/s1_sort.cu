@@ -1,16 +1,19 @@
 // S1 - per-sector, per-row cluster sort and 2-D (y,z) grid binning (BASELINE.json north_star (1);
-// DESIGN.md section 3.1).  Counting sort over the global bin id:
-//   k_zrange   per-sector exact min/max of z (block-local smem reduction on order-preserving keys)
-//   k_tables   nz_s, bin_base[(s,r)], N_b                                   (one block)
-//   k_zero     bins[0 .. N_b+2) = 0
-//   k_count    gbin[i]; histogram into bins[gbin+2]
-//   scan       inclusive: bins[g+1] = first position of bin g
-//   k_scatter  pos = bins[gbin+1]++  -> tmp_idx[pos] = i   (arrival order inside a bin is arbitrary;
-//              afterwards bins[0..N_b] is exactly the CSR bin_start)
-//   k_place    stable fix-up: rank of i among the indices of its bin, final position = start + rank;
-//              writes perm, ys, zs, srow                   (bins hold ~1-3 clusters)
-//   k_rowstart row_start[sr] = bin_start[bin_base[sr]]
+// DESIGN.md section 3.1).  Two-level counting sort whose random accesses stay inside L2:
+//   k_zrange_count  one streaming pass over (sector,row,z): exact per-sector min/max of z and the
+//                   number of clusters per (sector,row)               (smem reductions, then atomics)
+//   k_tables        nz_s, bin_base[(s,r)], N_b, row_start = exclusive scan of the (s,r) counts   (one block)
+//   k_partition     streaming pass over the input: every cluster goes to the bucket of its
+//                   (sector,row) as one 16-byte record (y, z, input index, -) - arrival order; the
+//                   5472 bucket heads live in L2, which merges the 16-byte stores into full lines
+//   k_binsort       one CTA per (sector,row) bucket (~17 k clusters, a few 10 k bins: L2 resident):
+//                   zero its bins, histogram (the atomic returns the arrival rank inside the bin),
+//                   CTA-wide exclusive scan -> CSR bin_start (the bucket's base is row_start, so no
+//                   device-wide scan), scatter perm / (y,z) / srow, then a stable fix-up that orders
+//                   the clusters of every multiply-occupied bin by input index
 // The result equals std::stable_sort by (sector,row,bin) whatever order the atomics resolved in.
+// (Round 1a-c used one device-wide counting sort over the ~N global bins: every one of its ~8 accesses
+// per cluster was a random 32-byte DRAM sector; 15.1 ms on cfg5, see profiles/.)
 #include "tpc_internal.cuh"
 #include "../../include/tpc_tracker.h"
 
@@ -18,62 +21,100 @@ namespace tpc {
 namespace {
 
 constexpr int kThreads = 256;
+constexpr int kHistMaxSR = 12288;   // (sector,row) histogram kept in shared memory up to this many buckets (48 KB)
 
 __global__ void __launch_bounds__(256) k_reset(Ctx c) {
-  const int i = threadIdx.x;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < c.S) { c.zmin_key[i] = 0x7FFFFFFF; c.zmax_key[i] = (int)0x80000000; }
+  for (int j = i; j < c.SR; j += gridDim.x * blockDim.x) c.sr_count[j] = 0;
   if (i == 0) {
     Counters z = {};
     *c.cnt = z;
   }
 }
 
-// ---------------------------------------------------------------------------------- z range
-__global__ void __launch_bounds__(kThreads) k_zrange(Ctx c) {
+// ---------------------------------------------------------------------------------- z range + (s,r) counts
+__global__ void __launch_bounds__(kThreads) k_zrange_count(Ctx c, int use_smem_hist) {
+  extern __shared__ int s_hist[];                 // [SR] when use_smem_hist
   __shared__ int smin[kMaxRows], smax[kMaxRows];
   for (int i = threadIdx.x; i < c.S; i += blockDim.x) { smin[i] = 0x7FFFFFFF; smax[i] = (int)0x80000000; }
+  if (use_smem_hist)
+    for (int i = threadIdx.x; i < c.SR; i += blockDim.x) s_hist[i] = 0;
   __syncthreads();
   bool bad = false;
   const long long n = c.n;
-  // 4 clusters per thread per step: one 32-bit load of the sector bytes, one float4 of z
+  auto one = [&](int s, int r, float z) {
+    if (s >= c.S || r >= c.R) { bad = true; return; }
+    const int key = float_key(z);
+    if (key < smin[s]) atomicMin(&smin[s], key);
+    if (key > smax[s]) atomicMax(&smax[s], key);
+    if (use_smem_hist) atomicAdd(&s_hist[s * c.R + r], 1);
+    else atomicAdd(c.sr_count + s * c.R + r, 1);
+  };
+  // 4 clusters per thread per step: one 32-bit load of the sector bytes, one of the row bytes, one float4 of z
   const long long n4 = n >> 2;
   const uint32_t* sec4 = reinterpret_cast<const uint32_t*>(c.in_sector);
+  const uint32_t* row4 = reinterpret_cast<const uint32_t*>(c.in_row);
   const float4* z4 = reinterpret_cast<const float4*>(c.in_z);
   for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n4; q += (long long)gridDim.x * blockDim.x) {
-    const uint32_t sw = __ldg(sec4 + q);
+    const uint32_t sw = __ldg(sec4 + q), rw = __ldg(row4 + q);
     const float4 zv = __ldg(z4 + q);
-    const float zz[4] = {zv.x, zv.y, zv.z, zv.w};
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const int s = (sw >> (8 * k)) & 0xFF;
-      if (s >= c.S) { bad = true; continue; }
-      const int key = float_key(zz[k]);
-      if (key < smin[s]) atomicMin(&smin[s], key);
-      if (key > smax[s]) atomicMax(&smax[s], key);
-    }
+    one(sw & 0xFF, rw & 0xFF, zv.x);
+    one((sw >> 8) & 0xFF, (rw >> 8) & 0xFF, zv.y);
+    one((sw >> 16) & 0xFF, (rw >> 16) & 0xFF, zv.z);
+    one(sw >> 24, rw >> 24, zv.w);
   }
   if (blockIdx.x == 0 && threadIdx.x < (int)(n & 3)) {   // ragged tail
     const long long i = (n4 << 2) + threadIdx.x;
-    const int s = c.in_sector[i];
-    if (s >= c.S) bad = true;
-    else {
-      const int key = float_key(c.in_z[i]);
-      atomicMin(&smin[s], key);
-      atomicMax(&smax[s], key);
-    }
+    one(c.in_sector[i], c.in_row[i], c.in_z[i]);
   }
   __syncthreads();
   for (int i = threadIdx.x; i < c.S; i += blockDim.x) {
     if (smin[i] != 0x7FFFFFFF) atomicMin(&c.zmin_key[i], smin[i]);
     if (smax[i] != (int)0x80000000) atomicMax(&c.zmax_key[i], smax[i]);
   }
+  if (use_smem_hist)
+    for (int i = threadIdx.x; i < c.SR; i += blockDim.x) {
+      const int v = s_hist[i];
+      if (v) atomicAdd(c.sr_count + i, v);
+    }
   if (bad) atomicOr(&c.cnt->status, (int)TPC_STATUS_BAD_CLUSTER);
 }
 
 // ---------------------------------------------------------------------------------- tables
+// exclusive prefix of `v` over the block (any blockDim <= 1024); *total = block sum.  smem: 33 ints.
+__device__ __forceinline__ int block_exclusive(int v, int* smem, int* total) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  int inc = v;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int o = __shfl_up_sync(0xffffffffu, inc, d);
+    if (lane >= d) inc += o;
+  }
+  if (lane == 31) smem[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    const int s = lane < nw ? smem[lane] : 0;
+    int si = s;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int o = __shfl_up_sync(0xffffffffu, si, d);
+      if (lane >= d) si += o;
+    }
+    smem[lane] = si - s;                       // exclusive warp offsets
+    if (lane == 31) smem[32] = si;
+  }
+  __syncthreads();
+  const int r = smem[w] + inc - v;
+  *total = smem[32];
+  __syncthreads();
+  return r;
+}
+
 __global__ void __launch_bounds__(1024) k_tables(Ctx c) {
   __shared__ long long sbase[kMaxRows + 1];
   __shared__ int snz[kMaxRows];
+  __shared__ int sscan[33];
   if (threadIdx.x == 0) {
     long long acc = 0;
     for (int s = 0; s < c.S; ++s) {
@@ -107,72 +148,140 @@ __global__ void __launch_bounds__(1024) k_tables(Ctx c) {
     }
     c.bin_base[sr] = v;
   }
-}
-
-__global__ void __launch_bounds__(kThreads) k_zero_bins(Ctx c) {
-  if (c.cnt->status) return;
-  const long long m = (long long)c.cnt->n_bins + 2;
-  const long long m4 = m >> 2;
-  int4* b4 = reinterpret_cast<int4*>(c.bins);
-  for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < m4; q += (long long)gridDim.x * blockDim.x)
-    b4[q] = make_int4(0, 0, 0, 0);
-  if (blockIdx.x == 0 && threadIdx.x < (int)(m & 3)) c.bins[(m4 << 2) + threadIdx.x] = 0;
-}
-
-// ---------------------------------------------------------------------------------- count
-__device__ __forceinline__ int global_bin(const Ctx& c, int s, int r, float y, float z) {
-  const RowTab& t = c.rowtab[r];
-  const int ny = __ldg(&t.ny);
-  const int iy = floor_clamp((y + __ldg(&t.ymax)) * c.inv_cy, ny - 1);
-  const int iz = floor_clamp((z - __ldg(c.zmin + s)) * c.inv_cz, __ldg(c.nz + s) - 1);
-  return __ldg(c.bin_base + s * c.R + r) + iz * ny + iy;
-}
-
-__global__ void __launch_bounds__(kThreads) k_count(Ctx c) {
-  if (c.cnt->status) return;
-  bool bad = false;
-  const long long n = c.n;
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-    const int s = __ldg(c.in_sector + i), r = __ldg(c.in_row + i);
-    if (s >= c.S || r >= c.R) { bad = true; c.gbin[i] = -1; continue; }
-    const int g = global_bin(c, s, r, __ldg(c.in_y + i), __ldg(c.in_z + i));
-    c.gbin[i] = g;
-    atomicAdd(c.bins + g + 2, 1);
+  // row_start = exclusive scan of the (sector,row) counts; the partition cursors start there
+  const bool dead = *reinterpret_cast<volatile int*>(&c.cnt->status) != 0;   // set before the barrier above (thread 0) or by k_zrange_count
+  int carry = 0;
+  for (int b = 0; b < c.SR; b += blockDim.x) {
+    const int i = b + threadIdx.x;
+    const int v = (i < c.SR && !dead) ? c.sr_count[i] : 0;
+    int total;
+    const int ex = block_exclusive(v, sscan, &total);
+    if (i < c.SR) { c.row_start[i] = carry + ex; c.sr_cursor[i] = carry + ex; }
+    carry += total;
   }
-  if (bad) atomicOr(&c.cnt->status, (int)TPC_STATUS_BAD_CLUSTER);
-}
-
-__global__ void __launch_bounds__(kThreads) k_scatter(Ctx c) {
-  if (c.cnt->status) return;
-  const long long n = c.n;
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-    const int g = __ldg(c.gbin + i);
-    const int pos = atomicAdd(c.bins + g + 1, 1);
-    c.tmp_idx[pos] = (int)i;
+  if (threadIdx.x == 0) {
+    c.row_start[c.SR] = carry;
+    if (ok) c.bins[(int)sbase[c.S]] = carry;   // bin_start[N_b] = N
   }
 }
 
-// stable fix-up + gather of the sorted payload
-__global__ void __launch_bounds__(kThreads) k_place(Ctx c) {
+// ---------------------------------------------------------------------------------- partition by (sector,row)
+__global__ void __launch_bounds__(kThreads) k_partition(Ctx c) {
   if (c.cnt->status) return;
   const long long n = c.n;
-  for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (long long)gridDim.x * blockDim.x) {
-    const int i = __ldg(c.tmp_idx + p);
-    const int g = __ldg(c.gbin + i);
-    const int bs = c.bins[g], be = c.bins[g + 1];
-    int rank = 0;
-    for (int j = bs; j < be; ++j) rank += (__ldg(c.tmp_idx + j) < i);
-    const int fp = bs + rank;
-    c.perm[fp] = i;
-    c.yz[fp] = make_float2(__ldg(c.in_y + i), __ldg(c.in_z + i));
-    c.srow[fp] = (uint16_t)((int)__ldg(c.in_sector + i) * c.R + (int)__ldg(c.in_row + i));
+  auto one = [&](int s, int r, float y, float z, long long i) {
+    const int pos = atomicAdd(c.sr_cursor + s * c.R + r, 1);
+    c.rec[pos] = make_float4(y, z, __int_as_float((int)i), 0.0f);
+  };
+  const long long n4 = n >> 2;
+  const uint32_t* sec4 = reinterpret_cast<const uint32_t*>(c.in_sector);
+  const uint32_t* row4 = reinterpret_cast<const uint32_t*>(c.in_row);
+  const float4* y4 = reinterpret_cast<const float4*>(c.in_y);
+  const float4* z4 = reinterpret_cast<const float4*>(c.in_z);
+  for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n4; q += (long long)gridDim.x * blockDim.x) {
+    const uint32_t sw = __ldg(sec4 + q), rw = __ldg(row4 + q);
+    const float4 yv = __ldg(y4 + q), zv = __ldg(z4 + q);
+    const long long i = q << 2;
+    one(sw & 0xFF, rw & 0xFF, yv.x, zv.x, i);
+    one((sw >> 8) & 0xFF, (rw >> 8) & 0xFF, yv.y, zv.y, i + 1);
+    one((sw >> 16) & 0xFF, (rw >> 16) & 0xFF, yv.z, zv.z, i + 2);
+    one(sw >> 24, rw >> 24, yv.w, zv.w, i + 3);
+  }
+  if (blockIdx.x == 0 && threadIdx.x < (int)(n & 3)) {
+    const long long i = (n4 << 2) + threadIdx.x;
+    one(c.in_sector[i], c.in_row[i], c.in_y[i], c.in_z[i], i);
   }
 }
 
-__global__ void __launch_bounds__(kThreads) k_rowstart(Ctx c) {
-  const bool dead = c.cnt->status != 0;
-  for (int sr = blockIdx.x * blockDim.x + threadIdx.x; sr <= c.SR; sr += gridDim.x * blockDim.x)
-    c.row_start[sr] = dead ? 0 : c.bins[c.bin_base[sr]];
+// ---------------------------------------------------------------------------------- bin sort inside a (sector,row) bucket
+// One CTA per bucket, buckets handed out by a ticket.  Everything the CTA touches at random (its bins,
+// its slice of rec / perm / yz) was written moments ago and sits in L2; DRAM sees each array once.
+// Reads of data that atomics or other threads of the CTA wrote go through L2 (__ldcg), never a stale L1 line.
+template <int kT, int kMinCtas>
+__global__ void __launch_bounds__(kT, kMinCtas) k_binsort(Ctx c) {
+  __shared__ int s_scan[33];
+  __shared__ int s_sr;
+  if (c.cnt->status) return;
+  const int tid = threadIdx.x;
+  for (;;) {
+    if (tid == 0) s_sr = atomicAdd(&c.cnt->s1_ticket, 1);
+    __syncthreads();
+    const int sr = s_sr;
+    __syncthreads();
+    if (sr >= c.SR) break;
+    const int b0 = __ldg(c.bin_base + sr), nb = __ldg(c.bin_base + sr + 1) - b0;
+    if (nb == 0) continue;                        // empty sector
+    const int p0 = __ldg(c.row_start + sr), p1 = __ldg(c.row_start + sr + 1);
+    const int s = sr / c.R, r = sr - s * c.R;
+    const int ny = __ldg(&c.rowtab[r].ny), nzm1 = __ldg(c.nz + s) - 1;
+    const float ymax = __ldg(&c.rowtab[r].ymax), zmin = __ldg(c.zmin + s);
+    int* __restrict__ bins = c.bins + b0;
+    auto local_bin = [&](float y, float z) {     // DESIGN.md section 3.1 step 3
+      const int iy = floor_clamp((y + ymax) * c.inv_cy, ny - 1);
+      const int iz = floor_clamp((z - zmin) * c.inv_cz, nzm1);
+      return iz * ny + iy;
+    };
+
+    for (int j = tid; j < nb; j += kT) bins[j] = 0;
+    __syncthreads();
+
+    // histogram; the atomic's return value is the cluster's arrival rank inside its bin
+#pragma unroll 4
+    for (int i = p0 + tid; i < p1; i += kT) {
+      const float4 v = __ldcg(c.rec + i);
+      const int a = atomicAdd(bins + local_bin(v.x, v.y), 1);
+      reinterpret_cast<int*>(c.rec + i)[3] = a;
+    }
+    __syncthreads();
+
+    // exclusive scan of the bucket's bins, starting at row_start: bins[] becomes the CSR bin_start
+    int carry = p0;
+    for (int base = 0; base < nb; base += kT * 4) {
+      const int j = base + tid * 4;
+      int x[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) x[k] = (j + k < nb) ? __ldcg(bins + j + k) : 0;
+      int total;
+      int o = carry + block_exclusive((x[0] + x[1]) + (x[2] + x[3]), s_scan, &total);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        if (j + k < nb) bins[j + k] = o;
+        o += x[k];
+      }
+      carry += total;
+    }
+    __syncthreads();
+
+    // scatter (arrival order inside a bin)
+#pragma unroll 4
+    for (int i = p0 + tid; i < p1; i += kT) {
+      const float4 v = __ldcg(c.rec + i);
+      const int pos = __ldcg(bins + local_bin(v.x, v.y)) + __float_as_int(v.w);
+      c.perm[pos] = __float_as_int(v.z);
+      c.yz[pos] = make_float2(v.x, v.y);
+      c.srow[pos] = (uint16_t)sr;
+    }
+    __syncthreads();
+
+    // stable fix-up: order the clusters of a multiply-occupied bin by input index (bins hold ~1-3 clusters)
+    for (int j = tid; j < nb; j += kT) {
+      const int bs = __ldcg(bins + j), be = (j + 1 < nb) ? __ldcg(bins + j + 1) : p1;
+      if (be - bs < 2) continue;
+      for (int a = bs + 1; a < be; ++a) {          // insertion sort on (perm, yz)
+        const int pa = __ldcg(c.perm + a);
+        const float2 va = __ldcg(c.yz + a);
+        int b = a - 1;
+        while (b >= bs) {
+          const int pb = __ldcg(c.perm + b);
+          if (pb < pa) break;
+          c.perm[b + 1] = pb;
+          c.yz[b + 1] = __ldcg(c.yz + b);
+          --b;
+        }
+        if (b + 1 != a) { c.perm[b + 1] = pa; c.yz[b + 1] = va; }
+      }
+    }
+  }
 }
 
 inline unsigned grid_for(long long n, int per_block, int n_sms, int waves) {
@@ -187,21 +296,19 @@ inline unsigned grid_for(long long n, int per_block, int n_sms, int waves) {
 
 int launches_reset() { return 1; }
 int launch_reset(const Ctx& c, cudaStream_t st) {
-  k_reset<<<1, 256, 0, st>>>(c);
+  k_reset<<<(c.SR + 255) / 256 < 64 ? (c.SR + 255) / 256 : 64, 256, 0, st>>>(c);
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 
-int launches_s1() { return 7 + 3; }
+int launches_s1() { return 4; }
 int launch_s1(const Ctx& c, cudaStream_t st) {
-  const unsigned g = grid_for(c.n, kThreads, c.n_sms, 8);
-  k_zrange<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 4), kThreads, 0, st>>>(c);
+  const int smem_hist = c.SR <= kHistMaxSR;
+  k_zrange_count<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 8), kThreads, smem_hist ? c.SR * sizeof(int) : 0, st>>>(c, smem_hist);
   k_tables<<<1, 1024, 0, st>>>(c);
-  k_zero_bins<<<grid_for((long long)c.max_bins / 4 + 1, kThreads, c.n_sms, 8), kThreads, 0, st>>>(c);
-  k_count<<<g, kThreads, 0, st>>>(c);
-  if (launch_scan_inclusive(c.bins, &c.cnt->n_bins, 2, (long long)c.max_bins + 2, c.tile_sums, nullptr, c.n_sms, st)) return -1;
-  k_scatter<<<g, kThreads, 0, st>>>(c);
-  k_place<<<g, kThreads, 0, st>>>(c);
-  k_rowstart<<<grid_for(c.SR + 1, kThreads, c.n_sms, 1), kThreads, 0, st>>>(c);
+  k_partition<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 8), kThreads, 0, st>>>(c);
+  // big buckets: 1024 threads per bucket, two buckets per SM in flight; small ones: 256 threads, eight per SM
+  if ((long long)c.n >= 2048LL * c.SR) k_binsort<1024, 2><<<grid_for(c.SR, 1, c.n_sms, 2), 1024, 0, st>>>(c);
+  else k_binsort<256, 8><<<grid_for(c.SR, 1, c.n_sms, 8), 256, 0, st>>>(c);
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 

@@ -38,7 +38,8 @@ struct Counters {
   unsigned long long kf_steps;
   unsigned long long n_hits;
   int s4_ticket;          // dynamic work counter of the S4 persistent kernel
-  int pad[3];
+  int s1_ticket;          // dynamic (sector,row) bucket counter of the S1 bin-sort kernel
+  int pad[2];
 };
 
 // Everything a kernel needs, passed by value (a few hundred bytes).
@@ -61,8 +62,9 @@ struct Ctx {
   float* zmin; float* zmax; int* nz;  // [S]
   int* bin_base;                      // [SR+1]
   int* row_start;                     // [SR+1]
-  int* gbin;                          // [n] global bin of the input cluster
-  int* tmp_idx;                       // [n] input indices grouped by bin, arrival order
+  int* sr_count;                      // [SR] clusters per (sector,row)
+  int* sr_cursor;                     // [SR] write cursor of the (sector,row) bucket during the partition
+  float4* rec;                        // [n] clusters grouped by (sector,row), arrival order: (y, z, input index, rank in bin)
   int* bins;                          // [max_bins+2]; after S1 bins[0..N_b] is the CSR bin_start
   int* perm; float2* yz; uint16_t* srow;              // [n] sorted: input index, (y,z) pair, sector*R+row
   int* tile_sums;                     // scan scratch
