@@ -40,6 +40,8 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg5", help="cfg1..cfg5 (BASELINE.json configs[0..4]); cfg5 = the metric's")
     ap.add_argument("--collisions", type=int, default=0, help="override n_collisions (debug; 0 = the config's own)")
+    ap.add_argument("--cell-y", type=float, default=0.0, help="override the grid cell along y, cm (debug; 0 = tpc_synth.choose_cell)")
+    ap.add_argument("--cell-z", type=float, default=0.0, help="override the grid cell along z, cm (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -196,6 +198,10 @@ def run_ours(args):
     tf = make_timeframe(args, rank)
     t_gen = time.perf_counter() - t_gen
     P = default_params(tf)
+    if args.cell_y > 0:
+        P["cell_y"] = np.float32(args.cell_y)
+    if args.cell_z > 0:
+        P["cell_z"] = np.float32(args.cell_z)
     caps = tpc.suggest_capacities(tf.n, P)
     caps["max_bins"] = tpc.max_bins_bound(tf.sector, tf.z, P)
 
@@ -328,7 +334,7 @@ def run_ours(args):
         "config": {"workload": tf.name, "n_clusters_per_gpu": tf.n, "n_clusters_total": n_total,
                    "parallelism": "replicas (one time frame per GPU, no collective)" if world > 1 else "single GPU",
                    "l2": "inputs larger than L2" if tf.n * 10 > 126e6 else "inputs fit L2 (small config)",
-                   "cell_cm": float(P["cell_y"]), "generate_s": round(t_gen, 1),
+                   "cell_cm": [float(P["cell_y"]), float(P["cell_z"])], "generate_s": round(t_gen, 1),
                    "workspace_GB": round(trk.workspace_bytes / 1e9, 2)},
         "counters": {kk: int(v) for kk, v in k.items()},
         "roofline": roofline,
