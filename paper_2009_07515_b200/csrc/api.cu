@@ -72,7 +72,7 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   c.tile_sums = cv.take<int>(max_scan / kScanTile + 2);
   c.link_up_raw = cv.take<int>(N); c.link_dn_raw = cv.take<int>(N);
   c.link_up = cv.take<int>(N); c.link_dn = cv.take<int>(N);
-  c.flag = cv.take<int>(N); c.flag_scan = cv.take<int>(N);
+  c.flag_scan = cv.take<int>(N);
   c.seed_head = cv.take<int>(K); c.seed_len = cv.take<int>(K);
   c.t_hit = cv.take<int>(K * R);
   c.t_first_row = cv.take<int>(K); c.t_last_row = cv.take<int>(K); c.t_n_hits = cv.take<int>(K);
@@ -81,6 +81,8 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   c.owner = cv.take<unsigned long long>(N);
   c.k_owned = cv.take<int>(K); c.k_first = cv.take<int>(K); c.k_last = cv.take<int>(K);
   c.surv_scan = cv.take<int>(K); c.owned_scan = cv.take<int>(K);
+  c.mask_words = (R + 31) / 32;
+  c.own_mask = cv.take<unsigned>(K * (size_t)c.mask_words);
   if (t->host_io) {
     const size_t T = (size_t)t->max_tracks, TC = (size_t)t->max_track_clusters;
     t->st_sector = cv.take<uint8_t>(N); t->st_row = cv.take<uint8_t>(N);

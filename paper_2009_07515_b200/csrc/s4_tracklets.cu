@@ -237,6 +237,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_tracklets(Ctx c) {
         r = cur + 1 + (cl >= __ldg(c.row_start + sR + cur + 2));   // links go up one row or two
         act = true;
       } else {
+        c.seed_len[sd] = nh;                      // end of the chain: every node was absorbed (S3 leaves the count to us)
         phase = kPhaseB; gap = 0;
       }
     }
@@ -292,7 +293,14 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_tracklets(Ctx c) {
       }
       if (stop) {
         if (phase == kPhaseC) done = true;
-        else go_c = true;                         // a failed step of A skips B
+        else {
+          go_c = true;                            // a failed step of A skips B
+          if (phase == kPhaseA) {                 // rare: count the chain nodes the filter did not reach
+            int len = nh;
+            for (int p = nextcl; p >= 0; p = __ldg(link_up + p)) ++len;
+            c.seed_len[sd] = len;
+          }
+        }
       }
     }
 

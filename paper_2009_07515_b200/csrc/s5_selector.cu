@@ -2,11 +2,13 @@
 // clusters.  Every cluster goes to the tracklet with the largest key = (n_hits << 32 | ~tracklet id)
 // among those holding it (u64 atomicMax); a tracklet survives if it still owns min_track_hits
 // clusters.  Tracklet ids, track ids and the CSR offsets are ranks from scans (deterministic).
-//   k_kept       kept flag per seed                      -> scan -> tracklet ids, n_tracklets
 //   k_owner      owner[cluster] = max key                 (one warp per tracklet, coalesced hit rows)
-//   k_owned      owned count, first/last owned row        -> scans -> track ids, CSR starts
+//   k_owned      owned count, first/last owned row, ownership bit mask per tracklet
+//                -> scans -> track ids, CSR starts
 //   k_finalize   capacity checks, n_tracks
-//   k_write      tracks SoA, trk_cl_idx (input indices, ascending row), cluster_track
+//   k_write      tracks SoA, trk_cl_idx (input indices, ascending row), cluster_track  (reads the masks, not owner[])
+//   k_kept / scan / k_tracklet_ids   tracklet ids for the debug view (off the critical path: the key carries the
+//                seed id, which orders kept tracklets exactly as their tracklet id would)
 #include "tpc_internal.cuh"
 #include "../../include/tpc_tracker.h"
 
@@ -28,6 +30,8 @@ __global__ void __launch_bounds__(kThreads) k_init_out(Ctx c, OutPtrs o) {
   }
 }
 
+// kept flag per seed + tracklet ids: only the debug view / the n_tracklets counter need them (the ownership key uses the
+// seed id, which orders kept tracklets exactly like their tracklet id does)
 __global__ void __launch_bounds__(kThreads) k_kept(Ctx c) {
   if (c.cnt->status) return;
   const int ns = c.cnt->n_seeds;
@@ -35,50 +39,73 @@ __global__ void __launch_bounds__(kThreads) k_kept(Ctx c) {
     c.kept_scan[sd] = c.t_n_hits[sd] >= c.min_tracklet_hits;
 }
 
+__global__ void __launch_bounds__(kThreads) k_tracklet_ids(Ctx c) {
+  if (c.cnt->status) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) c.cnt->n_tracklets = 0;
+    return;
+  }
+  const int ns = c.cnt->n_seeds;
+  for (int sd = blockIdx.x * blockDim.x + threadIdx.x; sd < ns; sd += gridDim.x * blockDim.x) {
+    const int inc = c.kept_scan[sd], prev = sd ? c.kept_scan[sd - 1] : 0;
+    c.tracklet_of_seed[sd] = inc != prev ? inc - 1 : -1;
+  }
+}
+
+// The hit tables are read once per pass and never again: streaming loads keep them from evicting the owner[] / perm[]
+// lines of the sector being worked on out of L2.
 __global__ void __launch_bounds__(kThreads) k_owner(Ctx c) {
   if (c.cnt->status) return;
   const int ns = c.cnt->n_seeds, R = c.R;
   const int lane = threadIdx.x & 31;
   const int warps = (gridDim.x * blockDim.x) >> 5;
   for (int sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < ns; sd += warps) {
-    const int inc = c.kept_scan[sd], prev = sd ? c.kept_scan[sd - 1] : 0;
-    const bool kept = inc != prev;
-    if (lane == 0) c.tracklet_of_seed[sd] = kept ? inc - 1 : -1;
-    if (!kept) continue;
-    const unsigned long long key = make_key(c.t_n_hits[sd], inc - 1);
+    const int nh = c.t_n_hits[sd];
+    if (nh < c.min_tracklet_hits) continue;
+    const unsigned long long key = make_key(nh, sd);
     const int* hit = c.t_hit + (size_t)sd * R;
     const int last = c.t_last_row[sd];
     for (int r = c.t_first_row[sd] + lane; r <= last; r += 32) {   // the table is defined on [first_row, last_row] only
-      const int cl = hit[r];
+      const int cl = __ldcs(hit + r);
       if (cl >= 0) atomicMax(c.owner + cl, key);
     }
   }
 }
 
+// owned count, first / last owned row and the ownership bit mask (bit k of word w: row first_row + 32 w + k is owned)
 __global__ void __launch_bounds__(kThreads) k_owned(Ctx c) {
   if (c.cnt->status) return;
   const int ns = c.cnt->n_seeds, R = c.R;
   const int lane = threadIdx.x & 31;
   const int warps = (gridDim.x * blockDim.x) >> 5;
   for (int sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < ns; sd += warps) {
-    const int tid = c.tracklet_of_seed[sd];
+    const int nh = c.t_n_hits[sd];
+    const bool kept = nh >= c.min_tracklet_hits;
     int owned = 0, first = 0x7FFFFFFF, last = -1;
-    if (tid >= 0) {
-      const unsigned long long key = make_key(c.t_n_hits[sd], tid);
+    unsigned mine = 0;                                   // lane w keeps mask word w
+    if (kept) {
+      const unsigned long long key = make_key(nh, sd);
       const int* hit = c.t_hit + (size_t)sd * R;
       const int hi = c.t_last_row[sd];
-      for (int r = c.t_first_row[sd] + lane; r <= hi; r += 32) {
-        const int cl = hit[r];
-        if (cl >= 0 && c.owner[cl] == key) { ++owned; first = min(first, r); last = max(last, r); }
+      int w = 0;
+      for (int rb = c.t_first_row[sd]; rb <= hi; rb += 32, ++w) {
+        const int r = rb + lane;
+        bool own = false;
+        if (r <= hi) {
+          const int cl = __ldcs(hit + r);
+          own = cl >= 0 && c.owner[cl] == key;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, own);
+        if (lane == w) mine = m;
+        if (m) {
+          owned += __popc(m);
+          first = min(first, rb + __ffs(m) - 1);
+          last = rb + 31 - __clz(m);
+        }
       }
     }
-    for (int o = 16; o; o >>= 1) {
-      owned += __shfl_xor_sync(0xffffffffu, owned, o);
-      first = min(first, __shfl_xor_sync(0xffffffffu, first, o));
-      last = max(last, __shfl_xor_sync(0xffffffffu, last, o));
-    }
+    if (lane < c.mask_words) c.own_mask[(size_t)sd * c.mask_words + lane] = mine;
     if (lane == 0) {
-      const bool surv = tid >= 0 && owned >= c.min_track_hits;
+      const bool surv = kept && owned >= c.min_track_hits;
       c.k_owned[sd] = owned; c.k_first[sd] = first; c.k_last[sd] = last;
       c.surv_scan[sd] = surv;
       c.owned_scan[sd] = surv ? owned : 0;
@@ -109,18 +136,13 @@ __global__ void __launch_bounds__(kThreads) k_write(Ctx c, OutPtrs o) {
     const int id = inc - 1;
     const int end = c.owned_scan[sd];
     int off = end - c.k_owned[sd];
-    const unsigned long long key = make_key(c.t_n_hits[sd], c.tracklet_of_seed[sd]);
     const int* hit = c.t_hit + (size_t)sd * R;
     const int hi = c.t_last_row[sd];
-    for (int rb = c.t_first_row[sd]; rb <= hi; rb += 32) {
-      const int r = rb + lane;
-      int cl = -1;
-      if (r <= hi) {
-        cl = hit[r];
-        if (cl >= 0 && c.owner[cl] != key) cl = -1;
-      }
-      const unsigned m = __ballot_sync(0xffffffffu, cl >= 0);
-      if (cl >= 0) {
+    const unsigned* mask = c.own_mask + (size_t)sd * c.mask_words;
+    for (int rb = c.t_first_row[sd]; rb <= hi; rb += 32, ++mask) {
+      const unsigned m = *mask;                          // rows of this chunk the track owns (k_owned)
+      if ((m >> lane) & 1u) {
+        const int cl = __ldcs(hit + rb + lane);
         const int in_idx = c.perm[cl];
         o.trk_cl_idx[off + __popc(m & ((1u << lane) - 1))] = in_idx;
         o.cluster_track[in_idx] = id;
@@ -154,20 +176,22 @@ inline unsigned grid_for(long long n, int per_block, int n_sms, int waves) {
 
 }  // namespace
 
-int launches_s5() { return 6 + 9; }
+int launches_s5() { return 7 + 9; }
 int launch_s5(const Ctx& c, const OutPtrs& o, cudaStream_t st) {
   const unsigned gn = grid_for(c.n, kThreads, c.n_sms, 8);
   const unsigned gs = grid_for(c.max_seeds, kThreads, c.n_sms, 8);          // thread per seed
   const unsigned gw = grid_for((long long)c.max_seeds * 32, kThreads, c.n_sms, 8);   // warp per seed
   k_init_out<<<gn, kThreads, 0, st>>>(c, o);
-  k_kept<<<gs, kThreads, 0, st>>>(c);
-  if (launch_scan_inclusive(c.kept_scan, &c.cnt->n_seeds, 0, c.max_seeds, c.tile_sums, &c.cnt->n_tracklets, c.n_sms, st)) return -1;
   k_owner<<<gw, kThreads, 0, st>>>(c);
   k_owned<<<gw, kThreads, 0, st>>>(c);
   if (launch_scan_inclusive(c.surv_scan, &c.cnt->n_seeds, 0, c.max_seeds, c.tile_sums, &c.cnt->n_tracks, c.n_sms, st)) return -1;
   if (launch_scan_inclusive(c.owned_scan, &c.cnt->n_seeds, 0, c.max_seeds, c.tile_sums, &c.cnt->n_track_clusters, c.n_sms, st)) return -1;
   k_finalize<<<1, 1, 0, st>>>(c, o);
   k_write<<<gw, kThreads, 0, st>>>(c, o);
+  // tracklet ids (debug view, n_tracklets counter): nothing downstream waits for them
+  k_kept<<<gs, kThreads, 0, st>>>(c);
+  if (launch_scan_inclusive(c.kept_scan, &c.cnt->n_seeds, 0, c.max_seeds, c.tile_sums, &c.cnt->n_tracklets, c.n_sms, st)) return -1;
+  k_tracklet_ids<<<gs, kThreads, 0, st>>>(c);
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 

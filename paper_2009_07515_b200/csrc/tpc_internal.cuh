@@ -70,8 +70,7 @@ struct Ctx {
   int* tile_sums;                     // scan scratch
   // S2 / S3
   int* link_up_raw; int* link_dn_raw; int* link_up; int* link_dn;
-  int* flag;                          // [n] S3: chain length at qualifying heads else 0; reused by scans
-  int* flag_scan;                     // [n] inclusive scan of (flag != 0)
+  int* flag_scan;                     // [n] S3: seed bit per sorted position, then its inclusive scan
   int* seed_head; int* seed_len;      // [max_seeds]
   // S4
   int* t_hit;                         // [max_seeds][R]
@@ -83,6 +82,7 @@ struct Ctx {
   unsigned long long* owner;          // [n]
   int* k_owned; int* k_first; int* k_last;   // [max_seeds]
   int* surv_scan; int* owned_scan;    // [max_seeds] inclusive scans
+  unsigned* own_mask; int mask_words; // [max_seeds][mask_words] bit k of word w: row first_row + 32 w + k is owned
   Counters* cnt;
   int n_sms;
 };

@@ -60,7 +60,7 @@ def test_workspace_bytes_is_host_only_and_monotone():
     b = ws(20_000, 20_000, 1000, 1000, 10_000, 0)
     c = ws(10_000, 20_000, 1000, 1000, 10_000, 1)
     assert 0 < a < b and a < c
-    assert a >= 10_000 * (16 + 4 + 8 + 2 + 4 * 4 + 8 + 8)   # rec, perm, yz, srow, four link arrays, flags, owner
+    assert a >= 10_000 * (16 + 4 + 8 + 2 + 4 * 4 + 4 + 8)   # rec, perm, yz, srow, four link arrays, seed bits, owner
     assert ws(0, 20_000, 1000, 1000, 10_000, 0) == 0         # capacities must be >= 1
     # bad geometry is rejected: non-increasing row_x
     Q = dict(P)
