@@ -261,9 +261,12 @@ def generate(rec: dict, geometry: Geometry | None = None, device: str = "cpu") -
 
 
 # --------------------------------------------------------------- harness rules
-def choose_cell(tf: TimeFrame, lo: float = 2.0, hi: float = 16.0) -> float:
+def choose_cell(tf: TimeFrame, lo: float = 2.0, hi: float = 16.0, scale: float = 0.5) -> float:
     """Grid cell size handed to BOTH the oracle and the CUDA path (neither derives it):
-    clamp(sqrt(mean over non-empty (sector,row) of area / n_clusters), lo, hi), in double."""
+    clamp(scale * sqrt(mean over non-empty (sector,row) of area / n_clusters), lo, hi), in double.
+    The cell only changes how many clusters a window query has to look at, never which ones it accepts
+    (DESIGN.md 3.1): scale = 0.5 (a quarter of a cluster per bin on average) was the fastest of a sweep on cfg5
+    (profiles/r01b_summary.md)."""
     g = tf.geometry
     if tf.n == 0:
         return lo
@@ -277,7 +280,7 @@ def choose_cell(tf: TimeFrame, lo: float = 2.0, hi: float = 16.0) -> float:
     area = (zspan[:, None] * width[None, :]).reshape(-1)
     nz = cnt > 0
     per = area[nz] / cnt[nz]
-    return float(min(hi, max(lo, math.sqrt(float(per.mean())))))
+    return float(min(hi, max(lo, scale * math.sqrt(float(per.mean())))))
 
 
 def default_params(tf: TimeFrame, cell: float | None = None) -> dict:
