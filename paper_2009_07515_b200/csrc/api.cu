@@ -70,8 +70,12 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   size_t max_scan = N > NB + 2 ? N : NB + 2;
   if (K > max_scan) max_scan = K;
   c.tile_sums = cv.take<int>(max_scan / kScanTile + 2);
-  c.link_up_raw = cv.take<int>(N); c.link_dn_raw = cv.take<int>(N);
-  c.link_up = cv.take<int>(N); c.link_dn = cv.take<int>(N);
+  // S1's second record buffer and the four link arrays of S2/S3 are never live together: one 16 N byte slice serves both
+  c.rec2 = cv.take<float4>(N);
+  c.link_up_raw = base ? reinterpret_cast<int*>(c.rec2) : nullptr;
+  c.link_dn_raw = base ? c.link_up_raw + N : nullptr;
+  c.link_up = base ? c.link_dn_raw + N : nullptr;
+  c.link_dn = base ? c.link_up + N : nullptr;
   c.flag_scan = cv.take<int>(N);
   c.seed_head = cv.take<int>(K); c.seed_len = cv.take<int>(K);
   c.t_hit = cv.take<int>(K * R);

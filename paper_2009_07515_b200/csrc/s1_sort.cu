@@ -9,8 +9,8 @@
 //   k_binsort       one CTA per (sector,row) bucket (~17 k clusters, a few 10 k bins: L2 resident):
 //                   zero its bins, histogram (the atomic returns the arrival rank inside the bin),
 //                   CTA-wide exclusive scan -> CSR bin_start (the bucket's base is row_start, so no
-//                   device-wide scan), scatter perm / (y,z) / srow, then a stable fix-up that orders
-//                   the clusters of every multiply-occupied bin by input index
+//                   device-wide scan), scatter perm / (y,z) / srow; the clusters of a multiply-occupied
+//                   bin take their stable rank (members with a smaller input index) in a final pass
 // The result equals std::stable_sort by (sector,row,bin) whatever order the atomics resolved in.
 // (Round 1a-c used one device-wide counting sort over the ~N global bins: every one of its ~8 accesses
 // per cluster was a random 32-byte DRAM sector; 15.1 ms on cfg5, see profiles/.)
@@ -194,93 +194,234 @@ __global__ void __launch_bounds__(kThreads) k_partition(Ctx c) {
 }
 
 // ---------------------------------------------------------------------------------- bin sort inside a (sector,row) bucket
-// One CTA per bucket, buckets handed out by a ticket.  Everything the CTA touches at random (its bins,
-// its slice of rec / perm / yz) was written moments ago and sits in L2; DRAM sees each array once.
+// One CTA per bucket, buckets handed out by a ticket.
+//
+// Slab path (the normal one).  A bucket of cfg5 holds ~17 k clusters and ~10^5 bins: with two buckets per SM in
+// flight the bins + records of all of them (~1 MB each) do not fit L2, and every random access to them was a DRAM
+// sector (19 GB of DRAM traffic for 4 GB of useful bytes, profiles/).  So the CTA first splits its bucket into z-slabs
+// of whole bin rows (a counting sort over <= 64 slab ids, shared-memory counters, records copied rec -> rec2), then
+// bin-sorts one slab at a time ENTIRELY in shared memory: slab histogram (shared atomics), exclusive scan, CSR
+// written out once with coalesced stores, stable rank inside multiply-occupied bins from a shared-memory table of
+// input indices.  Global memory sees: rec read twice, rec2 written and read (sequentially, per slab), outputs and
+// bin_start written once.
+// Global path (fallback when a slab's bins or clusters do not fit the shared-memory tables): the same steps on
+// the whole bucket with the bins in global memory.
 // Reads of data that atomics or other threads of the CTA wrote go through L2 (__ldcg), never a stale L1 line.
-template <int kT, int kMinCtas>
-__global__ void __launch_bounds__(kT, kMinCtas) k_binsort(Ctx c) {
-  __shared__ int s_scan[33];
-  __shared__ int s_sr;
-  if (c.cnt->status) return;
+constexpr int kMaxSlabs = 64;
+constexpr int kSlabTarget = 1024;     // clusters per slab aimed at
+constexpr int kSlabBinCap = 12288;    // bins of one slab held in shared memory (48 KB)
+constexpr int kSlabCluCap = 4096;     // clusters of one slab whose input indices fit the shared-memory table (16 KB)
+
+struct BucketGeom {
+  int sr, b0, nb, p0, p1, ny, nzm1;
+  float ymax, zmin;
+};
+
+__device__ __forceinline__ int local_bin_of(const Ctx& c, const BucketGeom& g, float y, float z) {   // DESIGN.md 3.1 step 3
+  const int iy = floor_clamp((y + g.ymax) * c.inv_cy, g.ny - 1);
+  const int iz = floor_clamp((z - g.zmin) * c.inv_cz, g.nzm1);
+  return iz * g.ny + iy;
+}
+
+template <int kT>
+__device__ void bucket_global(const Ctx& c, const BucketGeom& g, int* s_scan) {
   const int tid = threadIdx.x;
-  for (;;) {
-    if (tid == 0) s_sr = atomicAdd(&c.cnt->s1_ticket, 1);
-    __syncthreads();
-    const int sr = s_sr;
-    __syncthreads();
-    if (sr >= c.SR) break;
-    const int b0 = __ldg(c.bin_base + sr), nb = __ldg(c.bin_base + sr + 1) - b0;
-    if (nb == 0) continue;                        // empty sector
-    const int p0 = __ldg(c.row_start + sr), p1 = __ldg(c.row_start + sr + 1);
-    const int s = sr / c.R, r = sr - s * c.R;
-    const int ny = __ldg(&c.rowtab[r].ny), nzm1 = __ldg(c.nz + s) - 1;
-    const float ymax = __ldg(&c.rowtab[r].ymax), zmin = __ldg(c.zmin + s);
-    int* __restrict__ bins = c.bins + b0;
-    auto local_bin = [&](float y, float z) {     // DESIGN.md section 3.1 step 3
-      const int iy = floor_clamp((y + ymax) * c.inv_cy, ny - 1);
-      const int iz = floor_clamp((z - zmin) * c.inv_cz, nzm1);
-      return iz * ny + iy;
-    };
-
-    for (int j = tid; j < nb; j += kT) bins[j] = 0;
-    __syncthreads();
-
-    // histogram; the atomic's return value is the cluster's arrival rank inside its bin
+  const int nb = g.nb, p0 = g.p0, p1 = g.p1;
+  int* __restrict__ bins = c.bins + g.b0;
+  for (int j = tid; j < nb; j += kT) bins[j] = 0;
+  __syncthreads();
+  // histogram; the atomic's return value is the cluster's arrival rank inside its bin
 #pragma unroll 4
-    for (int i = p0 + tid; i < p1; i += kT) {
-      const float4 v = __ldcg(c.rec + i);
-      const int a = atomicAdd(bins + local_bin(v.x, v.y), 1);
-      reinterpret_cast<int*>(c.rec + i)[3] = a;
+  for (int i = p0 + tid; i < p1; i += kT) {
+    const float4 v = __ldcg(c.rec + i);
+    const int a = atomicAdd(bins + local_bin_of(c, g, v.x, v.y), 1);
+    reinterpret_cast<int*>(c.rec + i)[3] = a;
+  }
+  __syncthreads();
+  // exclusive scan of the bucket's bins, starting at row_start: bins[] becomes the CSR bin_start
+  int carry = p0;
+  for (int base = 0; base < nb; base += kT * 4) {
+    const int j = base + tid * 4;
+    int x[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) x[k] = (j + k < nb) ? __ldcg(bins + j + k) : 0;
+    int total;
+    int o = carry + block_exclusive((x[0] + x[1]) + (x[2] + x[3]), s_scan, &total);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (j + k < nb) bins[j + k] = o;
+      o += x[k];
+    }
+    carry += total;
+  }
+  __syncthreads();
+  // scatter: alone in its bin -> final place; else park the input index at bin_start + arrival rank
+  int* __restrict__ tmp = c.flag_scan;          // free until S3
+#pragma unroll 4
+  for (int i = p0 + tid; i < p1; i += kT) {
+    const float4 v = __ldcg(c.rec + i);
+    const int b = local_bin_of(c, g, v.x, v.y);
+    const int bs = __ldcg(bins + b), be = (b + 1 < nb) ? __ldcg(bins + b + 1) : p1;
+    if (be - bs == 1) {
+      c.perm[bs] = __float_as_int(v.z);
+      c.yz[bs] = make_float2(v.x, v.y);
+      c.srow[bs] = (uint16_t)g.sr;
+    } else {
+      tmp[bs + __float_as_int(v.w)] = __float_as_int(v.z);
+    }
+  }
+  __syncthreads();
+  // multiply-occupied bins: stable rank = number of members with a smaller input index
+#pragma unroll 2
+  for (int i = p0 + tid; i < p1; i += kT) {
+    const float4 v = __ldcg(c.rec + i);
+    const int b = local_bin_of(c, g, v.x, v.y);
+    const int bs = __ldcg(bins + b), be = (b + 1 < nb) ? __ldcg(bins + b + 1) : p1;
+    if (be - bs == 1) continue;
+    const int idx = __float_as_int(v.z);
+    int rank = 0;
+    for (int q = bs; q < be; ++q) rank += (__ldcg(tmp + q) < idx);
+    const int pos = bs + rank;
+    c.perm[pos] = idx;
+    c.yz[pos] = make_float2(v.x, v.y);
+    c.srow[pos] = (uint16_t)g.sr;
+  }
+}
+
+struct SlabShared {
+  int bins[kSlabBinCap];              // slab histogram, then exclusive offsets inside the slab
+  int idx[kSlabCluCap];               // input indices of the clusters of multiply-occupied bins, at offset + arrival rank
+  int cnt[kMaxSlabs + 1];             // clusters per slab, then exclusive offsets (cnt[n_slab] = bucket size)
+  int cur[kMaxSlabs];                 // write cursors of the slab split
+  int scan[33];
+  int sr;
+  int fits;
+};
+
+template <int kT>
+__device__ void bucket_slabs(const Ctx& c, const BucketGeom& g, SlabShared& sh, int n_slab, int slab_rows) {
+  const int tid = threadIdx.x;
+  const int p0 = g.p0, p1 = g.p1, ny = g.ny, nz = g.nzm1 + 1;
+  float4* __restrict__ rec2 = c.rec2;
+  // ---- split the bucket into z-slabs: count, offsets, copy rec -> rec2 (arrival order inside a slab is arbitrary)
+  auto slab_of = [&](float z) { return floor_clamp((z - g.zmin) * c.inv_cz, g.nzm1) / slab_rows; };
+  for (int i = p0 + tid; i < p1; i += kT) atomicAdd(&sh.cnt[slab_of(__ldcg(c.rec + i).y)], 1);
+  __syncthreads();
+  if (tid == 0) {
+    int acc = 0, fits = 1;
+    for (int k = 0; k < n_slab; ++k) {
+      const int v = sh.cnt[k];
+      if (v > kSlabCluCap) fits = 0;
+      sh.cnt[k] = acc; sh.cur[k] = acc;
+      acc += v;
+    }
+    sh.cnt[n_slab] = acc;
+    sh.fits = fits;
+  }
+  __syncthreads();
+  if (!sh.fits) { bucket_global<kT>(c, g, sh.scan); return; }     // a slab with too many clusters: whole bucket the slow way
+#pragma unroll 4
+  for (int i = p0 + tid; i < p1; i += kT) {
+    const float4 v = __ldcg(c.rec + i);
+    rec2[p0 + atomicAdd(&sh.cur[slab_of(v.y)], 1)] = v;
+  }
+  __syncthreads();
+
+  // ---- one slab at a time, in shared memory
+  for (int k = 0; k < n_slab; ++k) {
+    const int q0 = p0 + sh.cnt[k], m = sh.cnt[k + 1] - sh.cnt[k];
+    const int rows = min(slab_rows, nz - k * slab_rows);
+    const int nbs = rows * ny, bbase = k * slab_rows * ny;
+    for (int j = tid; j < nbs; j += kT) sh.bins[j] = 0;
+    __syncthreads();
+    // histogram: arrival rank inside the bin is the atomic's return value, kept in the record
+    for (int i = tid; i < m; i += kT) {
+      const float4 v = __ldcg(rec2 + q0 + i);
+      const int a = atomicAdd(&sh.bins[local_bin_of(c, g, v.x, v.y) - bbase], 1);
+      reinterpret_cast<int*>(rec2 + q0 + i)[3] = a;
     }
     __syncthreads();
-
-    // exclusive scan of the bucket's bins, starting at row_start: bins[] becomes the CSR bin_start
-    int carry = p0;
-    for (int base = 0; base < nb; base += kT * 4) {
+    // exclusive scan in place; the CSR goes out with coalesced stores
+    int carry = 0;
+    for (int base = 0; base < nbs; base += kT * 4) {
       const int j = base + tid * 4;
       int x[4];
 #pragma unroll
-      for (int k = 0; k < 4; ++k) x[k] = (j + k < nb) ? __ldcg(bins + j + k) : 0;
+      for (int e = 0; e < 4; ++e) x[e] = (j + e < nbs) ? sh.bins[j + e] : 0;
       int total;
-      int o = carry + block_exclusive((x[0] + x[1]) + (x[2] + x[3]), s_scan, &total);
+      int o = carry + block_exclusive((x[0] + x[1]) + (x[2] + x[3]), sh.scan, &total);
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        if (j + k < nb) bins[j + k] = o;
-        o += x[k];
+      for (int e = 0; e < 4; ++e) {
+        if (j + e < nbs) { sh.bins[j + e] = o; c.bins[g.b0 + bbase + j + e] = q0 + o; }
+        o += x[e];
       }
       carry += total;
     }
     __syncthreads();
-
-    // scatter (arrival order inside a bin)
-#pragma unroll 4
-    for (int i = p0 + tid; i < p1; i += kT) {
-      const float4 v = __ldcg(c.rec + i);
-      const int pos = __ldcg(bins + local_bin(v.x, v.y)) + __float_as_int(v.w);
-      c.perm[pos] = __float_as_int(v.z);
-      c.yz[pos] = make_float2(v.x, v.y);
-      c.srow[pos] = (uint16_t)sr;
-    }
-    __syncthreads();
-
-    // stable fix-up: order the clusters of a multiply-occupied bin by input index (bins hold ~1-3 clusters)
-    for (int j = tid; j < nb; j += kT) {
-      const int bs = __ldcg(bins + j), be = (j + 1 < nb) ? __ldcg(bins + j + 1) : p1;
-      if (be - bs < 2) continue;
-      for (int a = bs + 1; a < be; ++a) {          // insertion sort on (perm, yz)
-        const int pa = __ldcg(c.perm + a);
-        const float2 va = __ldcg(c.yz + a);
-        int b = a - 1;
-        while (b >= bs) {
-          const int pb = __ldcg(c.perm + b);
-          if (pb < pa) break;
-          c.perm[b + 1] = pb;
-          c.yz[b + 1] = __ldcg(c.yz + b);
-          --b;
-        }
-        if (b + 1 != a) { c.perm[b + 1] = pa; c.yz[b + 1] = va; }
+    // alone in its bin -> final place; else park the input index in the shared table
+    for (int i = tid; i < m; i += kT) {
+      const float4 v = __ldcg(rec2 + q0 + i);
+      const int bl = local_bin_of(c, g, v.x, v.y) - bbase;
+      const int bs = sh.bins[bl], be = (bl + 1 < nbs) ? sh.bins[bl + 1] : m;
+      if (be - bs == 1) {
+        c.perm[q0 + bs] = __float_as_int(v.z);
+        c.yz[q0 + bs] = make_float2(v.x, v.y);
+        c.srow[q0 + bs] = (uint16_t)g.sr;
+      } else {
+        sh.idx[bs + __float_as_int(v.w)] = __float_as_int(v.z);
       }
     }
+    __syncthreads();
+    // multiply-occupied bins: stable rank = number of members with a smaller input index
+    for (int i = tid; i < m; i += kT) {
+      const float4 v = __ldcg(rec2 + q0 + i);
+      const int bl = local_bin_of(c, g, v.x, v.y) - bbase;
+      const int bs = sh.bins[bl], be = (bl + 1 < nbs) ? sh.bins[bl + 1] : m;
+      if (be - bs == 1) continue;
+      const int idx = __float_as_int(v.z);
+      int rank = 0;
+      for (int q = bs; q < be; ++q) rank += (sh.idx[q] < idx);
+      const int pos = q0 + bs + rank;
+      c.perm[pos] = idx;
+      c.yz[pos] = make_float2(v.x, v.y);
+      c.srow[pos] = (uint16_t)g.sr;
+    }
+    __syncthreads();                               // sh.bins / sh.idx are reused by the next slab
+  }
+}
+
+template <int kT, int kMinCtas>
+__global__ void __launch_bounds__(kT, kMinCtas) k_binsort(Ctx c) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SlabShared& sh = *reinterpret_cast<SlabShared*>(smem_raw);
+  if (c.cnt->status) return;
+  const int tid = threadIdx.x;
+  for (;;) {
+    __syncthreads();                               // everybody is done with the previous bucket's shared state
+    if (tid == 0) sh.sr = atomicAdd(&c.cnt->s1_ticket, 1);
+    for (int k = tid; k <= kMaxSlabs; k += kT) sh.cnt[k] = 0;
+    __syncthreads();
+    BucketGeom g;
+    g.sr = sh.sr;
+    if (g.sr >= c.SR) break;
+    g.b0 = __ldg(c.bin_base + g.sr); g.nb = __ldg(c.bin_base + g.sr + 1) - g.b0;
+    if (g.nb == 0) continue;                       // empty sector
+    g.p0 = __ldg(c.row_start + g.sr); g.p1 = __ldg(c.row_start + g.sr + 1);
+    const int s = g.sr / c.R, r = g.sr - s * c.R;
+    g.ny = __ldg(&c.rowtab[r].ny); g.nzm1 = __ldg(c.nz + s) - 1;
+    g.ymax = __ldg(&c.rowtab[r].ymax); g.zmin = __ldg(c.zmin + s);
+    const int m = g.p1 - g.p0, nz = g.nzm1 + 1;
+    if (m == 0) {                                  // a row without clusters: its bins all start at row_start
+      for (int j = tid; j < g.nb; j += kT) c.bins[g.b0 + j] = g.p0;
+      continue;
+    }
+    int n_slab = (m + kSlabTarget - 1) / kSlabTarget;
+    if (n_slab > kMaxSlabs) n_slab = kMaxSlabs;
+    if (n_slab > nz) n_slab = nz;
+    const int slab_rows = (nz + n_slab - 1) / n_slab;
+    n_slab = (nz + slab_rows - 1) / slab_rows;
+    if ((long long)slab_rows * g.ny <= kSlabBinCap) bucket_slabs<kT>(c, g, sh, n_slab, slab_rows);
+    else bucket_global<kT>(c, g, sh.scan);
   }
 }
 
@@ -306,9 +447,16 @@ int launch_s1(const Ctx& c, cudaStream_t st) {
   k_zrange_count<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 8), kThreads, smem_hist ? c.SR * sizeof(int) : 0, st>>>(c, smem_hist);
   k_tables<<<1, 1024, 0, st>>>(c);
   k_partition<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 8), kThreads, 0, st>>>(c);
-  // big buckets: 1024 threads per bucket, two buckets per SM in flight; small ones: 256 threads, eight per SM
-  if ((long long)c.n >= 2048LL * c.SR) k_binsort<1024, 2><<<grid_for(c.SR, 1, c.n_sms, 2), 1024, 0, st>>>(c);
-  else k_binsort<256, 8><<<grid_for(c.SR, 1, c.n_sms, 8), 256, 0, st>>>(c);
+  static bool attr_set = false;
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(k_binsort<1024, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SlabShared)) != cudaSuccess ||
+        cudaFuncSetAttribute(k_binsort<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SlabShared)) != cudaSuccess)
+      return -1;
+    attr_set = true;
+  }
+  // big buckets: 1024 threads per bucket, two buckets per SM in flight; small ones: 256 threads, three per SM (shared memory)
+  if ((long long)c.n >= 2048LL * c.SR) k_binsort<1024, 2><<<grid_for(c.SR, 1, c.n_sms, 2), 1024, sizeof(SlabShared), st>>>(c);
+  else k_binsort<256, 3><<<grid_for(c.SR, 1, c.n_sms, 3), 256, sizeof(SlabShared), st>>>(c);
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 
