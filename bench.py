@@ -112,8 +112,7 @@ def make_timeframe(args, rank: int):
     if args.collisions:
         over["n_collisions"] = args.collisions
     if rank:
-        from tpc_synth import CONFIGS
-        over["seed"] = CONFIGS[args.workload]["seed"] + 1000 * rank     # replicas track different time frames
+        over["seed"] = replica_seed(args.workload, rank)                # replicas track different time frames
     dev = "cuda" if torch.cuda.is_available() and args.impl == "ours" else "cpu"
     return generate_config(args.workload, device=dev, **over)
 
@@ -132,6 +131,26 @@ def algorithmic_bytes(k: dict) -> dict:
     }
     b["total"] = sum(b.values())
     return b
+
+
+def aggregate_over_ranks(ms_device: float, ms_e2e: float, n_clusters: int, world: int, device=None):
+    """Replicas only: the job's time is the MAX over ranks, its work the SUM of the ranks'
+    clusters.  The only torch.distributed traffic of the bench (besides the barriers); works on nccl and gloo."""
+    if world <= 1:
+        return ms_device, ms_e2e, n_clusters
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_device, ms_e2e], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    nn = torch.tensor([n_clusters], dtype=torch.int64, device=device)
+    dist.all_reduce(nn, op=dist.ReduceOp.SUM)
+    return float(t[0]), float(t[1]), int(nn[0])
+
+
+def replica_seed(workload: str, rank: int) -> int:
+    """Rank r tracks its own time frame: the workload's seed + 1000 r."""
+    from tpc_synth import CONFIGS
+    return CONFIGS[workload]["seed"] + 1000 * rank
 
 
 def run_reference(args):
@@ -276,16 +295,9 @@ def run_ours(args):
         e2e = {"ms": ms_e2e / args.steps, "h2d": int(sum(t.numel() * t.element_size() for t in h_in)), "d2h": h_out.bytes_out()}
 
     # ---- max over ranks
-    n_total = tf.n
-    if world > 1:
-        t = torch.tensor([ms_total, e2e["ms"] if e2e else 0.0], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t[0]); ms_e2e_max = float(t[1])
-        if e2e:
-            e2e["ms"] = ms_e2e_max
-        nn = torch.tensor([tf.n], device=dev, dtype=torch.int64)
-        dist.all_reduce(nn)
-        n_total = int(nn[0])
+    ms_total, ms_e2e_max, n_total = aggregate_over_ranks(ms_total, e2e["ms"] if e2e else 0.0, tf.n, world, dev)
+    if e2e:
+        e2e["ms"] = ms_e2e_max
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

@@ -147,3 +147,42 @@ def test_edge_cases():
     assert out.numpy()["status"] & 2
     _, trk, out = run_gpu(tf, params=P, caps=dict(max_tracks=2))
     assert out.numpy()["status"] & 8
+
+
+def test_full_size_sector_sample():
+    """cfg5 at full size, launched as bench.py launches it: sectors are independent (one z range per
+    sector, section 3.1), so the oracle run on whole sectors of the frame must reproduce the CUDA result restricted to
+    them - links bit-exact, cluster-to-track assignment and parameters per the bars above."""
+    from tpc_synth import select_sectors
+    tf = generate_config("cfg5", device="cuda")
+    P, trk, out = run_gpu(tf)
+    k = trk.counters()
+    assert k["status"] == 0 and k["n_clusters"] == tf.n > 50_000_000
+    g = out.numpy()
+    R = P["n_rows"]
+    row_start = trk.stage_view("row_start")
+    link_up = trk.stage_view("link_up"); link_dn = trk.stage_view("link_dn"); perm = trk.stage_view("perm")
+    for s in (0, 23):
+        sub, idx = select_sectors(tf, [s])
+        o = run_oracle(sub, P)
+        a, b = int(row_start[s * R]), int(row_start[(s + 1) * R])
+        assert b - a == sub.n
+        # sorted order: the CUDA perm holds input indices of the full frame, the oracle's those of the sub-frame
+        assert np.array_equal(perm[a:b], idx[o.get("perm")])
+        for gl, name in ((link_up, "link_up"), (link_dn, "link_dn")):
+            want = o.get(name).astype(np.int64)
+            want = np.where(want >= 0, want + a, -1)
+            assert np.array_equal(gl[a:b], want), (s, name)
+        # tracks of a sector have consecutive ids (seed order is sector-major)
+        ct = g["cluster_track"][idx].astype(np.int64)
+        first = ct[ct >= 0].min()
+        ct = np.where(ct >= 0, ct - first, -1)
+        co = o.get("cluster_track")
+        To = int(o.get("trk_seed").shape[0])
+        assert ct.max() + 1 == To
+        same = float((ct == co).mean())
+        assert same >= 0.999, (s, same)
+        par_g = g["par"][first:first + To]; par_o = o.get("trk_par").reshape(-1, 5)
+        rel = np.abs(par_g - par_o) / np.maximum(np.abs(par_o), [1, 1, .1, .1, .1])
+        assert float((rel.max(axis=1) <= PAR_TOL).mean()) >= 0.995, (s, float(rel.max()))
+        print(f"sector {s}: {sub.n} clusters, {To} tracks, assignment identical for {same:.6f}, par max rel {rel.max():.2e}")
