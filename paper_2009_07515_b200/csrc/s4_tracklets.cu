@@ -26,6 +26,7 @@ namespace tpc {
 namespace {
 
 constexpr int kThreads = 128;
+constexpr int kW = 2;                         // candidates of a search loaded together
 constexpr int kCtasPerSm = 6;              // 80 registers per thread (measured: 4 -> 17.7 ms, 5 -> 15.5, 6 -> 13.9, 7 -> 13.9, 8 spills -> 14.7)
 
 // symmetric 5x5, lower triangle row-major: index(i,j) = i*(i+1)/2 + j for i >= j
@@ -144,14 +145,42 @@ __device__ __forceinline__ int kf_search(const Ctx& c, int b0, int ny, float yma
   const float wy = 1.0f / sy2, wz = 1.0f / sz2;
   float best = INFINITY;
   int arg = -1;
-  RowGrid g;
-  g.b0 = b0; g.ny = ny; g.nz = nz; g.ymax = ymax; g.zmin = zmin;
-  for_each_in_rect(g, c.inv_cy, c.inv_cz, c.bins, c.yz, ylo, yhi, zlo, zhi, [&](int j, float yj, float zj) {
-    const float dy = yj - k.p[0];
-    const float dz = (zj - zref) - k.p[1];
-    const float d2 = (dy * dy) * wy + (dz * dz) * wz;
-    if (d2 <= cut && d2 < best) { best = d2; arg = j; *ym = yj; *zm = zj; }
-  });
+  const int iy0 = floor_clamp((ylo + ymax) * c.inv_cy, ny - 1);
+  const int iy1 = floor_clamp((yhi + ymax) * c.inv_cy, ny - 1);
+  const int iz0 = floor_clamp((zlo - zmin) * c.inv_cz, nz - 1);
+  const int iz1 = floor_clamp((zhi - zmin) * c.inv_cz, nz - 1);
+  const int* __restrict__ bins = c.bins;
+  const float2* __restrict__ yz = c.yz;
+  // The window almost always covers one or two bin rows: their four bin_start entries are loaded together and the
+  // two candidate runs are walked as ONE loop (a nested row / candidate loop pays the load latency once per level
+  // and once per row).  Visiting order (row ascending, position ascending) is that of DESIGN.md section 3.1.
+  for (int iz = iz0; iz <= iz1; iz += 2) {
+    const int b = b0 + iz * ny;
+    const bool two = iz + 1 <= iz1;
+    const int jb0 = __ldg(bins + b + iy0), je0 = __ldg(bins + b + iy1 + 1);
+    const int jb1 = two ? __ldg(bins + b + ny + iy0) : 0, je1 = two ? __ldg(bins + b + ny + iy1 + 1) : 0;
+    const int n0 = je0 - jb0, total = n0 + (je1 - jb1);
+    const int shift = jb1 - n0;                   // t >= n0: j = jb1 + (t - n0)
+    for (int t = 0; t < total; t += kW) {         // kW candidates in flight
+      int j[kW];
+      float2 v[kW];
+#pragma unroll
+      for (int e = 0; e < kW; ++e) {
+        const int te = t + e;
+        j[e] = te < n0 ? jb0 + te : shift + te;
+        if (te < total) v[e] = __ldg(yz + j[e]);
+      }
+#pragma unroll
+      for (int e = 0; e < kW; ++e) {
+        if (t + e < total && v[e].x >= ylo && v[e].x <= yhi && v[e].y >= zlo && v[e].y <= zhi) {
+          const float dy = v[e].x - k.p[0];
+          const float dz = (v[e].y - zref) - k.p[1];
+          const float d2 = (dy * dy) * wy + (dz * dz) * wz;
+          if (d2 <= cut && d2 < best) { best = d2; arg = j[e]; *ym = v[e].x; *zm = v[e].y; }
+        }
+      }
+    }
+  }
   return arg;
 }
 
