@@ -3,7 +3,7 @@
 // inside a search window.  One thread per sorted position; consecutive positions are neighbours in
 // (z, y) of the same row, so a warp's rectangle queries hit the same few cache lines of the rows
 // above and below.  The per-row tables sit in shared memory.  Division-free, no candidate cap:
-// up to kCap candidates per side are kept in registers/local memory, beyond that the thread
+// up to kCap candidates per side are kept in shared-memory lists, beyond that the thread
 // re-walks the rectangles (same visiting order, same result).
 #include "tpc_internal.cuh"
 
@@ -13,11 +13,6 @@ namespace {
 constexpr int kThreads = 256;
 constexpr int kCap = 8;
 
-struct Cand {
-  int pos[kCap];
-  float y[kCap], z[kCap];
-  int n;
-};
 
 __device__ __forceinline__ RowGrid make_grid(const Ctx& c, const RowTab* tab, int s, int t) {
   RowGrid g;
@@ -31,6 +26,10 @@ __device__ __forceinline__ RowGrid make_grid(const Ctx& c, const RowTab* tab, in
 
 __global__ void __launch_bounds__(kThreads) k_neighbours(Ctx c) {
   extern __shared__ RowTab tab[];
+  // candidate lists: sorted positions only, [entry][thread] in shared memory (dynamic indexing of a register array
+  // would put them in local memory: 13 % of the instructions of round 1b)
+  int* listU = reinterpret_cast<int*>(tab + c.R) + threadIdx.x;
+  int* listD = listU + kCap * kThreads;
   for (int i = threadIdx.x; i < c.R * (int)(sizeof(RowTab) / 4); i += blockDim.x)
     reinterpret_cast<int*>(tab)[i] = __ldg(reinterpret_cast<const int*>(c.rowtab) + i);
   __syncthreads();
@@ -45,36 +44,35 @@ __global__ void __launch_bounds__(kThreads) k_neighbours(Ctx c) {
     const float y = me.x, z = me.y;
     int lu = -1, ld = -1;
 
-    Cand U, D;
-    U.n = 0; D.n = 0;
+    int nU = 0, nD = 0;
     int ku = 0, kd = 0;
     float uylo = 0, uyhi = 0, uzlo = 0, uzhi = 0, dylo = 0, dyhi = 0, dzlo = 0, dzhi = 0;
     RowGrid gu = {}, gd = {};
-    for (int k = 1; k <= 2 && U.n == 0; ++k) {
+    for (int k = 1; k <= 2 && nU == 0; ++k) {
       if (r + k >= c.R) break;
       const float yc = y * tab[r].up_ratio[k - 1], wy = tab[r].up_wy[k - 1], wz = tab[r].up_wz[k - 1];
       uylo = yc - wy; uyhi = yc + wy; uzlo = z - wz; uzhi = z + wz;
       gu = make_grid(c, tab, s, r + k);
       for_each_in_rect(gu, c.inv_cy, c.inv_cz, bin_start, yz, uylo, uyhi, uzlo, uzhi, [&](int j, float yj, float zj) {
-        if (U.n < kCap) { U.pos[U.n] = j; U.y[U.n] = yj; U.z[U.n] = zj; }
-        ++U.n;
+        if (nU < kCap) listU[nU * kThreads] = j;
+        ++nU;
       });
       ku = k;
     }
-    if (U.n > 0) {
-      for (int k = 1; k <= 2 && D.n == 0; ++k) {
+    if (nU > 0) {
+      for (int k = 1; k <= 2 && nD == 0; ++k) {
         if (r - k < 0) break;
         const float yc = y * tab[r].dn_ratio[k - 1], wy = tab[r].dn_wy[k - 1], wz = tab[r].dn_wz[k - 1];
         dylo = yc - wy; dyhi = yc + wy; dzlo = z - wz; dzhi = z + wz;
         gd = make_grid(c, tab, s, r - k);
         for_each_in_rect(gd, c.inv_cy, c.inv_cz, bin_start, yz, dylo, dyhi, dzlo, dzhi, [&](int j, float yj, float zj) {
-          if (D.n < kCap) { D.pos[D.n] = j; D.y[D.n] = yj; D.z[D.n] = zj; }
-          ++D.n;
+          if (nD < kCap) listD[nD * kThreads] = j;
+          ++nD;
         });
         kd = k;
       }
     }
-    if (U.n > 0 && D.n > 0) {
+    if (nU > 0 && nD > 0) {
       const float dxu = tab[r].up_dx[ku - 1], dxd = tab[r].dn_dx[kd - 1];
       const float cut = c.link_T * ((dxu * dxd) * (dxu * dxd));
       float best = INFINITY;
@@ -85,9 +83,16 @@ __global__ void __launch_bounds__(kThreads) k_neighbours(Ctx c) {
         const float Dv = Dy * Dy + Dz * Dz;
         if (Dv < best) { best = Dv; bu = u; bd = d; }
       };
-      if (U.n <= kCap && D.n <= kCap) {
-        for (int a = 0; a < U.n; ++a)
-          for (int b = 0; b < D.n; ++b) score(U.pos[a], U.y[a], U.z[a], D.pos[b], D.y[b], D.z[b]);
+      if (nU <= kCap && nD <= kCap) {
+        for (int a = 0; a < nU; ++a) {
+          const int u = listU[a * kThreads];
+          const float2 pu = __ldg(yz + u);
+          for (int b = 0; b < nD; ++b) {
+            const int d = listD[b * kThreads];
+            const float2 pd = __ldg(yz + d);
+            score(u, pu.x, pu.y, d, pd.x, pd.y);
+          }
+        }
       } else {   // rare: crowded window, walk the rectangles again
         for_each_in_rect(gu, c.inv_cy, c.inv_cz, bin_start, yz, uylo, uyhi, uzlo, uzhi, [&](int u, float yu, float zu) {
           for_each_in_rect(gd, c.inv_cy, c.inv_cz, bin_start, yz, dylo, dyhi, dzlo, dzhi,
@@ -109,7 +114,7 @@ int launch_s2(const Ctx& c, cudaStream_t st) {
   const long long cap = (long long)c.n_sms * 32;
   if (g > cap) g = cap;
   if (g < 1) g = 1;
-  k_neighbours<<<(unsigned)g, kThreads, c.R * sizeof(RowTab), st>>>(c);
+  k_neighbours<<<(unsigned)g, kThreads, c.R * sizeof(RowTab) + 2 * kCap * kThreads * sizeof(int), st>>>(c);
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 

@@ -145,12 +145,23 @@ __device__ __forceinline__ void for_each_in_rect(const RowGrid& g, float inv_cy,
   const int iy1 = floor_clamp((yhi + g.ymax) * inv_cy, g.ny - 1);
   const int iz0 = floor_clamp((zlo - g.zmin) * inv_cz, g.nz - 1);
   const int iz1 = floor_clamp((zhi - g.zmin) * inv_cz, g.nz - 1);
-  for (int iz = iz0; iz <= iz1; ++iz) {
+  // two bin rows per step: their four bin_start entries are loaded together and both candidate runs are walked as one
+  // loop, two candidates in flight (same visiting order: row ascending, position ascending)
+  for (int iz = iz0; iz <= iz1; iz += 2) {
     const int b = g.b0 + iz * g.ny;
-    const int jb = __ldg(bin_start + b + iy0), je = __ldg(bin_start + b + iy1 + 1);
-    for (int j = jb; j < je; ++j) {
-      const float2 v = __ldg(yz + j);
-      if (v.x >= ylo && v.x <= yhi && v.y >= zlo && v.y <= zhi) f(j, v.x, v.y);
+    const bool two = iz + 1 <= iz1;
+    const int jb0 = __ldg(bin_start + b + iy0), je0 = __ldg(bin_start + b + iy1 + 1);
+    const int jb1 = two ? __ldg(bin_start + b + g.ny + iy0) : 0, je1 = two ? __ldg(bin_start + b + g.ny + iy1 + 1) : 0;
+    const int n0 = je0 - jb0, total = n0 + (je1 - jb1);
+    const int shift = jb1 - n0;                   // t >= n0: j = jb1 + (t - n0)
+    for (int t = 0; t < total; t += 2) {
+      const int ja = t < n0 ? jb0 + t : shift + t;
+      const int jc = t + 1 < n0 ? jb0 + t + 1 : shift + t + 1;
+      const float2 va = __ldg(yz + ja);
+      float2 vc = va;
+      if (t + 1 < total) vc = __ldg(yz + jc);
+      if (va.x >= ylo && va.x <= yhi && va.y >= zlo && va.y <= zhi) f(ja, va.x, va.y);
+      if (t + 1 < total && vc.x >= ylo && vc.x <= yhi && vc.y >= zlo && vc.y <= zhi) f(jc, vc.x, vc.y);
     }
   }
 }
