@@ -47,6 +47,16 @@ def parse():
     return ap.parse_args()
 
 
+def ncu_traffic(kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on cfg5, copied from the committed
+    `ncu --set full` capture (profiles/traffic.json names the capture); None if there is none."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return float(json.load(f)[kernel]["dram_bytes"])
+    except Exception:
+        return None
+
+
 def hbm_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -309,11 +319,11 @@ def run_ours(args):
     bytes_ = algorithmic_bytes(k)
     names = ["S1", "S2", "S3", "S4", "S5"]
     dom = int(np.argmax(stage))
-    dom_kernel = {"S1": "S1 (sort+bin, 10 launches)", "S2": "k_neighbours", "S3": "S3 (cleaner, 7 launches)",
-                  "S4": "k_tracklets", "S5": "S5 (selector, 15 launches)"}[names[dom]]
+    dom_kernel = {"S1": "S1 (sort+bin, 4 launches)", "S2": "k_neighbours", "S3": "S3 (cleaner, 6 launches)",
+                  "S4": "k_tracklets", "S5": "S5 (selector, 16 launches)"}[names[dom]]
     achieved = bytes_[names[dom]] / (stage[dom] * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom_kernel, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_[names[dom]],
+                "traffic": ncu_traffic(dom_kernel) if tf.name == "cfg5" else None, "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_[names[dom]],
                 "kernel_ms": float(stage[dom]),
                 "whole_path": {"algorithmic_bytes": bytes_["total"], "achieved": bytes_["total"] / (ms_step * 1e-3) / 1e9,
                                "frac_of_measured": bytes_["total"] / (ms_step * 1e-3) / 1e9 / peak,

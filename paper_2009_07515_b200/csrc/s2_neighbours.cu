@@ -24,7 +24,7 @@ __device__ __forceinline__ RowGrid make_grid(const Ctx& c, const RowTab* tab, in
   return g;
 }
 
-__global__ void __launch_bounds__(kThreads) k_neighbours(Ctx c) {
+__global__ void __launch_bounds__(kThreads, 5) k_neighbours(Ctx c) {
   extern __shared__ RowTab tab[];
   // candidate lists: sorted positions only, [entry][thread] in shared memory (dynamic indexing of a register array
   // would put them in local memory: 13 % of the instructions of round 1b)
