@@ -139,7 +139,7 @@ typedef struct {
 enum tpc_stage_array {
   TPC_VIEW_PERM = 0,        /* int32 [n]      sorted position -> input index (S1) */
   TPC_VIEW_YZ = 1,          /* float [n][2]   sorted (y, z) pairs */
-  TPC_VIEW_SROW = 2,        /* uint16 [n]     sector*n_rows + row of the sorted cluster */
+  TPC_VIEW_SROW = 2,        /* uint16 [n]     (sector << 8) | row of the sorted cluster    */
   TPC_VIEW_BIN_START = 3,   /* int32 [n_bins+1] CSR over global bins */
   TPC_VIEW_ROW_START = 4,   /* int32 [n_sectors*n_rows+1] */
   TPC_VIEW_BIN_BASE = 5,    /* int32 [n_sectors*n_rows+1] first global bin of each (sector,row) */

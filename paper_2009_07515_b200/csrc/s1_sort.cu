@@ -214,6 +214,7 @@ constexpr int kSlabCluCap = 4096;     // clusters of one slab whose input indice
 
 struct BucketGeom {
   int sr, b0, nb, p0, p1, ny, nzm1;
+  uint16_t srow;                      // (sector << 8) | row, what the sorted srow[] array holds
   float ymax, zmin;
 };
 
@@ -265,7 +266,7 @@ __device__ void bucket_global(const Ctx& c, const BucketGeom& g, int* s_scan) {
     if (be - bs == 1) {
       c.perm[bs] = __float_as_int(v.z);
       c.yz[bs] = make_float2(v.x, v.y);
-      c.srow[bs] = (uint16_t)g.sr;
+      c.srow[bs] = g.srow;
     } else {
       tmp[bs + __float_as_int(v.w)] = __float_as_int(v.z);
     }
@@ -284,7 +285,7 @@ __device__ void bucket_global(const Ctx& c, const BucketGeom& g, int* s_scan) {
     const int pos = bs + rank;
     c.perm[pos] = idx;
     c.yz[pos] = make_float2(v.x, v.y);
-    c.srow[pos] = (uint16_t)g.sr;
+    c.srow[pos] = g.srow;
   }
 }
 
@@ -366,7 +367,7 @@ __device__ void bucket_slabs(const Ctx& c, const BucketGeom& g, SlabShared& sh, 
       if (be - bs == 1) {
         c.perm[q0 + bs] = __float_as_int(v.z);
         c.yz[q0 + bs] = make_float2(v.x, v.y);
-        c.srow[q0 + bs] = (uint16_t)g.sr;
+        c.srow[q0 + bs] = g.srow;
       } else {
         sh.idx[bs + __float_as_int(v.w)] = __float_as_int(v.z);
       }
@@ -384,7 +385,7 @@ __device__ void bucket_slabs(const Ctx& c, const BucketGeom& g, SlabShared& sh, 
       const int pos = q0 + bs + rank;
       c.perm[pos] = idx;
       c.yz[pos] = make_float2(v.x, v.y);
-      c.srow[pos] = (uint16_t)g.sr;
+      c.srow[pos] = g.srow;
     }
     __syncthreads();                               // sh.bins / sh.idx are reused by the next slab
   }
@@ -408,6 +409,7 @@ __global__ void __launch_bounds__(kT, kMinCtas) k_binsort(Ctx c) {
     if (g.nb == 0) continue;                       // empty sector
     g.p0 = __ldg(c.row_start + g.sr); g.p1 = __ldg(c.row_start + g.sr + 1);
     const int s = g.sr / c.R, r = g.sr - s * c.R;
+    g.srow = (uint16_t)((s << 8) | r);
     g.ny = __ldg(&c.rowtab[r].ny); g.nzm1 = __ldg(c.nz + s) - 1;
     g.ymax = __ldg(&c.rowtab[r].ymax); g.zmin = __ldg(c.zmin + s);
     const int m = g.p1 - g.p0, nz = g.nzm1 + 1;

@@ -38,8 +38,8 @@ __global__ void __launch_bounds__(kThreads, 5) k_neighbours(Ctx c) {
   const int* __restrict__ bin_start = c.bins;
   const long long n = c.n;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-    const int sr = c.srow[i];
-    const int s = sr / c.R, r = sr - s * c.R;
+    const int sr = c.srow[i];                            // (sector << 8) | row
+    const int s = sr >> 8, r = sr & 255;
     const float2 me = yz[i];
     const float y = me.x, z = me.y;
     int lu = -1, ld = -1;

@@ -238,9 +238,9 @@ __global__ void __launch_bounds__(kThreads, kCtas) k_tracklets(Ctx c) {
           sd = mine;
           hit = c.t_hit + (size_t)sd * R;
           const int h = __ldg(c.seed_head + sd), nx = __ldg(link_up + h);
-          const int srh = c.srow[h];
-          const int s = srh / R;
-          sR = s * R; r0 = srh - sR;
+          const int srh = c.srow[h];              // (sector << 8) | row
+          const int s = srh >> 8;
+          sR = s * R; r0 = srh & 255;
           nz = __ldg(c.nz + s); zmin = __ldg(c.zmin + s);
           const float2 ph = __ldg(yz + h), pn = __ldg(yz + nx);
           zref = ph.y;

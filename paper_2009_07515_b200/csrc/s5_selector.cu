@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(kThreads) k_write(Ctx c, OutPtrs o) {
     if (lane < 15) o.cov[lane * mt + id] = c.t_cov[(size_t)sd * 15 + lane];
     if (lane == 0) {
       const int low = c.t_first_row[sd];
-      o.sector[id] = (int)c.srow[c.seed_head[sd]] / R;
+      o.sector[id] = (int)c.srow[c.seed_head[sd]] >> 8;
       o.first_row[id] = c.k_first[sd];
       o.last_row[id] = c.k_last[sd];
       o.n_clusters[id] = c.k_owned[sd];

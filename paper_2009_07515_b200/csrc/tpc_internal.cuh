@@ -67,7 +67,7 @@ struct Ctx {
   float4* rec;                        // [n] clusters grouped by (sector,row), arrival order: (y, z, input index, rank in bin)
   float4* rec2;                       // [n] the same records grouped by (sector,row,z-slab); shares memory with the four link arrays
   int* bins;                          // [max_bins+2]; after S1 bins[0..N_b] is the CSR bin_start
-  int* perm; float2* yz; uint16_t* srow;              // [n] sorted: input index, (y,z) pair, sector*R+row
+  int* perm; float2* yz; uint16_t* srow;              // [n] sorted: input index, (y,z) pair, (sector << 8) | row
   int* tile_sums;                     // scan scratch
   // S2 / S3
   int* link_up_raw; int* link_dn_raw; int* link_up; int* link_dn;

@@ -65,7 +65,7 @@ def compare_integer_stages(trk, o, upto=3):
             bad[name] = "differs"
     R = trk.params["n_rows"]
     srow = trk.stage_view("srow").astype(np.int64)
-    if not np.array_equal(srow, o.get("s_sector").astype(np.int64) * R + o.get("s_row")):
+    if not np.array_equal(srow, o.get("s_sector").astype(np.int64) * 256 + o.get("s_row")):   # (sector << 8) | row
         bad["srow"] = "differs"
     return bad
 
