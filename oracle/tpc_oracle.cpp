@@ -22,8 +22,12 @@
 // brute-force all-pairs search; S3 invariants + brute-force chain walk; helix step vs closed-form
 // circle, Jacobian vs finite differences; KF vs closed-form weighted line fit at Bz=0 and vs
 // generator truth (q/pT 1e-4 rel.) on noise-free helices, pulls on smeared input; S5 vs
-// brute-force ownership.  Unpinned beyond invariants + truth efficiency: the S4 pick-up /
-// phase logic (stated in DESIGN.md section 6, "parity unpinned").
+// brute-force ownership; the S4 phase logic (chain, pick-up across holes, gap rule, downward pass) vs
+// generator truth on isolated noise-free helices with rows removed (tests/test_oracle_phases.py);
+// the field constant vs the textbook radius of curvature (tests/golden/helix_radius.txt).
+// "parity unpinned": the S2 pair score and the S4 nearest-candidate choice
+// among several gated clusters are definitions of this reading - only invariants and the
+// end-to-end truth efficiency check them.
 // =============================================================================================
 #include <algorithm>
 #include <chrono>
