@@ -17,15 +17,23 @@ namespace {
 
 constexpr int kThreads = 256;
 
-__device__ __forceinline__ unsigned long long make_key(int n_hits, int tracklet_id) {
-  return ((unsigned long long)(unsigned)n_hits << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)tracklet_id);
+// Ownership key: larger n_hits wins, then the smaller id.  64-bit in general; when every seed id fits 24 bits and
+// n_hits fits 8 (max_seeds <= 2^24, n_rows <= 255) a 32-bit key gives the same order and owner[] is half as large -
+// S5 is bound by random DRAM sectors of that array.
+template <class K> __device__ __forceinline__ K make_key(int n_hits, int id);
+template <> __device__ __forceinline__ unsigned long long make_key<unsigned long long>(int n_hits, int id) {
+  return ((unsigned long long)(unsigned)n_hits << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)id);
+}
+template <> __device__ __forceinline__ unsigned make_key<unsigned>(int n_hits, int id) {
+  return ((unsigned)n_hits << 24) | (0xFFFFFFu - (unsigned)id);
 }
 
+template <class K>
 __global__ void __launch_bounds__(kThreads) k_init_out(Ctx c, OutPtrs o) {
   // owner = 0, cluster_track = -1 (vectorised where aligned; n is host-known)
   const long long n = c.n;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-    c.owner[i] = 0ull;
+    reinterpret_cast<K*>(c.owner)[i] = 0;
     o.cluster_track[i] = -1;
   }
 }
@@ -53,6 +61,7 @@ __global__ void __launch_bounds__(kThreads) k_tracklet_ids(Ctx c) {
 
 // The hit tables are read once per pass and never again: streaming loads keep them from evicting the owner[] / perm[]
 // lines of the sector being worked on out of L2.
+template <class K>
 __global__ void __launch_bounds__(kThreads) k_owner(Ctx c) {
   if (c.cnt->status) return;
   const int ns = c.cnt->n_seeds, R = c.R;
@@ -61,17 +70,19 @@ __global__ void __launch_bounds__(kThreads) k_owner(Ctx c) {
   for (int sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < ns; sd += warps) {
     const int nh = c.t_n_hits[sd];
     if (nh < c.min_tracklet_hits) continue;
-    const unsigned long long key = make_key(nh, sd);
+    const K key = make_key<K>(nh, sd);
+    K* owner = reinterpret_cast<K*>(c.owner);
     const int* hit = c.t_hit + (size_t)sd * R;
     const int last = c.t_last_row[sd];
     for (int r = c.t_first_row[sd] + lane; r <= last; r += 32) {   // the table is defined on [first_row, last_row] only
       const int cl = __ldcs(hit + r);
-      if (cl >= 0) atomicMax(c.owner + cl, key);
+      if (cl >= 0) atomicMax(owner + cl, key);
     }
   }
 }
 
 // owned count, first / last owned row and the ownership bit mask (bit k of word w: row first_row + 32 w + k is owned)
+template <class K>
 __global__ void __launch_bounds__(kThreads) k_owned(Ctx c) {
   if (c.cnt->status) return;
   const int ns = c.cnt->n_seeds, R = c.R;
@@ -83,7 +94,8 @@ __global__ void __launch_bounds__(kThreads) k_owned(Ctx c) {
     int owned = 0, first = 0x7FFFFFFF, last = -1;
     unsigned mine = 0;                                   // lane w keeps mask word w
     if (kept) {
-      const unsigned long long key = make_key(nh, sd);
+      const K key = make_key<K>(nh, sd);
+      const K* owner = reinterpret_cast<const K*>(c.owner);
       const int* hit = c.t_hit + (size_t)sd * R;
       const int hi = c.t_last_row[sd];
       int w = 0;
@@ -92,7 +104,7 @@ __global__ void __launch_bounds__(kThreads) k_owned(Ctx c) {
         bool own = false;
         if (r <= hi) {
           const int cl = __ldcs(hit + r);
-          own = cl >= 0 && c.owner[cl] == key;
+          own = cl >= 0 && owner[cl] == key;
         }
         const unsigned m = __ballot_sync(0xffffffffu, own);
         if (lane == w) mine = m;
@@ -181,9 +193,15 @@ int launch_s5(const Ctx& c, const OutPtrs& o, cudaStream_t st) {
   const unsigned gn = grid_for(c.n, kThreads, c.n_sms, 8);
   const unsigned gs = grid_for(c.max_seeds, kThreads, c.n_sms, 8);          // thread per seed
   const unsigned gw = grid_for((long long)c.max_seeds * 32, kThreads, c.n_sms, 8);   // warp per seed
-  k_init_out<<<gn, kThreads, 0, st>>>(c, o);
-  k_owner<<<gw, kThreads, 0, st>>>(c);
-  k_owned<<<gw, kThreads, 0, st>>>(c);
+  if (c.max_seeds <= (1 << 24) && c.R <= 255) {
+    k_init_out<unsigned><<<gn, kThreads, 0, st>>>(c, o);
+    k_owner<unsigned><<<gw, kThreads, 0, st>>>(c);
+    k_owned<unsigned><<<gw, kThreads, 0, st>>>(c);
+  } else {
+    k_init_out<unsigned long long><<<gn, kThreads, 0, st>>>(c, o);
+    k_owner<unsigned long long><<<gw, kThreads, 0, st>>>(c);
+    k_owned<unsigned long long><<<gw, kThreads, 0, st>>>(c);
+  }
   if (launch_scan_inclusive(c.surv_scan, &c.cnt->n_seeds, 0, c.max_seeds, c.tile_sums, &c.cnt->n_tracks, c.n_sms, st)) return -1;
   if (launch_scan_inclusive(c.owned_scan, &c.cnt->n_seeds, 0, c.max_seeds, c.tile_sums, &c.cnt->n_track_clusters, c.n_sms, st)) return -1;
   k_finalize<<<1, 1, 0, st>>>(c, o);

@@ -186,3 +186,16 @@ def test_full_size_sector_sample():
         rel = np.abs(par_g - par_o) / np.maximum(np.abs(par_o), [1, 1, .1, .1, .1])
         assert float((rel.max(axis=1) <= PAR_TOL).mean()) >= 0.995, (s, float(rel.max()))
         print(f"sector {s}: {sub.n} clusters, {To} tracks, assignment identical for {same:.6f}, par max rel {rel.max():.2e}")
+
+
+def test_wide_ownership_keys(mini_event):
+    """S5 uses 32-bit ownership keys when every seed id fits 24 bits and 64-bit keys otherwise: a capacity above 2^24
+    seeds forces the wide path (~12 GB of workspace), which must give the same tracks."""
+    P, trk32, out32 = run_gpu(mini_event)
+    _, trk64, out64 = run_gpu(mini_event, caps=dict(max_seeds=(1 << 24) + 1))
+    a, b = out32.numpy(), out64.numpy()
+    assert a["status"] == b["status"] == 0 and a["n_tracks"] == b["n_tracks"] > 0
+    for k in a:
+        if isinstance(a[k], np.ndarray):
+            assert np.array_equal(a[k], b[k]), k
+    assert np.array_equal(trk32.stage_view("k_owned"), trk64.stage_view("k_owned")[: trk32.stage_view("k_owned").shape[0]])
