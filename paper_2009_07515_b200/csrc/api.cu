@@ -78,6 +78,7 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   c.link_dn = base ? c.link_up + N : nullptr;
   c.flag_scan = cv.take<int>(N);
   c.seed_head = cv.take<int>(K); c.seed_len = cv.take<int>(K);
+  c.seed_rec = cv.take<float4>(2 * K);
   c.t_hit = cv.take<int>(K * R);
   c.t_first_row = cv.take<int>(K); c.t_last_row = cv.take<int>(K); c.t_n_hits = cv.take<int>(K);
   c.t_par = cv.take<float>(K * 5); c.t_cov = cv.take<float>(K * 15); c.t_chi2 = cv.take<float>(K); c.t_zref = cv.take<float>(K);

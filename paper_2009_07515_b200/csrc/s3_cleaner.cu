@@ -58,7 +58,17 @@ __global__ void __launch_bounds__(kThreads) k_seeds(Ctx c) {
   const long long n = c.n;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
     const int inc = c.flag_scan[i], prev = i ? c.flag_scan[i - 1] : 0;
-    if (inc != prev) c.seed_head[inc - 1] = (int)i;     // seed_len[id] is written by S4
+    if (inc != prev) {                                   // seed_len[id] is written by S4
+      const int id = inc - 1;
+      c.seed_head[id] = (int)i;
+      // everything S4 needs to start the tracklet, gathered here (3 dependent loads per seed that S4's refill would
+      // otherwise take with one active lane): head, next, their (y,z), (sector << 8 | row) of the head, row of next
+      const int nx = c.link_up[i];
+      const float2 ph = c.yz[i], pn = c.yz[nx];
+      const int srh = c.srow[i], r1 = c.srow[nx] & 255;
+      c.seed_rec[2 * (size_t)id] = make_float4(ph.x, ph.y, pn.x, pn.y);
+      c.seed_rec[2 * (size_t)id + 1] = make_float4(__int_as_float((int)i), __int_as_float(nx), __int_as_float(srh), __int_as_float(r1));
+    }
   }
 }
 

@@ -237,14 +237,13 @@ __global__ void __launch_bounds__(kThreads, kCtas) k_tracklets(Ctx c) {
         if (mine < n_seeds) {
           sd = mine;
           hit = c.t_hit + (size_t)sd * R;
-          const int h = __ldg(c.seed_head + sd), nx = __ldg(link_up + h);
-          const int srh = c.srow[h];              // (sector << 8) | row
-          const int s = srh >> 8;
+          const float4 sa = __ldg(c.seed_rec + 2 * (size_t)sd), sb = __ldg(c.seed_rec + 2 * (size_t)sd + 1);   // written by S3's k_seeds
+          const int h = __float_as_int(sb.x), nx = __float_as_int(sb.y), srh = __float_as_int(sb.z), r1 = __float_as_int(sb.w);
+          const int s = srh >> 8;                 // srh = (sector << 8) | row
           sR = s * R; r0 = srh & 255;
           nz = __ldg(c.nz + s); zmin = __ldg(c.zmin + s);
-          const float2 ph = __ldg(yz + h), pn = __ldg(yz + nx);
+          const float2 ph = make_float2(sa.x, sa.y), pn = make_float2(sa.z, sa.w);
           zref = ph.y;
-          const int r1 = r0 + 1 + (nx >= __ldg(c.row_start + sR + r0 + 2));
           const float dx = tx[r1] - tx[r0];
           const float dy = pn.x - ph.x;
           const float dz = pn.y - zref;

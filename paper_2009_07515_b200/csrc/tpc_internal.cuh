@@ -73,6 +73,7 @@ struct Ctx {
   int* link_up_raw; int* link_dn_raw; int* link_up; int* link_dn;
   int* flag_scan;                     // [n] S3: seed bit per sorted position, then its inclusive scan
   int* seed_head; int* seed_len;      // [max_seeds]
+  float4* seed_rec;                   // [max_seeds][2] (y,z) of head and next; head, next, (sector << 8 | row) of head, row of next
   // S4
   int* t_hit;                         // [max_seeds][R]
   int* t_first_row; int* t_last_row; int* t_n_hits;   // [max_seeds]
