@@ -64,6 +64,7 @@ STATUS_BITS = {1: "BAD_CLUSTER", 2: "BINS_OVERFLOW", 4: "SEEDS_OVERFLOW", 8: "TR
 
 EXPORTS = [
     "tpc_tracker_workspace_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
+    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end",
     "tpc_tracker_counters", "tpc_tracker_enable_stage_timing", "tpc_tracker_stage_ms", "tpc_tracker_stage_view",
     "tpc_tracker_launches_per_call", "tpc_tracker_destroy", "tpc_error_string",
 ]
@@ -100,6 +101,10 @@ def load_library(build: bool = True) -> C.CDLL:
         f = getattr(lib, name)
         f.restype = C.c_int
         f.argtypes = [C.c_void_p, P(tpc_clusters_t), P(tpc_tracks_t), C.c_void_p]
+    lib.tpc_track_timeframe_host_begin.restype = C.c_int
+    lib.tpc_track_timeframe_host_begin.argtypes = [C.c_void_p, P(tpc_clusters_t), C.c_int32]
+    lib.tpc_track_timeframe_host_end.restype = C.c_int
+    lib.tpc_track_timeframe_host_end.argtypes = [C.c_void_p, P(tpc_tracks_t), C.c_int32]
     lib.tpc_tracker_counters.restype = C.c_int
     lib.tpc_tracker_counters.argtypes = [C.c_void_p, P(tpc_counters_t)]
     lib.tpc_tracker_enable_stage_timing.restype = C.c_int
@@ -187,7 +192,7 @@ class Tracker:
     """tpc_tracker_create / tpc_track_timeframe / tpc_tracker_destroy with torch-owned memory."""
 
     def __init__(self, params: dict, max_clusters: int, max_bins: int, max_seeds: int, max_tracks: int,
-                 max_track_clusters: int, host_io: bool = False, device="cuda:0"):
+                 max_track_clusters: int, host_io: int = 0, device="cuda:0"):
         if not torch.cuda.is_available():
             raise RuntimeError("tpc tracker needs a CUDA device: there is no CPU fallback")
         self.lib = load_library()
@@ -249,6 +254,18 @@ class Tracker:
         s = out.struct()
         _check(self.lib, self.lib.tpc_track_timeframe_host(self._h, C.byref(c), C.byref(s), C.c_void_p(st.cuda_stream)),
                "tpc_track_timeframe_host")
+
+    def track_timeframe_host_begin(self, sector, row, y, z, slot: int):
+        """Pipelined host path (host_io=2): enqueue H2D + S1..S5 of one frame, do not wait."""
+        for t in (sector, row, y, z):
+            assert (not t.is_cuda) and t.is_contiguous()
+        c = self._clusters(sector, row, y, z)
+        _check(self.lib, self.lib.tpc_track_timeframe_host_begin(self._h, C.byref(c), int(slot)), "tpc_track_timeframe_host_begin")
+
+    def track_timeframe_host_end(self, out: Tracks, slot: int):
+        """Wait for the frame begun on `slot` and copy its tracks into the (pinned host) buffers of `out`."""
+        s = out.struct()
+        _check(self.lib, self.lib.tpc_track_timeframe_host_end(self._h, C.byref(s), int(slot)), "tpc_track_timeframe_host_end")
 
     def counters(self) -> dict:
         k = tpc_counters_t()

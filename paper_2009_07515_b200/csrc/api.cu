@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <initializer_list>
 #include <new>
 #include <vector>
 
@@ -16,9 +17,16 @@ struct tpc_tracker {
   Ctx ctx;                        // pointers into the workspace; input fields set per call
   int64_t max_clusters, max_bins, max_seeds, max_tracks, max_track_clusters;
   int host_io;
-  // staging for the host variant (device)
-  uint8_t* st_sector; uint8_t* st_row; float* st_y; float* st_z;
-  OutPtrs st_out;
+  // staging for the host variants (device): slot 0 serves tpc_track_timeframe_host, slots 0 and 1 the pipelined pair
+  struct Slot {
+    uint8_t* sector; uint8_t* row; float* y; float* z;
+    OutPtrs out;
+    int64_t n;
+    cudaEvent_t h2d_done, in_free, done, out_free;   // pipelined path only
+    bool busy;
+  } slot[2];
+  cudaStream_t s_in, s_compute, s_out;                // pipelined path only (host_io == 2)
+  int* h_counts;                                      // pinned host: [slot][4] = n_tracks, status, n_track_clusters, -
   cudaStream_t last_stream;
   bool timing;
   cudaEvent_t ev[6];
@@ -88,11 +96,12 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   c.surv_scan = cv.take<int>(K); c.owned_scan = cv.take<int>(K);
   c.mask_words = (R + 31) / 32;
   c.own_mask = cv.take<unsigned>(K * (size_t)c.mask_words);
-  if (t->host_io) {
+  for (int k = 0; k < (t->host_io >= 2 ? 2 : t->host_io ? 1 : 0); ++k) {
     const size_t T = (size_t)t->max_tracks, TC = (size_t)t->max_track_clusters;
-    t->st_sector = cv.take<uint8_t>(N); t->st_row = cv.take<uint8_t>(N);
-    t->st_y = cv.take<float>(N); t->st_z = cv.take<float>(N);
-    OutPtrs& o = t->st_out;
+    tpc_tracker::Slot& sl = t->slot[k];
+    sl.sector = cv.take<uint8_t>(N); sl.row = cv.take<uint8_t>(N);
+    sl.y = cv.take<float>(N); sl.z = cv.take<float>(N);
+    OutPtrs& o = sl.out;
     o.n_tracks = cv.take<int>(1); o.status = cv.take<int>(1);
     o.sector = cv.take<int>(T); o.first_row = cv.take<int>(T); o.last_row = cv.take<int>(T); o.n_clusters = cv.take<int>(T);
     o.par = cv.take<float>(T * 5); o.cov = cv.take<float>(T * 15);
@@ -154,7 +163,7 @@ void fill_ctx_constants(tpc_tracker* t, std::vector<RowTab>& tab) {
 
 bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
-int run_device(tpc_tracker* t, const tpc_clusters_t* in, const OutPtrs& o, cudaStream_t st) {
+int run_device(tpc_tracker* t, const tpc_clusters_t* in, const OutPtrs& o, cudaStream_t st, cudaEvent_t after_s1 = nullptr) {
   Ctx& c = t->ctx;
   c.n = (int)in->n;
   c.in_sector = in->sector; c.in_row = in->row; c.in_y = in->y; c.in_z = in->z;
@@ -164,6 +173,7 @@ int run_device(tpc_tracker* t, const tpc_clusters_t* in, const OutPtrs& o, cudaS
   if (tm) cudaEventRecord(t->ev[0], st);
   if (launch_reset(c, st)) return TPC_ERR_CUDA;
   if (launch_s1(c, st)) return TPC_ERR_CUDA;
+  if (after_s1) cudaEventRecord(after_s1, st);     // the input arrays are not read again
   if (tm) cudaEventRecord(t->ev[1], st);
   if (launch_s2(c, st)) return TPC_ERR_CUDA;
   if (tm) cudaEventRecord(t->ev[2], st);
@@ -189,6 +199,28 @@ OutPtrs to_out(const tpc_tracks_t* o) {
   r.z_ref = o->z_ref; r.chi2 = o->chi2; r.ndf = o->ndf; r.trk_cl_start = o->trk_cl_start; r.trk_cl_idx = o->trk_cl_idx;
   r.cluster_track = o->cluster_track; r.max_tracks = (int)o->max_tracks; r.max_track_clusters = (int)o->max_track_clusters;
   return r;
+}
+
+// D2H of exactly the tracks found (T tracks, n_tc attached clusters) from the staging outputs `o` to the caller's HOST
+// buffers, enqueued on `st`.
+bool copy_tracks_d2h(const OutPtrs& o, const tpc_tracks_t* out, size_t n, size_t T, size_t n_tc, cudaStream_t st) {
+  const size_t mt = (size_t)out->max_tracks;
+  auto d2h = [&](void* dst, const void* src, size_t bytes) {
+    return bytes == 0 || cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  };
+  bool ok = true;
+  if (T) {
+    ok = d2h(out->sector, o.sector, T * 4) && d2h(out->first_row, o.first_row, T * 4) &&
+         d2h(out->last_row, o.last_row, T * 4) && d2h(out->n_clusters, o.n_clusters, T * 4) &&
+         d2h(out->x_ref, o.x_ref, T * 4) && d2h(out->z_ref, o.z_ref, T * 4) && d2h(out->chi2, o.chi2, T * 4) &&
+         d2h(out->ndf, o.ndf, T * 4) && d2h(out->trk_cl_start, o.trk_cl_start, (T + 1) * 4);
+    for (int i = 0; i < 5 && ok; ++i) ok = d2h(out->par + i * mt, o.par + i * mt, T * 4);
+    for (int i = 0; i < 15 && ok; ++i) ok = d2h(out->cov + i * mt, o.cov + i * mt, T * 4);
+    ok = ok && d2h(out->trk_cl_idx, o.trk_cl_idx, n_tc * 4);
+  } else {
+    out->trk_cl_start[0] = 0;
+  }
+  return ok && d2h(out->cluster_track, o.cluster_track, n * 4);
 }
 
 }  // namespace
@@ -239,6 +271,16 @@ int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t
   }
   for (auto& e : t->ev)
     if (cudaEventCreate(&e) != cudaSuccess) { delete t; return TPC_ERR_CUDA; }
+  if (host_io >= 2) {
+    bool ok = cudaStreamCreateWithFlags(&t->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&t->s_compute, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&t->s_out, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaHostAlloc(reinterpret_cast<void**>(&t->h_counts), 8 * sizeof(int), cudaHostAllocDefault) == cudaSuccess;
+    for (auto& sl : t->slot)
+      for (cudaEvent_t* e : {&sl.h2d_done, &sl.in_free, &sl.done, &sl.out_free})
+        ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { tpc_tracker_destroy(t); return TPC_ERR_CUDA; }
+  }
   *out = t;
   return TPC_OK;
 }
@@ -260,15 +302,16 @@ int tpc_track_timeframe_host(tpc_tracker_t* t, const tpc_clusters_t* in, const t
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const size_t n = (size_t)in->n;
   tpc_clusters_t d = *in;
-  d.sector = t->st_sector; d.row = t->st_row; d.y = t->st_y; d.z = t->st_z; d.x = nullptr;
+  tpc_tracker::Slot& sl = t->slot[0];
+  d.sector = sl.sector; d.row = sl.row; d.y = sl.y; d.z = sl.z; d.x = nullptr;
   if (n) {
-    if (cudaMemcpyAsync(t->st_sector, in->sector, n, cudaMemcpyHostToDevice, st) != cudaSuccess ||
-        cudaMemcpyAsync(t->st_row, in->row, n, cudaMemcpyHostToDevice, st) != cudaSuccess ||
-        cudaMemcpyAsync(t->st_y, in->y, n * 4, cudaMemcpyHostToDevice, st) != cudaSuccess ||
-        cudaMemcpyAsync(t->st_z, in->z, n * 4, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    if (cudaMemcpyAsync(sl.sector, in->sector, n, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(sl.row, in->row, n, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(sl.y, in->y, n * 4, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        cudaMemcpyAsync(sl.z, in->z, n * 4, cudaMemcpyHostToDevice, st) != cudaSuccess)
       return TPC_ERR_CUDA;
   }
-  OutPtrs o = t->st_out;
+  OutPtrs o = sl.out;
   o.max_tracks = (int)out->max_tracks; o.max_track_clusters = (int)out->max_track_clusters;
   const int rc = run_device(t, &d, o, st);
   if (rc != TPC_OK) return rc;
@@ -279,26 +322,64 @@ int tpc_track_timeframe_host(tpc_tracker_t* t, const tpc_clusters_t* in, const t
       cudaStreamSynchronize(st) != cudaSuccess)
     return TPC_ERR_CUDA;
   *out->n_tracks = head[0]; *out->status = head[1];
-  const size_t T = (size_t)head[0], mt = (size_t)out->max_tracks;
-  auto d2h = [&](void* dst, const void* src, size_t bytes) {
-    return bytes == 0 || cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st) == cudaSuccess;
-  };
-  bool ok = true;
   int n_tc = 0;
-  if (T) {
-    ok = ok && d2h(out->sector, o.sector, T * 4) && d2h(out->first_row, o.first_row, T * 4) &&
-         d2h(out->last_row, o.last_row, T * 4) && d2h(out->n_clusters, o.n_clusters, T * 4) &&
-         d2h(out->x_ref, o.x_ref, T * 4) && d2h(out->z_ref, o.z_ref, T * 4) && d2h(out->chi2, o.chi2, T * 4) &&
-         d2h(out->ndf, o.ndf, T * 4) && d2h(out->trk_cl_start, o.trk_cl_start, (T + 1) * 4);
-    for (int i = 0; i < 5 && ok; ++i) ok = d2h(out->par + i * mt, o.par + i * mt, T * 4);
-    for (int i = 0; i < 15 && ok; ++i) ok = d2h(out->cov + i * mt, o.cov + i * mt, T * 4);
-    ok = ok && d2h(&n_tc, &t->ctx.cnt->n_track_clusters, 4) && cudaStreamSynchronize(st) == cudaSuccess;
-    ok = ok && d2h(out->trk_cl_idx, o.trk_cl_idx, (size_t)n_tc * 4);
-  } else {
-    out->trk_cl_start[0] = 0;
+  if (head[0] && (cudaMemcpyAsync(&n_tc, &t->ctx.cnt->n_track_clusters, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+                  cudaStreamSynchronize(st) != cudaSuccess))
+    return TPC_ERR_CUDA;
+  if (!copy_tracks_d2h(o, out, n, (size_t)head[0], (size_t)n_tc, st) || cudaStreamSynchronize(st) != cudaSuccess) return TPC_ERR_CUDA;
+  return TPC_OK;
+}
+
+// ---- pipelined host path (host_io == 2): H2D of frame i+1 and D2H of frame i-1 overlap the kernels of frame i.
+// Three library-owned streams; two staging slots; events order the reuse of a slot's input staging (free once S1 of
+// the frame that used it has run), of its output staging (free once its D2H has finished) and of the single workspace
+// (frames compute one after the other on s_compute).
+int tpc_track_timeframe_host_begin(tpc_tracker_t* t, const tpc_clusters_t* in, int32_t slot) {
+  if (!t || !in || t->host_io < 2 || slot < 0 || slot > 1) return TPC_ERR_INVALID_ARG;
+  if (in->n < 0 || (in->n > 0 && (!in->sector || !in->row || !in->y || !in->z))) return TPC_ERR_INVALID_ARG;
+  if (in->n > t->max_clusters) return TPC_ERR_CAPACITY;
+  tpc_tracker::Slot& sl = t->slot[slot];
+  if (sl.busy) return TPC_ERR_INVALID_ARG;          // begin / end must alternate per slot
+  const size_t n = (size_t)in->n;
+  sl.n = in->n;
+  if (cudaStreamWaitEvent(t->s_in, sl.in_free, 0) != cudaSuccess) return TPC_ERR_CUDA;
+  if (n) {
+    if (cudaMemcpyAsync(sl.sector, in->sector, n, cudaMemcpyHostToDevice, t->s_in) != cudaSuccess ||
+        cudaMemcpyAsync(sl.row, in->row, n, cudaMemcpyHostToDevice, t->s_in) != cudaSuccess ||
+        cudaMemcpyAsync(sl.y, in->y, n * 4, cudaMemcpyHostToDevice, t->s_in) != cudaSuccess ||
+        cudaMemcpyAsync(sl.z, in->z, n * 4, cudaMemcpyHostToDevice, t->s_in) != cudaSuccess)
+      return TPC_ERR_CUDA;
   }
-  ok = ok && d2h(out->cluster_track, o.cluster_track, n * 4);
-  if (!ok || cudaStreamSynchronize(st) != cudaSuccess) return TPC_ERR_CUDA;
+  if (cudaEventRecord(sl.h2d_done, t->s_in) != cudaSuccess ||
+      cudaStreamWaitEvent(t->s_compute, sl.h2d_done, 0) != cudaSuccess ||
+      cudaStreamWaitEvent(t->s_compute, sl.out_free, 0) != cudaSuccess)
+    return TPC_ERR_CUDA;
+  tpc_clusters_t d = *in;
+  d.sector = sl.sector; d.row = sl.row; d.y = sl.y; d.z = sl.z; d.x = nullptr;
+  const int rc = run_device(t, &d, sl.out, t->s_compute, sl.in_free);
+  if (rc != TPC_OK) return rc;
+  int* hc = t->h_counts + 4 * slot;
+  if (cudaMemcpyAsync(hc + 0, sl.out.n_tracks, 4, cudaMemcpyDeviceToHost, t->s_compute) != cudaSuccess ||
+      cudaMemcpyAsync(hc + 1, sl.out.status, 4, cudaMemcpyDeviceToHost, t->s_compute) != cudaSuccess ||
+      cudaMemcpyAsync(hc + 2, &t->ctx.cnt->n_track_clusters, 4, cudaMemcpyDeviceToHost, t->s_compute) != cudaSuccess ||
+      cudaEventRecord(sl.done, t->s_compute) != cudaSuccess)
+    return TPC_ERR_CUDA;
+  sl.busy = true;
+  return TPC_OK;
+}
+
+int tpc_track_timeframe_host_end(tpc_tracker_t* t, const tpc_tracks_t* out, int32_t slot) {
+  if (!t || !out_ok(out) || t->host_io < 2 || slot < 0 || slot > 1) return TPC_ERR_INVALID_ARG;
+  tpc_tracker::Slot& sl = t->slot[slot];
+  if (!sl.busy) return TPC_ERR_INVALID_ARG;
+  if (out->max_tracks != t->max_tracks || out->max_track_clusters != t->max_track_clusters) return TPC_ERR_INVALID_ARG;
+  if (cudaEventSynchronize(sl.done) != cudaSuccess) return TPC_ERR_CUDA;
+  const int* hc = t->h_counts + 4 * slot;
+  *out->n_tracks = hc[0]; *out->status = hc[1];
+  const bool ok = copy_tracks_d2h(sl.out, out, (size_t)sl.n, (size_t)hc[0], (size_t)hc[2], t->s_out);
+  if (!ok || cudaEventRecord(sl.out_free, t->s_out) != cudaSuccess || cudaStreamSynchronize(t->s_out) != cudaSuccess)
+    return TPC_ERR_CUDA;
+  sl.busy = false;
   return TPC_OK;
 }
 
@@ -377,6 +458,14 @@ int tpc_tracker_destroy(tpc_tracker_t* t) {
   if (!t) return TPC_ERR_INVALID_ARG;
   for (auto& e : t->ev)
     if (e) cudaEventDestroy(e);
+  if (t->s_compute) cudaStreamSynchronize(t->s_compute);
+  if (t->s_out) cudaStreamSynchronize(t->s_out);
+  for (auto& sl : t->slot)
+    for (cudaEvent_t e : {sl.h2d_done, sl.in_free, sl.done, sl.out_free})
+      if (e) cudaEventDestroy(e);
+  for (cudaStream_t st : {t->s_in, t->s_compute, t->s_out})
+    if (st) cudaStreamDestroy(st);
+  if (t->h_counts) cudaFreeHost(t->h_counts);
   delete t;
   return TPC_OK;
 }
