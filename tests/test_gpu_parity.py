@@ -238,3 +238,23 @@ def test_pipelined_host_path(mini_event, mini_tf):
     # a slot used out of order is refused
     with pytest.raises(RuntimeError):
         trk.track_timeframe_host_end(outs[0], 0)
+
+
+def test_crowded_slab_falls_back_and_stays_exact():
+    """5000 tracks (2 x 2250 per row) squeezed into +-5 cm of z of one sector, one bin row per (sector,row) bucket: the bucket's only z-slab
+    holds more clusters than the shared-memory tables of the bin sort take (global-memory path), the link windows hold
+    far more than kCap candidates (rectangle re-walk in S2), and bins hold many clusters (stable order by input index)."""
+    tf = generate_config("cfg1", n_tracks=5000, seed=7)
+    tf.z = (tf.z * np.float32(0.02)).astype(np.float32)
+    P = default_params(tf, cell=4.0)
+    P["cell_z"] = np.float32(16.0)
+    Pg, trk, out = run_gpu(tf, params=P)
+    o = run_oracle(tf, P)
+    assert trk.counters()["status"] == 0
+    assert int(np.diff(trk.stage_view("row_start")).max()) > 2048
+    bad = compare_integer_stages(trk, o)
+    assert not bad, bad
+    t = compare_tracklets(trk, o)
+    assert t["hit_mismatch_seeds"] == 0 and t["par_rel"] <= PAR_TOL and t["cov_rel"] <= COV_TOL, t
+    res = compare_tracks(out.numpy(), o, tf.n)
+    assert res["cluster_track_equal"] and res["csr_equal"], res
