@@ -6,7 +6,8 @@
 //   k_owned      owned count, first/last owned row, ownership bit mask per tracklet
 //                -> scans -> track ids, CSR starts
 //   k_finalize   capacity checks, n_tracks
-//   k_write      tracks SoA, trk_cl_idx (input indices, ascending row), cluster_track  (reads the masks, not owner[])
+//   k_write      trk_cl_idx (input indices, ascending row), cluster_track  (warp per track; reads the masks, not owner[])
+//   k_params     tracks SoA (thread per track id: coalesced stores)
 //   k_kept / scan / k_tracklet_ids   tracklet ids for the debug view (off the critical path: the key carries the
 //                seed id, which orders kept tracklets exactly as their tracklet id would)
 #include "tpc_internal.cuh"
@@ -161,21 +162,38 @@ __global__ void __launch_bounds__(kThreads) k_write(Ctx c, OutPtrs o) {
       }
       off += __popc(m);
     }
-    if (lane < 5) o.par[lane * mt + id] = c.t_par[(size_t)sd * 5 + lane];
-    if (lane < 15) o.cov[lane * mt + id] = c.t_cov[(size_t)sd * 15 + lane];
     if (lane == 0) {
-      const int low = c.t_first_row[sd];
-      o.sector[id] = (int)c.srow[c.seed_head[sd]] >> 8;
-      o.first_row[id] = c.k_first[sd];
-      o.last_row[id] = c.k_last[sd];
-      o.n_clusters[id] = c.k_owned[sd];
-      o.x_ref[id] = c.rowtab[low].x;
-      o.z_ref[id] = c.t_zref[sd];
-      o.chi2[id] = c.t_chi2[sd];
-      o.ndf[id] = 2 * c.t_n_hits[sd] - 5;
+      c.kept_scan[id] = sd;                          // seed of track id, for k_params (kept_scan is free until k_kept)
       o.trk_cl_start[id + 1] = end;
     }
   }
+}
+
+// Track parameters: one thread per TRACK id, so every output component is written with coalesced full-sector stores
+// (one warp per track wrote 29 scattered 4-byte stores per track: 50 M partial sectors on cfg5).
+__global__ void __launch_bounds__(kThreads) k_params(Ctx c, OutPtrs o) {
+  if (c.cnt->status) return;
+  const int nt = c.cnt->n_tracks, R = c.R;
+  const size_t mt = (size_t)o.max_tracks;
+  for (int id = blockIdx.x * blockDim.x + threadIdx.x; id < nt; id += gridDim.x * blockDim.x) {
+    const int sd = c.kept_scan[id];
+    const float* p = c.t_par + (size_t)sd * 5;
+    const float* q = c.t_cov + (size_t)sd * 15;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) o.par[i * mt + id] = p[i];
+#pragma unroll
+    for (int i = 0; i < 15; ++i) o.cov[i * mt + id] = q[i];
+    const int low = c.t_first_row[sd];
+    o.sector[id] = (int)c.srow[c.seed_head[sd]] >> 8;
+    o.first_row[id] = c.k_first[sd];
+    o.last_row[id] = c.k_last[sd];
+    o.n_clusters[id] = c.k_owned[sd];
+    o.x_ref[id] = c.rowtab[low].x;
+    o.z_ref[id] = c.t_zref[sd];
+    o.chi2[id] = c.t_chi2[sd];
+    o.ndf[id] = 2 * c.t_n_hits[sd] - 5;
+  }
+  (void)R;
 }
 
 inline unsigned grid_for(long long n, int per_block, int n_sms, int waves) {
@@ -188,7 +206,7 @@ inline unsigned grid_for(long long n, int per_block, int n_sms, int waves) {
 
 }  // namespace
 
-int launches_s5() { return 7 + 9; }
+int launches_s5() { return 8 + 9; }
 int launch_s5(const Ctx& c, const OutPtrs& o, cudaStream_t st) {
   const unsigned gn = grid_for(c.n, kThreads, c.n_sms, 8);
   const unsigned gs = grid_for(c.max_seeds, kThreads, c.n_sms, 8);          // thread per seed
@@ -206,6 +224,7 @@ int launch_s5(const Ctx& c, const OutPtrs& o, cudaStream_t st) {
   if (launch_scan_inclusive(c.owned_scan, &c.cnt->n_seeds, 0, c.max_seeds, c.tile_sums, &c.cnt->n_track_clusters, c.n_sms, st)) return -1;
   k_finalize<<<1, 1, 0, st>>>(c, o);
   k_write<<<gw, kThreads, 0, st>>>(c, o);
+  k_params<<<grid_for(o.max_tracks, kThreads, c.n_sms, 8), kThreads, 0, st>>>(c, o);
   // tracklet ids (debug view, n_tracklets counter): nothing downstream waits for them
   k_kept<<<gs, kThreads, 0, st>>>(c);
   if (launch_scan_inclusive(c.kept_scan, &c.cnt->n_seeds, 0, c.max_seeds, c.tile_sums, &c.cnt->n_tracklets, c.n_sms, st)) return -1;
