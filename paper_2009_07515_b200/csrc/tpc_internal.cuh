@@ -115,10 +115,10 @@ int launches_reset(); int launches_s1(); int launches_s2(); int launches_s3(); i
 #ifdef __CUDACC__
 // floor(v) clamped to [0, hi]; NaN and negatives -> 0
 __device__ __forceinline__ int floor_clamp(float v, int hi) {
-  const float f = floorf(v);
-  if (!(f >= 0.0f)) return 0;
-  if (f >= (float)hi) return hi;
-  return (int)f;
+  // cvt.rmi.s32.f32 is floor() with saturation and NaN -> 0, so this is exactly
+  //   f = floorf(v); !(f >= 0) ? 0 : f >= (float)hi ? hi : (int)f      (hi >= 0)
+  // in three instructions
+  return min(max(__float2int_rd(v), 0), hi);
 }
 
 // order-preserving float <-> int key (signed compare)
