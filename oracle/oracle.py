@@ -57,6 +57,8 @@ def _load():
         lib.orc_kf_fit.restype = C.c_int
         lib.orc_kf_fit.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                    C.c_void_p, C.c_void_p]
+        lib.orc_beam_z.restype = C.c_double
+        lib.orc_beam_z.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double]
         assert lib.orc_params_size() == C.sizeof(_Params)
         _lib = lib
     return _lib
@@ -123,6 +125,10 @@ class Oracle:
         self._lib.orc_kf_update(C.byref(self._p), precision, par.ctypes.data, cov.ctypes.data, float(ym), float(zm_rel),
                                 c2.ctypes.data)
         return par, cov, float(c2[0])
+
+    def beam_z(self, x, y, z, tanl, qpt, precision=64) -> float:
+        """z of the track at the beam line, assuming a primary from the origin."""
+        return float(self._lib.orc_beam_z(C.byref(self._p), precision, float(x), float(y), float(z), float(tanl), float(qpt)))
 
     def kf_fit(self, x, y, z, precision=64):
         x = np.ascontiguousarray(x, dtype=np.float64); y = np.ascontiguousarray(y, dtype=np.float64)

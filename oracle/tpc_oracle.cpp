@@ -71,6 +71,29 @@ struct KF {
   T chi2;
 };
 
+// Beam-line z of a track ("Track seeds are extrapolated to the beam line and the most
+// likely z coordinate is computed under the assumption that the track is a primary and the vertex is at the origin").
+// A primary's circle passes through the origin of the xy plane: the chord d from the origin to (x, y) subtends the
+// turning angle theta with sin(theta/2) = |c| d / 2, the path length is d * asin(a)/a with a = |c| d / 2, and
+// z_beam = z - tan(lambda) * path.  asin(a)/a without libm: two half-angle reductions sin(t/2) = sin t / sqrt(2 (1 +
+// cos t)), then the 5-term series of section 3.4.1.
+template <class T>
+T beam_z(T kb, T x, T y, T z, T t, T q) {
+  const T c = kb * q;
+  const T d = std::sqrt(x * x + y * y);
+  T a = std::fabs((T(0.5) * c) * d);
+  if (!(a < T(1))) a = T(1);
+  const T c1 = std::sqrt(T(1) - a * a);
+  const T a1 = a / std::sqrt(T(2) * (T(1) + c1));
+  const T c2 = std::sqrt(T(1) - a1 * a1);
+  const T a2 = a1 / std::sqrt(T(2) * (T(1) + c2));
+  const T w = a2 * a2;
+  const T ser = T(1) + w * (T(1.0 / 6.0) + w * (T(3.0 / 40.0) + w * (T(5.0 / 112.0) + w * T(35.0 / 1152.0))));
+  const T ratio = a > T(0) ? (T(4) * (a2 * ser)) / a : T(1);
+  const T path = d * ratio;
+  return z - t * path;
+}
+
 // Helix step x -> x+dx in a uniform Bz (exact circle in xy), DESIGN.md section 3.4.1.
 // Returns false and leaves (p, C) untouched if |s| or |s1| >= max_sinphi.
 template <class T>
@@ -213,7 +236,8 @@ struct Oracle {
   std::vector<uint64_t> owner;                                    // [n] by sorted position
   std::vector<int32_t> k_owned;                                   // [n_seeds]
   std::vector<int32_t> trk_seed, trk_sector, trk_first_row, trk_last_row, trk_n_clusters, trk_ndf;
-  std::vector<double> trk_par, trk_cov, trk_x_ref, trk_z_ref, trk_chi2;
+  std::vector<double> trk_par, trk_cov, trk_x_ref, trk_z_ref, trk_chi2, trk_z_beam;
+  int s4_prec = 32;
   std::vector<int32_t> trk_cl_start, trk_cl_idx, cluster_track;
   std::vector<double> stage_seconds;                              // [5]
 
@@ -511,7 +535,7 @@ struct Oracle {
       }
     }
     trk_seed.clear(); trk_sector.clear(); trk_first_row.clear(); trk_last_row.clear(); trk_n_clusters.clear();
-    trk_ndf.clear(); trk_par.clear(); trk_cov.clear(); trk_x_ref.clear(); trk_z_ref.clear(); trk_chi2.clear();
+    trk_ndf.clear(); trk_par.clear(); trk_cov.clear(); trk_x_ref.clear(); trk_z_ref.clear(); trk_chi2.clear(); trk_z_beam.clear();
     trk_cl_start.assign(1, 0); trk_cl_idx.clear();
     cluster_track.assign(n, -1);
     for (size_t sd = 0; sd < K; ++sd) {
@@ -535,6 +559,13 @@ struct Oracle {
       for (int i = 0; i < 5; ++i) trk_par.push_back(t_par[sd * 5 + i]);
       for (int i = 0; i < 15; ++i) trk_cov.push_back(t_cov[sd * 15 + i]);
       trk_x_ref.push_back(t_x_ref[sd]); trk_z_ref.push_back(t_z_ref[sd]); trk_chi2.push_back(t_chi2[sd]);
+      // section 3.6: absolute pseudo-z of the state = z_ref + z_rel (one rounding), then the beam-line extrapolation
+      const double* pp = &t_par[sd * 5];
+      if (s4_prec == 64)
+        trk_z_beam.push_back(beam_z<double>((double)kb, t_x_ref[sd], pp[0], t_z_ref[sd] + pp[1], pp[3], pp[4]));
+      else
+        trk_z_beam.push_back((double)beam_z<float>(kb, (float)t_x_ref[sd], (float)pp[0], (float)t_z_ref[sd] + (float)pp[1],
+                                                   (float)pp[3], (float)pp[4]));
     }
   }
 
@@ -553,6 +584,7 @@ struct Oracle {
     stage3();
     auto t3 = now(); stage_seconds[2] = secs(t2, t3);
     if (last_stage < 4) return 0;
+    s4_prec = prec;
     if (prec == 64) stage4<double>(); else stage4<float>();
     auto t4 = now(); stage_seconds[3] = secs(t3, t4);
     if (last_stage < 5) return 0;
@@ -646,7 +678,7 @@ int orc_get(void* h, const char* name, const void** ptr, int64_t* n, int* kind) 
   F64(t_par); F64(t_cov); F64(t_x_ref); F64(t_z_ref); F64(t_chi2); I64(t_kf_steps);
   I32(tracklet_of_seed); U64(owner); I32(k_owned);
   I32(trk_seed); I32(trk_sector); I32(trk_first_row); I32(trk_last_row); I32(trk_n_clusters); I32(trk_ndf);
-  F64(trk_par); F64(trk_cov); F64(trk_x_ref); F64(trk_z_ref); F64(trk_chi2);
+  F64(trk_par); F64(trk_cov); F64(trk_x_ref); F64(trk_z_ref); F64(trk_chi2); F64(trk_z_beam);
   I32(trk_cl_start); I32(trk_cl_idx); I32(cluster_track); F64(stage_seconds);
   F32(up_dx); F32(up_ratio); F32(up_wy); F32(up_wz); F32(dn_dx); F32(dn_ratio); F32(dn_wy); F32(dn_wz);
 #undef I32
@@ -681,6 +713,14 @@ int orc_kf_fit(const void* params, int prec, int npt, const double* x, const dou
   const Params& P = *reinterpret_cast<const Params*>(params);
   return prec == 64 ? kf_fit_entry<double>(P, npt, x, y, z, par, cov15, chi2)
                     : kf_fit_entry<float>(P, npt, x, y, z, par, cov15, chi2);
+}
+
+// beam-line z of one state, for the pins (prec 32 or 64)
+double orc_beam_z(const void* params, int prec, double x, double y, double z, double tanl, double qpt) {
+  const Params& P = *static_cast<const Params*>(params);
+  const float kb = -0.00299792458f * P.bz_tesla;
+  if (prec == 64) return beam_z<double>((double)kb, x, y, z, tanl, qpt);
+  return (double)beam_z<float>(kb, (float)x, (float)y, (float)z, (float)tanl, (float)qpt);
 }
 
 }  // extern "C"
