@@ -117,6 +117,8 @@ typedef struct {
   int32_t* trk_cl_start;
   int32_t* trk_cl_idx;
   int32_t* cluster_track;
+  float* z_beam;          /* [max_tracks] pseudo-z of the track at the beam line, assuming a primary from the origin
+                           * (DESIGN.md section 3.6): vertex time = -+ z_beam / v_drift on the A / C side */
 } tpc_tracks_t;
 
 /* Small counter block read back by tpc_tracker_counters (sizes of the last run). */

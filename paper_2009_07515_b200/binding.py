@@ -37,7 +37,7 @@ class tpc_clusters_t(C.Structure):
 
 
 _TRACK_FIELDS = ["n_tracks", "status", "sector", "first_row", "last_row", "n_clusters", "par", "cov", "x_ref", "z_ref",
-                 "chi2", "ndf", "trk_cl_start", "trk_cl_idx", "cluster_track"]
+                 "chi2", "ndf", "trk_cl_start", "trk_cl_idx", "cluster_track", "z_beam"]
 
 
 class tpc_tracks_t(C.Structure):
@@ -155,6 +155,7 @@ class Tracks:
         self.n_clusters = i32(max_tracks)
         self.par = f32(5, max_tracks); self.cov = f32(15, max_tracks)
         self.x_ref = f32(max_tracks); self.z_ref = f32(max_tracks); self.chi2 = f32(max_tracks); self.ndf = i32(max_tracks)
+        self.z_beam = f32(max_tracks)
         self.trk_cl_start = i32(max_tracks + 1); self.trk_cl_idx = i32(max_track_clusters)
         self.cluster_track = i32(max(1, n_clusters))
         self.n_in = int(n_clusters)
@@ -170,7 +171,7 @@ class Tracks:
         """Bytes a host run copies back for the tracks found (d2h_bytes_per_step)."""
         T = int(self.n_tracks.item())
         ntc = int(self.trk_cl_start[T].item()) if T else 0
-        return 8 + T * 4 * (8 + 5 + 15) + (T + 1) * 4 + ntc * 4 + self.n_in * 4
+        return 8 + T * 4 * (9 + 5 + 15) + (T + 1) * 4 + ntc * 4 + self.n_in * 4
 
     def numpy(self) -> dict:
         """Host copies trimmed to the tracks found."""
@@ -184,6 +185,7 @@ class Tracks:
             sector=g(self.sector)[:T].copy(), first_row=g(self.first_row)[:T].copy(), last_row=g(self.last_row)[:T].copy(),
             n_clusters=g(self.n_clusters)[:T].copy(), par=g(self.par)[:, :T].T.copy(), cov=g(self.cov)[:, :T].T.copy(),
             x_ref=g(self.x_ref)[:T].copy(), z_ref=g(self.z_ref)[:T].copy(), chi2=g(self.chi2)[:T].copy(),
+            z_beam=g(self.z_beam)[:T].copy(),
             ndf=g(self.ndf)[:T].copy(), trk_cl_start=st, trk_cl_idx=g(self.trk_cl_idx)[: int(st[-1])].copy(),
             cluster_track=g(self.cluster_track)[: self.n_in].copy())
 

@@ -107,6 +107,7 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
     o.par = cv.take<float>(T * 5); o.cov = cv.take<float>(T * 15);
     o.x_ref = cv.take<float>(T); o.z_ref = cv.take<float>(T); o.chi2 = cv.take<float>(T); o.ndf = cv.take<int>(T);
     o.trk_cl_start = cv.take<int>(T + 1); o.trk_cl_idx = cv.take<int>(TC); o.cluster_track = cv.take<int>(N);
+    o.z_beam = cv.take<float>(T);
     o.max_tracks = (int)T; o.max_track_clusters = (int)TC;
   }
   *total = cv.off;
@@ -188,7 +189,7 @@ int run_device(tpc_tracker* t, const tpc_clusters_t* in, const OutPtrs& o, cudaS
 
 bool out_ok(const tpc_tracks_t* o) {
   return o && o->n_tracks && o->status && o->sector && o->first_row && o->last_row && o->n_clusters && o->par && o->cov &&
-         o->x_ref && o->z_ref && o->chi2 && o->ndf && o->trk_cl_start && o->trk_cl_idx && o->cluster_track &&
+         o->x_ref && o->z_ref && o->chi2 && o->ndf && o->trk_cl_start && o->trk_cl_idx && o->cluster_track && o->z_beam &&
          o->max_tracks >= 1 && o->max_track_clusters >= 1;
 }
 
@@ -197,7 +198,7 @@ OutPtrs to_out(const tpc_tracks_t* o) {
   r.n_tracks = o->n_tracks; r.status = o->status; r.sector = o->sector; r.first_row = o->first_row;
   r.last_row = o->last_row; r.n_clusters = o->n_clusters; r.par = o->par; r.cov = o->cov; r.x_ref = o->x_ref;
   r.z_ref = o->z_ref; r.chi2 = o->chi2; r.ndf = o->ndf; r.trk_cl_start = o->trk_cl_start; r.trk_cl_idx = o->trk_cl_idx;
-  r.cluster_track = o->cluster_track; r.max_tracks = (int)o->max_tracks; r.max_track_clusters = (int)o->max_track_clusters;
+  r.cluster_track = o->cluster_track; r.z_beam = o->z_beam; r.max_tracks = (int)o->max_tracks; r.max_track_clusters = (int)o->max_track_clusters;
   return r;
 }
 
@@ -213,7 +214,8 @@ bool copy_tracks_d2h(const OutPtrs& o, const tpc_tracks_t* out, size_t n, size_t
     ok = d2h(out->sector, o.sector, T * 4) && d2h(out->first_row, o.first_row, T * 4) &&
          d2h(out->last_row, o.last_row, T * 4) && d2h(out->n_clusters, o.n_clusters, T * 4) &&
          d2h(out->x_ref, o.x_ref, T * 4) && d2h(out->z_ref, o.z_ref, T * 4) && d2h(out->chi2, o.chi2, T * 4) &&
-         d2h(out->ndf, o.ndf, T * 4) && d2h(out->trk_cl_start, o.trk_cl_start, (T + 1) * 4);
+         d2h(out->ndf, o.ndf, T * 4) && d2h(out->z_beam, o.z_beam, T * 4) &&
+         d2h(out->trk_cl_start, o.trk_cl_start, (T + 1) * 4);
     for (int i = 0; i < 5 && ok; ++i) ok = d2h(out->par + i * mt, o.par + i * mt, T * 4);
     for (int i = 0; i < 15 && ok; ++i) ok = d2h(out->cov + i * mt, o.cov + i * mt, T * 4);
     ok = ok && d2h(out->trk_cl_idx, o.trk_cl_idx, n_tc * 4);

@@ -169,6 +169,23 @@ __global__ void __launch_bounds__(kThreads) k_write(Ctx c, OutPtrs o) {
   }
 }
 
+// pseudo-z of the track at the beam line, assuming a primary from the origin
+__device__ __forceinline__ float beam_z(float kb, float x, float y, float z, float t, float q) {
+  const float cv = kb * q;
+  const float d = sqrtf(x * x + y * y);
+  float a = fabsf((0.5f * cv) * d);
+  if (!(a < 1.0f)) a = 1.0f;
+  const float c1 = sqrtf(1.0f - a * a);
+  const float a1 = a / sqrtf(2.0f * (1.0f + c1));
+  const float c2 = sqrtf(1.0f - a1 * a1);
+  const float a2 = a1 / sqrtf(2.0f * (1.0f + c2));
+  const float w = a2 * a2;
+  const float ser = 1.0f + w * ((float)(1.0 / 6.0) + w * ((float)(3.0 / 40.0) + w * ((float)(5.0 / 112.0) + w * (float)(35.0 / 1152.0))));
+  const float ratio = a > 0.0f ? (4.0f * (a2 * ser)) / a : 1.0f;
+  const float path = d * ratio;
+  return z - t * path;
+}
+
 // Track parameters: one thread per TRACK id, so every output component is written with coalesced full-sector stores
 // (one warp per track wrote 29 scattered 4-byte stores per track: 50 M partial sectors on cfg5).
 __global__ void __launch_bounds__(kThreads) k_params(Ctx c, OutPtrs o) {
@@ -192,6 +209,7 @@ __global__ void __launch_bounds__(kThreads) k_params(Ctx c, OutPtrs o) {
     o.z_ref[id] = c.t_zref[sd];
     o.chi2[id] = c.t_chi2[sd];
     o.ndf[id] = 2 * c.t_n_hits[sd] - 5;
+    o.z_beam[id] = beam_z(c.kb, c.rowtab[low].x, p[0], c.t_zref[sd] + p[1], p[3], p[4]);
   }
   (void)R;
 }

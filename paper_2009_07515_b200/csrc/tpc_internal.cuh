@@ -97,6 +97,7 @@ int launch_s4(const Ctx& c, cudaStream_t st);
 struct OutPtrs {
   int* n_tracks; int* status; int* sector; int* first_row; int* last_row; int* n_clusters; float* par; float* cov;
   float* x_ref; float* z_ref; float* chi2; int* ndf; int* trk_cl_start; int* trk_cl_idx; int* cluster_track;
+  float* z_beam;
   int max_tracks; int max_track_clusters;
 };
 int launch_s5(const Ctx& c, const OutPtrs& o, cudaStream_t st);

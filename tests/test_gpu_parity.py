@@ -41,6 +41,7 @@ def _full_parity(tf, exact_assignment):
                       np.maximum(np.abs(o.get("trk_par").reshape(-1, 5)), [1, 1, .1, .1, .1])) <= PAR_TOL
         assert np.array_equal(g["x_ref"], o.get("trk_x_ref").astype(np.float32))
         assert np.array_equal(g["z_ref"], o.get("trk_z_ref").astype(np.float32))
+        assert np.array_equal(g["z_beam"], o.get("trk_z_beam").astype(np.float32))     # DESIGN.md 3.6, bit-exact
     # counters agree with the oracle's own sizes
     assert k["n_seeds"] == o.get("seed_head").shape[0]
     assert k["n_tracklets"] == int(o.get("t_kept").sum())
@@ -76,6 +77,9 @@ def test_reports_bit_exactness(mini_event):
     res = compare_tracks(out.numpy(), o, mini_event.n)
     assert t["hit_mismatch_seeds"] == 0 and t["par_bitexact"] and t["cov_bitexact"] and t["chi2_bitexact"], t
     assert res["cluster_track_equal"] and res["csr_equal"], res
+    zb_g, zb_o = out.numpy()["z_beam"], o.get("trk_z_beam")
+    assert zb_g.shape == zb_o.shape and np.array_equal(zb_g, zb_o.astype(np.float32))
+    assert np.max(np.abs(zb_g - zb_o) / np.maximum(np.abs(zb_o), 1.0)) <= PAR_TOL   # the stated bar: 1e-4 relative
 
 
 def test_host_path_equals_device_path(mini_event):
@@ -185,6 +189,7 @@ def test_full_size_sector_sample():
         par_g = g["par"][first:first + To]; par_o = o.get("trk_par").reshape(-1, 5)
         rel = np.abs(par_g - par_o) / np.maximum(np.abs(par_o), [1, 1, .1, .1, .1])
         assert float((rel.max(axis=1) <= PAR_TOL).mean()) >= 0.995, (s, float(rel.max()))
+        assert np.array_equal(g["z_beam"][first:first + To], o.get("trk_z_beam").astype(np.float32))
         print(f"sector {s}: {sub.n} clusters, {To} tracks, assignment identical for {same:.6f}, par max rel {rel.max():.2e}")
 
 
