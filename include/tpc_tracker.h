@@ -177,7 +177,7 @@ typedef struct {
 
 /* Bytes of DEVICE workspace the tracker needs for the given capacities.  `host_io` = 1 adds the
  * staging buffers tpc_track_timeframe_host uses (inputs for max_clusters, outputs for max_tracks /
- * max_track_clusters); `host_io` = 2 adds two such sets for the pipelined begin/end pair.  Returns 0 on invalid arguments. */
+ * max_track_clusters); `host_io` = 2 or 3 adds that many sets for the pipelined begin/end pair (0 <= host_io <= 3).  Returns 0 on invalid arguments. */
 TPC_API size_t tpc_tracker_workspace_bytes(const tpc_params_t* params, int64_t max_clusters, int64_t max_bins,
                                    int64_t max_seeds, int64_t max_tracks, int64_t max_track_clusters,
                                    int32_t host_io);
@@ -201,12 +201,13 @@ TPC_API int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, cons
  * capacities; the per-track arrays are copied for the n_tracks tracks found. */
 TPC_API int tpc_track_timeframe_host(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tracks_t* out, void* cuda_stream);
 
-/* Pipelined host path (tracker created with host_io == 2; BASELINE.json north_star: whole time frames arrive one
+/* Pipelined host path (tracker created with host_io = 2 or 3 = number of staging slots; BASELINE.json north_star: whole time frames arrive one
  * after the other).  `begin` enqueues the H2D copy of one frame's HOST (pinned) inputs and its
  * S1..S5 on streams the library owns and returns without waiting; `end` waits for that frame, copies exactly the
  * tracks found into the caller's HOST buffers (capacities must equal the tracker's) and returns when they are there.
- * Two frames may be in flight (slot 0 and slot 1, begin/end strictly alternating per slot): the copies of one frame
- * overlap the kernels of the other.  Inputs must stay valid and unchanged until the matching `end` returns.
+ * host_io frames may be in flight (slots 0 .. host_io-1, begin/end strictly alternating per slot): the copies of one
+ * frame overlap the kernels of another; with 3 slots the upload of frame i+1 can be started before the download of
+ * frame i-1 has been collected, which keeps all three streams busy.  Inputs must stay valid and unchanged until the matching `end` returns.
  * Returns INVALID_ARG for a slot used out of order. */
 TPC_API int tpc_track_timeframe_host_begin(tpc_tracker_t* t, const tpc_clusters_t* in, int32_t slot);
 TPC_API int tpc_track_timeframe_host_end(tpc_tracker_t* t, const tpc_tracks_t* out, int32_t slot);

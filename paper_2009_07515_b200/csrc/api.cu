@@ -12,6 +12,8 @@
 
 using namespace tpc;
 
+constexpr int kMaxSlots = 3;          // host_io = number of staging slots (0 none, 1 synchronous host path, 2-3 pipelined)
+
 struct tpc_tracker {
   tpc_params_t params;            // row_x pointer is NOT kept (copied into rowtab)
   Ctx ctx;                        // pointers into the workspace; input fields set per call
@@ -24,8 +26,8 @@ struct tpc_tracker {
     int64_t n;
     cudaEvent_t h2d_done, in_free, done, out_free;   // pipelined path only
     bool busy;
-  } slot[2];
-  cudaStream_t s_in, s_compute, s_out;                // pipelined path only (host_io == 2)
+  } slot[kMaxSlots];
+  cudaStream_t s_in, s_compute, s_out;                // pipelined path only (host_io >= 2)
   int* h_counts;                                      // pinned host: [slot][4] = n_tracks, status, n_track_clusters, -
   cudaStream_t last_stream;
   bool timing;
@@ -96,7 +98,7 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   c.surv_scan = cv.take<int>(K); c.owned_scan = cv.take<int>(K);
   c.mask_words = (R + 31) / 32;
   c.own_mask = cv.take<unsigned>(K * (size_t)c.mask_words);
-  for (int k = 0; k < (t->host_io >= 2 ? 2 : t->host_io ? 1 : 0); ++k) {
+  for (int k = 0; k < t->host_io; ++k) {
     const size_t T = (size_t)t->max_tracks, TC = (size_t)t->max_track_clusters;
     tpc_tracker::Slot& sl = t->slot[k];
     sl.sector = cv.take<uint8_t>(N); sl.row = cv.take<uint8_t>(N);
@@ -232,6 +234,7 @@ extern "C" {
 size_t tpc_tracker_workspace_bytes(const tpc_params_t* params, int64_t max_clusters, int64_t max_bins, int64_t max_seeds,
                                    int64_t max_tracks, int64_t max_track_clusters, int32_t host_io) {
   if (!params_ok(params) || !caps_ok(max_clusters, max_bins, max_seeds, max_tracks, max_track_clusters)) return 0;
+  if (host_io < 0 || host_io > kMaxSlots) return 0;
   tpc_tracker tmp{};
   tmp.params = *params;
   tmp.max_clusters = max_clusters; tmp.max_bins = max_bins; tmp.max_seeds = max_seeds;
@@ -247,6 +250,7 @@ int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t
   if (!out) return TPC_ERR_INVALID_ARG;
   *out = nullptr;
   if (!params_ok(params) || !caps_ok(max_clusters, max_bins, max_seeds, max_tracks, max_track_clusters)) return TPC_ERR_INVALID_ARG;
+  if (host_io < 0 || host_io > kMaxSlots) return TPC_ERR_INVALID_ARG;
   if (!d_workspace || !aligned(d_workspace, kAlign)) return TPC_ERR_INVALID_ARG;
   tpc_tracker* t = new (std::nothrow) tpc_tracker{};
   if (!t) return TPC_ERR_INVALID_ARG;
@@ -277,7 +281,7 @@ int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t
     bool ok = cudaStreamCreateWithFlags(&t->s_in, cudaStreamNonBlocking) == cudaSuccess &&
               cudaStreamCreateWithFlags(&t->s_compute, cudaStreamNonBlocking) == cudaSuccess &&
               cudaStreamCreateWithFlags(&t->s_out, cudaStreamNonBlocking) == cudaSuccess &&
-              cudaHostAlloc(reinterpret_cast<void**>(&t->h_counts), 8 * sizeof(int), cudaHostAllocDefault) == cudaSuccess;
+              cudaHostAlloc(reinterpret_cast<void**>(&t->h_counts), 4 * kMaxSlots * sizeof(int), cudaHostAllocDefault) == cudaSuccess;
     for (auto& sl : t->slot)
       for (cudaEvent_t* e : {&sl.h2d_done, &sl.in_free, &sl.done, &sl.out_free})
         ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
@@ -332,12 +336,13 @@ int tpc_track_timeframe_host(tpc_tracker_t* t, const tpc_clusters_t* in, const t
   return TPC_OK;
 }
 
-// ---- pipelined host path (host_io == 2): H2D of frame i+1 and D2H of frame i-1 overlap the kernels of frame i.
+// ---- pipelined host path (host_io = 2 or 3 staging slots): H2D of frame i+1 and D2H of frame i-1 overlap the
+// kernels of frame i (with 3 slots the next upload does not have to wait for the previous download to be collected).
 // Three library-owned streams; two staging slots; events order the reuse of a slot's input staging (free once S1 of
 // the frame that used it has run), of its output staging (free once its D2H has finished) and of the single workspace
 // (frames compute one after the other on s_compute).
 int tpc_track_timeframe_host_begin(tpc_tracker_t* t, const tpc_clusters_t* in, int32_t slot) {
-  if (!t || !in || t->host_io < 2 || slot < 0 || slot > 1) return TPC_ERR_INVALID_ARG;
+  if (!t || !in || t->host_io < 2 || slot < 0 || slot >= t->host_io) return TPC_ERR_INVALID_ARG;
   if (in->n < 0 || (in->n > 0 && (!in->sector || !in->row || !in->y || !in->z))) return TPC_ERR_INVALID_ARG;
   if (in->n > t->max_clusters) return TPC_ERR_CAPACITY;
   tpc_tracker::Slot& sl = t->slot[slot];
@@ -371,7 +376,7 @@ int tpc_track_timeframe_host_begin(tpc_tracker_t* t, const tpc_clusters_t* in, i
 }
 
 int tpc_track_timeframe_host_end(tpc_tracker_t* t, const tpc_tracks_t* out, int32_t slot) {
-  if (!t || !out_ok(out) || t->host_io < 2 || slot < 0 || slot > 1) return TPC_ERR_INVALID_ARG;
+  if (!t || !out_ok(out) || t->host_io < 2 || slot < 0 || slot >= t->host_io) return TPC_ERR_INVALID_ARG;
   tpc_tracker::Slot& sl = t->slot[slot];
   if (!sl.busy) return TPC_ERR_INVALID_ARG;
   if (out->max_tracks != t->max_tracks || out->max_track_clusters != t->max_track_clusters) return TPC_ERR_INVALID_ARG;

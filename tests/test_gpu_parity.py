@@ -206,10 +206,11 @@ def test_wide_ownership_keys(mini_event):
     assert np.array_equal(trk32.stage_view("k_owned"), trk64.stage_view("k_owned")[: trk32.stage_view("k_owned").shape[0]])
 
 
-def test_pipelined_host_path(mini_event, mini_tf):
-    """tpc_track_timeframe_host_begin/_end with two frames in flight gives, frame by frame, what the device path gives."""
+@pytest.mark.parametrize("slots", [2, 3])
+def test_pipelined_host_path(mini_event, mini_tf, slots):
+    """tpc_track_timeframe_host_begin/_end with `slots` frames in flight gives, frame by frame, what the device path gives."""
     import paper_2009_07515_b200 as tpc
-    frames = [mini_event, mini_tf, mini_event, mini_tf, mini_tf]
+    frames = [mini_event, mini_tf, mini_event, mini_tf, mini_tf, mini_event, mini_event]
     P = default_params(mini_event)
     want = {}
     for tf in (mini_event, mini_tf):
@@ -218,31 +219,35 @@ def test_pipelined_host_path(mini_event, mini_tf):
     nmax = max(tf.n for tf in frames)
     c = tpc.suggest_capacities(nmax, P)
     nb = max(tpc.max_bins_bound(tf.sector, tf.z, P) for tf in frames)
-    trk = tpc.Tracker(P, c["max_clusters"], nb, c["max_seeds"], c["max_tracks"], c["max_track_clusters"], host_io=2)
+    trk = tpc.Tracker(P, c["max_clusters"], nb, c["max_seeds"], c["max_tracks"], c["max_track_clusters"], host_io=slots)
     th = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()  # noqa: E731
     pinned = {id(tf): [th(a) for a in (tf.sector, tf.row, tf.y, tf.z)] for tf in (mini_event, mini_tf)}
-    outs = [trk.new_tracks(nmax, host=True) for _ in range(2)]
+    outs = [trk.new_tracks(nmax, host=True) for _ in range(slots)]
     got = []
 
     def finish(i):
-        trk.track_timeframe_host_end(outs[i % 2], i % 2)
-        o = outs[i % 2]; o.n_in = frames[i].n
+        trk.track_timeframe_host_end(outs[i % slots], i % slots)
+        o = outs[i % slots]; o.n_in = frames[i].n
         got.append(o.numpy())
 
-    trk.track_timeframe_host_begin(*pinned[id(frames[0])], 0)
-    for i in range(1, len(frames)):
-        trk.track_timeframe_host_begin(*pinned[id(frames[i])], i % 2)
-        finish(i - 1)
-    finish(len(frames) - 1)
+    for i in range(len(frames)):
+        trk.track_timeframe_host_begin(*pinned[id(frames[i])], i % slots)
+        if i >= slots - 1:
+            finish(i - (slots - 1))
+    for j in range(len(frames) - (slots - 1), len(frames)):
+        finish(j)
+    assert len(got) == len(frames)
     for tf, g in zip(frames, got):
         w = want[id(tf)]
         assert g["status"] == 0 and g["n_tracks"] == w["n_tracks"] > 0
         for k in w:
             if isinstance(w[k], np.ndarray):
                 assert np.array_equal(g[k], w[k]), k
-    # a slot used out of order is refused
+    # a slot used out of order, or one the tracker does not have, is refused
     with pytest.raises(RuntimeError):
         trk.track_timeframe_host_end(outs[0], 0)
+    with pytest.raises(RuntimeError):
+        trk.track_timeframe_host_begin(*pinned[id(mini_event)], slots)
 
 
 def test_crowded_slab_falls_back_and_stays_exact():
