@@ -18,6 +18,11 @@
 // [first_row, last_row] are all defined and nothing outside that range is ever read (S5 and the debug
 // view honour the range).
 //
+// Measured and rejected on cfg5 (this version: 12.8 ms): the searches of a warp laid end to end and tested 32
+// candidates at a time (warp scan, owner lookup, 64-bit shared-memory atomicMin of (d2, position)): 12.9 ms, bit-exact
+// but no faster; the known-cluster loads hoisted above the transport: no change; S5's ownership votes cast by the
+// finishing lane: S4 +4.2 ms for S5 -2.8 ms; 8 CTAs per SM (64 registers, spills): 14.7 ms.
+//
 // Arithmetic is written operation by operation in the order of DESIGN.md section 3.4 (compiled with
 // -fmad=false): the transport J C J^T skips only the terms that are structurally 0*x or 1*x.
 #include "tpc_internal.cuh"
