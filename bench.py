@@ -49,12 +49,16 @@ def parse():
 
 def ncu_traffic(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on cfg5, copied from the committed
-    `ncu --set full` capture (profiles/traffic.json names the capture); None if there is none."""
+    `ncu --set full` capture (profiles/traffic.csv names the capture); None if there is none."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return float(json.load(f)[kernel]["dram_bytes"])
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for ln in f:
+                p = ln.strip().split(",")
+                if p[0] == kernel:
+                    return float(p[1])
     except Exception:
-        return None
+        pass
+    return None
 
 
 def hbm_peak():
