@@ -13,8 +13,9 @@
 // paper_2009_07515_b200/csrc (the CUDA product) and neither includes the other.
 //
 // Arithmetic contract: fp32, round-to-nearest-even, one rounding per written
-// operation, evaluation order exactly as written, no FMA contraction (build with
-// -ffp-contract=off, no -ffast-math), only + - * / sqrt floor fabs.  Stage 4 is templated on the
+// operation, evaluation order exactly as written, no FMA contraction by the compiler (build with
+// -ffp-contract=off, no -ffast-math), only + - * / sqrt floor fabs and - in the Kalman transport and update of
+// stage 4 only - the fused multiply-add std::fma exactly where DESIGN.md sections 3.4.1 / 3.4.2 write fma().  Stage 4 is templated on the
 // scalar: the float instance is the parity reference, the double instance exists for the
 // analytic pins (tests/test_oracle_*.py) and to measure the fp32 error.
 //
@@ -100,32 +101,32 @@ template <class T>
 bool kf_propagate(KF<T>& k, T kb, T dx, T max_sinphi, T* jac_out /*25, row-major, may be null*/) {
   const T y = k.p[0], z = k.p[1], s = k.p[2], t = k.p[3], q = k.p[4];
   const T c = kb * q;                                   // curvature
-  const T s1 = s + c * dx;
+  const T s1 = std::fma(c, dx, s);
   if (!(std::fabs(s) < max_sinphi) || !(std::fabs(s1) < max_sinphi)) return false;
-  const T c0 = std::sqrt(T(1) - s * s);
-  const T c1 = std::sqrt(T(1) - s1 * s1);
+  const T c0 = std::sqrt(std::fma(-s, s, T(1)));
+  const T c1 = std::sqrt(std::fma(-s1, s1, T(1)));
   const T cc = c0 + c1;
   const T ss = s + s1;
   const T Tn = ss / cc;                                 // tan of the chord direction
-  const T y1 = y + dx * Tn;
-  const T dl = dx * std::sqrt(T(1) + Tn * Tn);          // signed chord length
+  const T y1 = std::fma(dx, Tn, y);
+  const T dl = dx * std::sqrt(std::fma(Tn, Tn, T(1)));  // signed chord length
   const T u = (T(0.5) * c) * dl;
   const T w = u * u;
   // asin(u)/u = 1 + w/6 + 3w^2/40 + 5w^3/112 + 35w^4/1152 + ...   (no libm transcendental)
-  const T ser = T(1) + w * (T(1.0 / 6.0) + w * (T(3.0 / 40.0) + w * (T(5.0 / 112.0) + w * T(35.0 / 1152.0))));
+  const T ser = std::fma(w, std::fma(w, std::fma(w, std::fma(w, T(35.0 / 1152.0), T(5.0 / 112.0)), T(3.0 / 40.0)), T(1.0 / 6.0)), T(1));
   const T arc = dl * ser;                               // signed xy arc length
-  const T z1 = z + t * arc;
+  const T z1 = std::fma(t, arc, z);
 
   // Jacobian d(p1)/d(p0); identity except the six entries below.
   const T c0c1 = c0 * c1;
   const T kdx = kb * dx;
-  const T j_ys = dx * (c0 + s * Tn) / c0c1;
-  const T j_yq = (kdx * dx) * (c1 * cc + s1 * ss) / (c1 * (cc * cc));
+  const T j_ys = dx * std::fma(s, Tn, c0) / c0c1;
+  const T j_yq = (kdx * dx) * std::fma(s1, ss, c1 * cc) / (c1 * (cc * cc));
   const T j_sq = kdx;
   const T j_zt = arc;
   const T j_zs = (t * dx) * Tn / c0c1;
-  const T sm = s + (T(0.5) * c) * dx;                   // sin(phi) at the step midpoint (Simpson)
-  const T cm = std::sqrt(T(1) - sm * sm);
+  const T sm = std::fma(T(0.5) * c, dx, s);             // sin(phi) at the step midpoint (Simpson)
+  const T cm = std::sqrt(std::fma(-sm, sm, T(1)));
   const T j_zq = ((t * kdx) * dx) * T(1.0 / 6.0) * (T(2) * sm / (cm * cm * cm) + s1 / (c1 * c1 * c1));
 
   T J[5][5];
@@ -133,19 +134,20 @@ bool kf_propagate(KF<T>& k, T kb, T dx, T max_sinphi, T* jac_out /*25, row-major
     for (int j = 0; j < 5; ++j) J[i][j] = (i == j) ? T(1) : T(0);
   J[0][2] = j_ys; J[0][4] = j_yq; J[1][2] = j_zs; J[1][3] = j_zt; J[1][4] = j_zq; J[2][4] = j_sq;
 
-  // C1 = J C J^T: M = J C (k ascending), C1[i][j] = sum_l M[i][l] J[j][l] (l ascending) for i >= j, mirrored.
+  // C1 = J C J^T: M = J C (k ascending), C1[i][j] = sum_l M[i][l] J[j][l] (l ascending) for i >= j, mirrored; every
+  // term enters its sum by one fused multiply-add.
   T M[5][5];
   for (int i = 0; i < 5; ++i)
     for (int l = 0; l < 5; ++l) {
       T acc = T(0);
-      for (int kk = 0; kk < 5; ++kk) acc = acc + J[i][kk] * k.C[kk][l];
+      for (int kk = 0; kk < 5; ++kk) acc = std::fma(J[i][kk], k.C[kk][l], acc);
       M[i][l] = acc;
     }
   T C1[5][5];
   for (int i = 0; i < 5; ++i)
     for (int j = 0; j <= i; ++j) {
       T acc = T(0);
-      for (int l = 0; l < 5; ++l) acc = acc + M[i][l] * J[j][l];
+      for (int l = 0; l < 5; ++l) acc = std::fma(M[i][l], J[j][l], acc);
       C1[i][j] = acc;
       C1[j][i] = acc;
     }
@@ -167,23 +169,23 @@ void kf_update(KF<T>& k, T ym, T zm, T err_y2, T err_z2) {
   const T S00 = k.C[0][0] + err_y2;
   const T S10 = k.C[1][0];
   const T S11 = k.C[1][1] + err_z2;
-  const T det = S00 * S11 - S10 * S10;
+  const T det = std::fma(S00, S11, -(S10 * S10));
   const T idet = T(1) / det;
   const T I00 = S11 * idet, I10 = (T(0) - S10) * idet, I11 = S00 * idet;   // S^-1 (symmetric)
-  k.chi2 = k.chi2 + ((r0 * r0) * I00 + (T(2) * (r0 * r1)) * I10 + (r1 * r1) * I11);
+  k.chi2 = k.chi2 + std::fma(r1 * r1, I11, std::fma(T(2) * (r0 * r1), I10, (r0 * r0) * I00));
   T K0[5], K1[5];                                       // gain K = C H^T S^-1   (5x2)
   for (int i = 0; i < 5; ++i) {
-    K0[i] = k.C[i][0] * I00 + k.C[i][1] * I10;
-    K1[i] = k.C[i][0] * I10 + k.C[i][1] * I11;
+    K0[i] = std::fma(k.C[i][1], I10, k.C[i][0] * I00);
+    K1[i] = std::fma(k.C[i][1], I11, k.C[i][0] * I10);
   }
   T C1[5][5];
   for (int i = 0; i < 5; ++i)
     for (int j = 0; j <= i; ++j) {                      // C -= K (H C), lower triangle then mirror
-      const T v = k.C[i][j] - (K0[i] * k.C[0][j] + K1[i] * k.C[1][j]);
+      const T v = std::fma(-K1[i], k.C[1][j], std::fma(-K0[i], k.C[0][j], k.C[i][j]));
       C1[i][j] = v;
       C1[j][i] = v;
     }
-  for (int i = 0; i < 5; ++i) k.p[i] = k.p[i] + (K0[i] * r0 + K1[i] * r1);
+  for (int i = 0; i < 5; ++i) k.p[i] = std::fma(K1[i], r1, std::fma(K0[i], r0, k.p[i]));
   for (int i = 0; i < 5; ++i)
     for (int j = 0; j < 5; ++j) k.C[i][j] = C1[i][j];
 }
