@@ -239,6 +239,10 @@ struct Oracle {
   std::vector<int32_t> k_owned;                                   // [n_seeds]
   std::vector<int32_t> trk_seed, trk_sector, trk_first_row, trk_last_row, trk_n_clusters, trk_ndf;
   std::vector<double> trk_par, trk_cov, trk_x_ref, trk_z_ref, trk_chi2, trk_z_beam;
+  std::vector<int32_t> trk_cl_pos;                                 // sorted positions parallel to trk_cl_idx
+  // S7 refit over the owned clusters
+  std::vector<double> fit_par, fit_cov, fit_x_ref, fit_z_ref, fit_chi2;
+  std::vector<int32_t> fit_ndf, fit_n;
   int s4_prec = 32;
   std::vector<int32_t> trk_cl_start, trk_cl_idx, cluster_track;
   std::vector<double> stage_seconds;                              // [5]
@@ -538,7 +542,7 @@ struct Oracle {
     }
     trk_seed.clear(); trk_sector.clear(); trk_first_row.clear(); trk_last_row.clear(); trk_n_clusters.clear();
     trk_ndf.clear(); trk_par.clear(); trk_cov.clear(); trk_x_ref.clear(); trk_z_ref.clear(); trk_chi2.clear(); trk_z_beam.clear();
-    trk_cl_start.assign(1, 0); trk_cl_idx.clear();
+    trk_cl_start.assign(1, 0); trk_cl_idx.clear(); trk_cl_pos.clear();
     cluster_track.assign(n, -1);
     for (size_t sd = 0; sd < K; ++sd) {
       if (!t_kept[sd] || k_owned[sd] < P.min_track_hits) continue;
@@ -551,6 +555,7 @@ struct Oracle {
           if (first < 0) first = r;
           lastr = r;
           trk_cl_idx.push_back(perm[c]);
+          trk_cl_pos.push_back(c);
           cluster_track[perm[c]] = id;
         }
       }
@@ -568,6 +573,43 @@ struct Oracle {
       else
         trk_z_beam.push_back((double)beam_z<float>(kb, (float)t_x_ref[sd], (float)pp[0], (float)t_z_ref[sd] + (float)pp[1],
                                                    (float)pp[3], (float)pp[4]));
+    }
+  }
+
+  // ---------------------------------------------------------------------------------------- S7
+  // Refit of every track over the clusters it OWNS after the selector, top row downwards (
+  // PAPER.md:99, 138 "Track Fit": the step after track finding; here without merging and without corrections).
+  // Seed at the top owned cluster from the direction to the next lower one (the S4 seed rule, oriented towards +x),
+  // q/pT of the track as the starting value, initial covariance, chi2 = 0; then propagate + update (no gate) through
+  // the owned clusters in descending row.  A failed propagation stops the fit at the last updated cluster.
+  template <class T>
+  void stage6() {
+    const size_t nt = trk_seed.size();
+    fit_par.assign(nt * 5, 0.0); fit_cov.assign(nt * 15, 0.0); fit_x_ref.assign(nt, 0.0); fit_z_ref.assign(nt, 0.0);
+    fit_chi2.assign(nt, 0.0); fit_ndf.assign(nt, 0); fit_n.assign(nt, 0);
+    const T kbT = T(kb), msp = T(P.max_sinphi), ey2 = T(P.err_y2), ez2 = T(P.err_z2);
+    for (size_t id = 0; id < nt; ++id) {
+      const int32_t* cl = &trk_cl_pos[trk_cl_start[id]];
+      const int m = trk_cl_start[id + 1] - trk_cl_start[id];
+      if (m < 2) continue;                                  // cannot happen with min_track_hits >= 2
+      const int top = cl[m - 1], nxt = cl[m - 2];
+      const T zref = T(zs[top]);
+      const T dx = T(P.row_x[s_row[top]]) - T(P.row_x[s_row[nxt]]);
+      const T dy = T(ys[top]) - T(ys[nxt]), dz = T(zs[top]) - T(zs[nxt]);
+      const T dl = std::sqrt(dx * dx + dy * dy);
+      KF<T> k;
+      k.p[0] = T(ys[top]); k.p[1] = T(0); k.p[2] = dy / dl; k.p[3] = dz / dl; k.p[4] = T(trk_par[id * 5 + 4]);
+      kf_reset_cov(k, P);
+      int cur = s_row[top], nfit = 1;
+      for (int i = m - 2; i >= 0; --i) {
+        const int c = cl[i], r = s_row[c];
+        if (!kf_propagate<T>(k, kbT, T(P.row_x[r]) - T(P.row_x[cur]), msp, (T*)nullptr)) break;
+        kf_update<T>(k, T(ys[c]), T(zs[c]) - zref, ey2, ez2);
+        cur = r; ++nfit;
+      }
+      store_kf(k, &fit_par[id * 5], &fit_cov[id * 15], &fit_chi2[id]);
+      fit_x_ref[id] = (double)P.row_x[cur]; fit_z_ref[id] = (double)zref;
+      fit_n[id] = nfit; fit_ndf[id] = 2 * nfit - 5;
     }
   }
 
@@ -592,6 +634,8 @@ struct Oracle {
     if (last_stage < 5) return 0;
     stage5();
     auto t5 = now(); stage_seconds[4] = secs(t4, t5);
+    if (last_stage < 6) return 0;
+    if (prec == 64) stage6<double>(); else stage6<float>();
     return 0;
   }
 };
@@ -658,7 +702,7 @@ void* orc_create(const void* params) { return new Oracle(*reinterpret_cast<const
 void orc_destroy(void* h) { delete reinterpret_cast<Oracle*>(h); }
 int orc_params_size() { return (int)sizeof(Params); }
 
-// prec: 32 (parity reference) or 64; last_stage: 1..5
+// prec: 32 (parity reference) or 64; last_stage: 1..5, 6 = also the refit of section 3.7
 int orc_run(void* h, int64_t n, const uint8_t* sector, const uint8_t* row, const float* y, const float* z, int prec,
             int last_stage) {
   return reinterpret_cast<Oracle*>(h)->run(n, sector, row, y, z, prec, last_stage);
@@ -681,7 +725,8 @@ int orc_get(void* h, const char* name, const void** ptr, int64_t* n, int* kind) 
   I32(tracklet_of_seed); U64(owner); I32(k_owned);
   I32(trk_seed); I32(trk_sector); I32(trk_first_row); I32(trk_last_row); I32(trk_n_clusters); I32(trk_ndf);
   F64(trk_par); F64(trk_cov); F64(trk_x_ref); F64(trk_z_ref); F64(trk_chi2); F64(trk_z_beam);
-  I32(trk_cl_start); I32(trk_cl_idx); I32(cluster_track); F64(stage_seconds);
+  I32(trk_cl_start); I32(trk_cl_idx); I32(trk_cl_pos); I32(cluster_track); F64(stage_seconds);
+  F64(fit_par); F64(fit_cov); F64(fit_x_ref); F64(fit_z_ref); F64(fit_chi2); I32(fit_ndf); I32(fit_n);
   F32(up_dx); F32(up_ratio); F32(up_wy); F32(up_wz); F32(dn_dx); F32(dn_ratio); F32(dn_wy); F32(dn_wz);
 #undef I32
 #undef F32
