@@ -201,6 +201,24 @@ TPC_API int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, cons
  * capacities; the per-track arrays are copied for the n_tracks tracks found. */
 TPC_API int tpc_track_timeframe_host(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tracks_t* out, void* cuda_stream);
 
+/* Refitted tracks (DEVICE pointers, caller-allocated for max_tracks tracks; layouts as in tpc_tracks_t). */
+typedef struct {
+  int64_t max_tracks;
+  float* par;        /* [5][max_tracks] */
+  float* cov;        /* [15][max_tracks] */
+  float* x_ref;      /* [max_tracks] x of the lowest fitted row */
+  float* z_ref;      /* [max_tracks] z of the top owned cluster: absolute z = par[1] + z_ref */
+  float* chi2;       /* [max_tracks] */
+  int32_t* ndf;      /* [max_tracks] 2*n_fit - 5 */
+  int32_t* n_fit;    /* [max_tracks] clusters that entered the fit */
+} tpc_fit_t;
+
+/* Refit of every track of the LAST tpc_track_timeframe call on this handle over the clusters it owns after the
+ * selector, top row downwards (the first slice of "Track Fit").  Enqueued on
+ * `cuda_stream`, which must be ordered after that call; does not synchronise; entries [0, n_tracks) are written.
+ * Not part of tpc_track_timeframe (and not of the timed hot path).  CAPACITY if out->max_tracks exceeds the tracker's. */
+TPC_API int tpc_tracker_refit(tpc_tracker_t* t, const tpc_fit_t* out, void* cuda_stream);
+
 /* Pipelined host path (tracker created with host_io = 2 or 3 = number of staging slots; BASELINE.json north_star: whole time frames arrive one
  * after the other).  `begin` enqueues the H2D copy of one frame's HOST (pinned) inputs and its
  * S1..S5 on streams the library owns and returns without waiting; `end` waits for that frame, copies exactly the

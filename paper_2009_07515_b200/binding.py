@@ -44,6 +44,10 @@ class tpc_tracks_t(C.Structure):
     _fields_ = [("max_tracks", C.c_int64), ("max_track_clusters", C.c_int64)] + [(f, C.c_void_p) for f in _TRACK_FIELDS]
 
 
+class tpc_fit_t(C.Structure):
+    _fields_ = [("max_tracks", C.c_int64)] + [(f, C.c_void_p) for f in ("par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit")]
+
+
 class tpc_counters_t(C.Structure):
     _fields_ = [("n_clusters", C.c_int64), ("n_bins", C.c_int64), ("n_seeds", C.c_int64), ("n_tracklets", C.c_int64),
                 ("n_tracks", C.c_int64), ("n_track_clusters", C.c_int64), ("n_linked", C.c_int64),
@@ -64,7 +68,7 @@ STATUS_BITS = {1: "BAD_CLUSTER", 2: "BINS_OVERFLOW", 4: "SEEDS_OVERFLOW", 8: "TR
 
 EXPORTS = [
     "tpc_tracker_workspace_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
-    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end",
+    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit",
     "tpc_tracker_counters", "tpc_tracker_enable_stage_timing", "tpc_tracker_stage_ms", "tpc_tracker_stage_view",
     "tpc_tracker_launches_per_call", "tpc_tracker_destroy", "tpc_error_string",
 ]
@@ -105,6 +109,8 @@ def load_library(build: bool = True) -> C.CDLL:
     lib.tpc_track_timeframe_host_begin.argtypes = [C.c_void_p, P(tpc_clusters_t), C.c_int32]
     lib.tpc_track_timeframe_host_end.restype = C.c_int
     lib.tpc_track_timeframe_host_end.argtypes = [C.c_void_p, P(tpc_tracks_t), C.c_int32]
+    lib.tpc_tracker_refit.restype = C.c_int
+    lib.tpc_tracker_refit.argtypes = [C.c_void_p, P(tpc_fit_t), C.c_void_p]
     lib.tpc_tracker_counters.restype = C.c_int
     lib.tpc_tracker_counters.argtypes = [C.c_void_p, P(tpc_counters_t)]
     lib.tpc_tracker_enable_stage_timing.restype = C.c_int
@@ -268,6 +274,33 @@ class Tracker:
         """Wait for the frame begun on `slot` and copy its tracks into the (pinned host) buffers of `out`."""
         s = out.struct()
         _check(self.lib, self.lib.tpc_track_timeframe_host_end(self._h, C.byref(s), int(slot)), "tpc_track_timeframe_host_end")
+
+    def new_fit(self) -> dict:
+        """Device buffers for tpc_tracker_refit (layouts as in tpc_fit_t)."""
+        mt, dev = self.caps[3], self.device
+        f32 = lambda *s: torch.empty(*s, dtype=torch.float32, device=dev)   # noqa: E731
+        i32 = lambda *s: torch.empty(*s, dtype=torch.int32, device=dev)     # noqa: E731
+        return dict(par=f32(5, mt), cov=f32(15, mt), x_ref=f32(mt), z_ref=f32(mt), chi2=f32(mt), ndf=i32(mt), n_fit=i32(mt))
+
+    def refit_into(self, fit: dict, stream=None):
+        """Enqueues tpc_tracker_refit for the tracks of the last track_timeframe call (does not synchronise)."""
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        f = tpc_fit_t()
+        f.max_tracks = self.caps[3]
+        for k, v in fit.items():
+            setattr(f, k, v.data_ptr())
+        _check(self.lib, self.lib.tpc_tracker_refit(self._h, C.byref(f), C.c_void_p(st.cuda_stream)), "tpc_tracker_refit")
+
+    def refit(self, n_tracks: int, stream=None) -> dict:
+        """Convenience: refit + host copies trimmed to n_tracks."""
+        buf = self.new_fit()
+        self.refit_into(buf, stream)
+        torch.cuda.synchronize(self.device)
+        T = int(n_tracks)
+        out = {k: v.cpu().numpy() for k, v in buf.items()}
+        return dict(par=out["par"][:, :T].T.copy(), cov=out["cov"][:, :T].T.copy(), x_ref=out["x_ref"][:T].copy(),
+                    z_ref=out["z_ref"][:T].copy(), chi2=out["chi2"][:T].copy(), ndf=out["ndf"][:T].copy(),
+                    n_fit=out["n_fit"][:T].copy())
 
     def counters(self) -> dict:
         k = tpc_counters_t()

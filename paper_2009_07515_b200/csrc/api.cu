@@ -96,6 +96,7 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   c.owner = cv.take<unsigned long long>(N);
   c.k_owned = cv.take<int>(K); c.k_first = cv.take<int>(K); c.k_last = cv.take<int>(K);
   c.surv_scan = cv.take<int>(K); c.owned_scan = cv.take<int>(K);
+  c.track_seed = cv.take<int>(K);
   c.mask_words = (R + 31) / 32;
   c.own_mask = cv.take<unsigned>(K * (size_t)c.mask_words);
   for (int k = 0; k < t->host_io; ++k) {
@@ -388,6 +389,18 @@ int tpc_track_timeframe_host_end(tpc_tracker_t* t, const tpc_tracks_t* out, int3
     return TPC_ERR_CUDA;
   sl.busy = false;
   return TPC_OK;
+}
+
+int tpc_tracker_refit(tpc_tracker_t* t, const tpc_fit_t* out, void* cuda_stream) {
+  if (!t || !out || !out->par || !out->cov || !out->x_ref || !out->z_ref || !out->chi2 || !out->ndf || !out->n_fit)
+    return TPC_ERR_INVALID_ARG;
+  if (out->max_tracks < 1 || out->max_tracks > t->max_tracks) return TPC_ERR_CAPACITY;
+  FitPtrs o;
+  o.par = out->par; o.cov = out->cov; o.x_ref = out->x_ref; o.z_ref = out->z_ref; o.chi2 = out->chi2; o.ndf = out->ndf;
+  o.n_fit = out->n_fit; o.max_tracks = (int)out->max_tracks;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  t->last_stream = st;
+  return launch_refit(t->ctx, o, st) ? TPC_ERR_CUDA : TPC_OK;
 }
 
 int tpc_tracker_counters(tpc_tracker_t* t, tpc_counters_t* out) {

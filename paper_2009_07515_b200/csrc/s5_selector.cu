@@ -163,7 +163,7 @@ __global__ void __launch_bounds__(kThreads) k_write(Ctx c, OutPtrs o) {
       off += __popc(m);
     }
     if (lane == 0) {
-      c.kept_scan[id] = sd;                          // seed of track id, for k_params (kept_scan is free until k_kept)
+      c.track_seed[id] = sd;                         // seed of track id, for k_params and the refit
       o.trk_cl_start[id + 1] = end;
     }
   }
@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(kThreads) k_params(Ctx c, OutPtrs o) {
   const int nt = c.cnt->n_tracks, R = c.R;
   const size_t mt = (size_t)o.max_tracks;
   for (int id = blockIdx.x * blockDim.x + threadIdx.x; id < nt; id += gridDim.x * blockDim.x) {
-    const int sd = c.kept_scan[id];
+    const int sd = c.track_seed[id];
     const float* p = c.t_par + (size_t)sd * 5;
     const float* q = c.t_cov + (size_t)sd * 15;
 #pragma unroll

@@ -84,6 +84,7 @@ struct Ctx {
   unsigned long long* owner;          // [n]
   int* k_owned; int* k_first; int* k_last;   // [max_seeds]
   int* surv_scan; int* owned_scan;    // [max_seeds] inclusive scans
+  int* track_seed;                    // [max_seeds] seed of track id (S5 k_write; read by k_params and the refit)
   unsigned* own_mask; int mask_words; // [max_seeds][mask_words] bit k of word w: row first_row + 32 w + k is owned
   Counters* cnt;
   int n_sms;
@@ -102,6 +103,11 @@ struct OutPtrs {
 };
 int launch_s5(const Ctx& c, const OutPtrs& o, cudaStream_t st);
 int launch_reset(const Ctx& c, cudaStream_t st);
+struct FitPtrs {
+  float* par; float* cov; float* x_ref; float* z_ref; float* chi2; int* ndf; int* n_fit;
+  int max_tracks;
+};
+int launch_refit(const Ctx& c, const FitPtrs& o, cudaStream_t st);   // S7, separate call
 
 // In-place inclusive scan of data[0 .. *n_ptr + n_add) (int32), length known only on the device.
 // max_n bounds the grid; tile_sums needs ceil(max_n / kScanTile) + 1 ints.  total_out (nullable)

@@ -36,7 +36,7 @@ def run_gpu(tf, params=None, host=False, caps=None, timing=False):
     return P, trk, out
 
 
-def run_oracle(tf, P, last_stage=5):
+def run_oracle(tf, P, last_stage=6):
     return Oracle(P).run(tf.sector, tf.row, tf.y, tf.z, precision=32, last_stage=last_stage)
 
 

@@ -166,6 +166,7 @@ def test_full_size_sector_sample():
     R = P["n_rows"]
     row_start = trk.stage_view("row_start")
     link_up = trk.stage_view("link_up"); link_dn = trk.stage_view("link_dn"); perm = trk.stage_view("perm")
+    fit = trk.refit(g["n_tracks"])
     for s in (0, 23):
         sub, idx = select_sectors(tf, [s])
         o = run_oracle(sub, P)
@@ -190,6 +191,9 @@ def test_full_size_sector_sample():
         rel = np.abs(par_g - par_o) / np.maximum(np.abs(par_o), [1, 1, .1, .1, .1])
         assert float((rel.max(axis=1) <= PAR_TOL).mean()) >= 0.995, (s, float(rel.max()))
         assert np.array_equal(g["z_beam"][first:first + To], o.get("trk_z_beam").astype(np.float32))
+        assert np.array_equal(fit["n_fit"][first:first + To], o.get("fit_n"))
+        assert np.array_equal(fit["par"][first:first + To], o.get("fit_par").astype(np.float32).reshape(-1, 5))
+        assert np.array_equal(fit["chi2"][first:first + To], o.get("fit_chi2").astype(np.float32))
         print(f"sector {s}: {sub.n} clusters, {To} tracks, assignment identical for {same:.6f}, par max rel {rel.max():.2e}")
 
 
@@ -268,3 +272,24 @@ def test_crowded_slab_falls_back_and_stays_exact():
     assert t["hit_mismatch_seeds"] == 0 and t["par_rel"] <= PAR_TOL and t["cov_rel"] <= COV_TOL, t
     res = compare_tracks(out.numpy(), o, tf.n)
     assert res["cluster_track_equal"] and res["csr_equal"], res
+
+
+@pytest.mark.parametrize("which", ["cfg1", "mini_event", "mini_tf"])
+def test_refit_parity(which, cfg1, mini_event, mini_tf):
+    """tpc_tracker_refit against the oracle's refit: bit-exact, and within the stated bars."""
+    tf = {"cfg1": cfg1, "mini_event": mini_event, "mini_tf": mini_tf}[which]
+    P, trk, out = run_gpu(tf)
+    o = run_oracle(tf, P, last_stage=6)
+    g = out.numpy()
+    T = g["n_tracks"]
+    assert T == o.get("trk_seed").shape[0] > 0
+    fit = trk.refit(T)
+    assert np.array_equal(fit["n_fit"], o.get("fit_n")) and np.array_equal(fit["ndf"], o.get("fit_ndf"))
+    ref = o.get("fit_par").reshape(-1, 5)
+    assert np.max(np.abs(fit["par"] - ref) / np.maximum(np.abs(ref), [1, 1, .1, .1, .1])) <= PAR_TOL
+    for nm, key in (("par", "fit_par"), ("cov", "fit_cov"), ("chi2", "fit_chi2"), ("x_ref", "fit_x_ref"), ("z_ref", "fit_z_ref")):
+        want = o.get(key).astype(np.float32).reshape(fit[nm].shape)
+        assert np.array_equal(fit[nm], want), nm
+    # the refit leaves the tracks of the call untouched and can be repeated
+    again = trk.refit(T)
+    assert all(np.array_equal(fit[k], again[k]) for k in fit)
