@@ -141,7 +141,6 @@ __global__ void __launch_bounds__(kThreads) k_write(Ctx c, OutPtrs o) {
   const int ns = c.cnt->n_seeds, R = c.R;
   const int lane = threadIdx.x & 31;
   const int warps = (gridDim.x * blockDim.x) >> 5;
-  const size_t mt = (size_t)o.max_tracks;
   if (blockIdx.x == 0 && threadIdx.x == 0) o.trk_cl_start[0] = 0;
   for (int sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < ns; sd += warps) {
     const int inc = c.surv_scan[sd], prev = sd ? c.surv_scan[sd - 1] : 0;
