@@ -12,12 +12,30 @@ LIB = os.path.join(HERE, "liboracle.so")
 FLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared", "-Wall", "-Wextra"]
 
 
+def _host_flags() -> list[str]:
+    """std::fma (DESIGN.md section 3.0) compiles to one hardware instruction where the host has FMA3, else glibc's
+    correctly rounded software fmaf/fma is called: the same bits either way, only the oracle's speed differs."""
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.startswith("flags"):
+                    return ["-mfma"] if " fma " in ln + " " else []
+    except OSError:
+        pass
+    return []
+
+
 def build(force: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
+    flags = _host_flags()
+    stamp = LIB + ".flags"                      # the library travels between hosts: rebuild if it was made for another one
+    same_host = os.path.exists(stamp) and open(stamp).read().split() == flags
+    if not force and same_host and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    subprocess.run(["g++", *FLAGS, SRC, "-o", tmp], check=True)
+    subprocess.run(["g++", *FLAGS, *flags, SRC, "-o", tmp], check=True)
     os.replace(tmp, LIB)
+    with open(stamp, "w") as f:
+        f.write(" ".join(flags))
     return LIB
 
 
