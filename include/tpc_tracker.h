@@ -133,7 +133,7 @@ typedef struct {
   int64_t kf_steps;      /* S: Kalman propagate calls */
   int64_t n_hits;        /* H: hits over all kept tracklets */
   int32_t status;
-  int32_t reserved;
+  int32_t s1_global_buckets; /* (sector,row) buckets whose bin sort took the global-memory path (a slab did not fit shared memory) */
 } tpc_counters_t;
 
 /* Debug views into the workspace, valid until the next track call on the handle (DEVICE pointers).

@@ -51,7 +51,7 @@ class tpc_fit_t(C.Structure):
 class tpc_counters_t(C.Structure):
     _fields_ = [("n_clusters", C.c_int64), ("n_bins", C.c_int64), ("n_seeds", C.c_int64), ("n_tracklets", C.c_int64),
                 ("n_tracks", C.c_int64), ("n_track_clusters", C.c_int64), ("n_linked", C.c_int64),
-                ("kf_steps", C.c_int64), ("n_hits", C.c_int64), ("status", C.c_int32), ("reserved", C.c_int32)]
+                ("kf_steps", C.c_int64), ("n_hits", C.c_int64), ("status", C.c_int32), ("s1_global_buckets", C.c_int32)]
 
 
 class tpc_stage_view_t(C.Structure):
@@ -305,7 +305,7 @@ class Tracker:
     def counters(self) -> dict:
         k = tpc_counters_t()
         _check(self.lib, self.lib.tpc_tracker_counters(self._h, C.byref(k)), "tpc_tracker_counters")
-        return {f: getattr(k, f) for f, _ in tpc_counters_t._fields_ if f != "reserved"}
+        return {f: getattr(k, f) for f, _ in tpc_counters_t._fields_}
 
     def enable_stage_timing(self, on: bool = True):
         _check(self.lib, self.lib.tpc_tracker_enable_stage_timing(self._h, int(on)), "tpc_tracker_enable_stage_timing")

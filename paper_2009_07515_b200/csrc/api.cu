@@ -411,7 +411,7 @@ int tpc_tracker_counters(tpc_tracker_t* t, tpc_counters_t* out) {
     return TPC_ERR_CUDA;
   out->n_clusters = t->last_n; out->n_bins = k.n_bins; out->n_seeds = k.n_seeds; out->n_tracklets = k.n_tracklets;
   out->n_tracks = k.n_tracks; out->n_track_clusters = k.n_track_clusters; out->n_linked = k.n_linked;
-  out->kf_steps = (int64_t)k.kf_steps; out->n_hits = (int64_t)k.n_hits; out->status = k.status; out->reserved = 0;
+  out->kf_steps = (int64_t)k.kf_steps; out->n_hits = (int64_t)k.n_hits; out->status = k.status; out->s1_global_buckets = k.s1_global;
   return TPC_OK;
 }
 

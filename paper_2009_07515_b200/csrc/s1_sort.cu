@@ -207,8 +207,8 @@ __global__ void __launch_bounds__(kThreads) k_partition(Ctx c) {
 // Global path (fallback when a slab's bins or clusters do not fit the shared-memory tables): the same steps on
 // the whole bucket with the bins in global memory.
 // Reads of data that atomics or other threads of the CTA wrote go through L2 (__ldcg), never a stale L1 line.
-constexpr int kMaxSlabs = 64;
-constexpr int kSlabTarget = 1024;     // clusters per slab aimed at
+constexpr int kMaxSlabs = 128;
+constexpr int kSlabTarget = 768;  // clusters per slab aimed at (cap / target = 2.7: no bucket of cfg5 falls back; 1024 -> 10 % did)
 constexpr int kSlabBinCap = 8192;     // bins of one slab held in shared memory (48 KB)
 constexpr int kSlabCluCap = 2048;     // clusters of one slab whose input indices fit the shared-memory table (16 KB)
 
@@ -320,7 +320,11 @@ __device__ void bucket_slabs(const Ctx& c, const BucketGeom& g, SlabShared& sh, 
     sh.fits = fits;
   }
   __syncthreads();
-  if (!sh.fits) { bucket_global<kT>(c, g, sh.scan); return; }     // a slab with too many clusters: whole bucket the slow way
+  if (!sh.fits) {
+    if (tid == 0) atomicAdd(&c.cnt->s1_global, 1);
+    bucket_global<kT>(c, g, sh.scan);
+    return;
+  }     // a slab with too many clusters: whole bucket the slow way
 #pragma unroll 4
   for (int i = p0 + tid; i < p1; i += kT) {
     const float4 v = __ldcg(c.rec + i);
@@ -423,7 +427,10 @@ __global__ void __launch_bounds__(kT, kMinCtas) k_binsort(Ctx c) {
     const int slab_rows = (nz + n_slab - 1) / n_slab;
     n_slab = (nz + slab_rows - 1) / slab_rows;
     if ((long long)slab_rows * g.ny <= kSlabBinCap) bucket_slabs<kT>(c, g, sh, n_slab, slab_rows);
-    else bucket_global<kT>(c, g, sh.scan);
+    else {
+      if (tid == 0) atomicAdd(&c.cnt->s1_global, 1);
+      bucket_global<kT>(c, g, sh.scan);
+    }
   }
 }
 

@@ -39,7 +39,8 @@ struct Counters {
   unsigned long long n_hits;
   int s4_ticket;          // dynamic work counter of the S4 persistent kernel
   int s1_ticket;          // dynamic (sector,row) bucket counter of the S1 bin-sort kernel
-  int pad[2];
+  int s1_global;          // buckets bin-sorted on the global-memory path
+  int pad[1];
 };
 
 // Everything a kernel needs, passed by value (a few hundred bytes).
