@@ -266,6 +266,7 @@ def test_crowded_slab_falls_back_and_stays_exact():
     o = run_oracle(tf, P)
     assert trk.counters()["status"] == 0
     assert int(np.diff(trk.stage_view("row_start")).max()) > 2048
+    assert trk.counters()["s1_global_buckets"] > 0             # the fallback path really ran
     bad = compare_integer_stages(trk, o)
     assert not bad, bad
     t = compare_tracklets(trk, o)
