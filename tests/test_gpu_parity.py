@@ -294,3 +294,19 @@ def test_refit_parity(which, cfg1, mini_event, mini_tf):
     # the refit leaves the tracks of the call untouched and can be repeated
     again = trk.refit(T)
     assert all(np.array_equal(fit[k], again[k]) for k in fit)
+
+
+def test_non_uniform_pad_row_pitch():
+    """A 4-region pad-row pitch: up and down row distances differ at the region borders; every
+    stage and the refit must still match the oracle bit for bit."""
+    from tpc_synth import FOUR_REGION_PITCH, Geometry, generate
+    from tpc_synth.generator import CONFIGS
+    rec = dict(CONFIGS["cfg3"]); rec.update(n_collisions=2, seed=9)
+    tf = generate(rec, geometry=Geometry(pitch_regions=FOUR_REGION_PITCH))
+    t, res = _full_parity(tf, exact_assignment=True)
+    assert t["par_bitexact"] and t["cov_bitexact"] and t["chi2_bitexact"], t
+    P, trk, out = run_gpu(tf)
+    o = run_oracle(tf, P, last_stage=6)
+    fit = trk.refit(out.numpy()["n_tracks"])
+    assert np.array_equal(fit["par"], o.get("fit_par").astype(np.float32).reshape(-1, 5))
+    assert np.array_equal(fit["n_fit"], o.get("fit_n"))

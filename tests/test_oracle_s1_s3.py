@@ -203,3 +203,33 @@ def test_s3_invariants_and_chain_walk(name, over):
     keep = lens >= P["min_chain_len"]
     assert np.array_equal(o.get("seed_head"), heads[keep]) and np.array_equal(o.get("seed_len"), lens[keep])
     assert keep.sum() > 0
+
+
+def test_s2_brute_force_and_straight_lines_on_non_uniform_pitch():
+    """Pad rows with a 4-region pitch (0.75 / 1.0 / 1.2 / 1.5 cm): the distances to the row above and below differ at the
+    region borders, so a swapped dx_up / dx_down table or window would show.  Brute force as above; and straight,
+    noise-free tracks (Bz = 0) must still link every interior cluster to its own track with zero deviation."""
+    from tpc_synth import FOUR_REGION_PITCH, Geometry, generate
+    from tpc_synth.generator import CONFIGS
+    g = Geometry(pitch_regions=FOUR_REGION_PITCH)
+    rx = g.row_x()
+    assert not np.allclose(np.diff(rx), np.diff(rx)[0])
+    rec = dict(CONFIGS["cfg2"]); rec.update(n_tracks=300)
+    tf = generate(rec, geometry=g)
+    P = default_params(tf, cell=5.0)
+    o = Oracle(P).run(tf.sector, tf.row, tf.y, tf.z, last_stage=2)
+    idx = np.arange(tf.n) if tf.n <= 7000 else np.sort(np.random.default_rng(1).choice(tf.n, 6000, replace=False))
+    lu, ld = _brute_links(o, P, idx)
+    assert np.array_equal(o.get("link_up_raw")[idx], lu[idx]) and np.array_equal(o.get("link_dn_raw")[idx], ld[idx])
+    assert (lu[idx] >= 0).mean() > 0.5
+    # straight lines through the region borders
+    rec = dict(CONFIGS["cfg1"]); rec.update(sigma=0.0)
+    tf = generate(rec, geometry=Geometry(pitch_regions=FOUR_REGION_PITCH, bz_tesla=0.0))
+    P = default_params(tf)
+    o = Oracle(P).run(tf.sector, tf.row, tf.y, tf.z, last_stage=3)
+    perm = o.get("perm"); up = o.get("link_up"); rows = o.get("s_row")
+    tid = tf.track_id[perm]
+    linked = up >= 0
+    assert np.all(tid[up[linked]] == tid[linked])                     # links never leave the track
+    border = np.isin(rows, [62, 63, 96, 97, 126, 127])
+    assert linked[border].mean() > 0.9                                 # and the region borders are linked through

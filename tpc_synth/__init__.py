@@ -11,6 +11,7 @@ from .generator import (  # noqa: F401
     Geometry,
     TimeFrame,
     CONFIGS,
+    FOUR_REGION_PITCH,
     generate,
     generate_config,
     choose_cell,

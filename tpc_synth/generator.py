@@ -45,8 +45,15 @@ class Geometry:
     bz_tesla: float = 0.5
     v_drift: float = 2.5          # cm / us
     drift_length: float = 250.0   # cm
+    # optional non-uniform pad-row pitch: ((pitch_cm, n_rows), ...) regions from x_first outwards, n_rows summing to
+    # n_rows (a second geometry that makes the up and down row distances differ)
+    pitch_regions: tuple = ()
 
     def row_x(self) -> np.ndarray:
+        if self.pitch_regions:
+            steps = np.concatenate([np.full(int(n), float(p)) for p, n in self.pitch_regions])
+            assert steps.shape[0] == self.n_rows
+            return self.x_first + np.concatenate([[0.0], np.cumsum(steps[1:] * 0.5 + steps[:-1] * 0.5)])
         r = np.arange(self.n_rows, dtype=np.float64)
         return self.x_first + r * (self.x_last - self.x_first) / (self.n_rows - 1)
 
@@ -88,6 +95,10 @@ _STREAM_NOISE = 1
 _STREAM_TRACKS = 2
 _STREAM_SMEAR0 = 1000
 _SMEAR_CHUNK = 8192  # tracks per smear stream; fixed, part of the recipe
+
+
+# the 4-region pitch of SURVEY.md section 8c-2 (0.75 / 1.0 / 1.2 / 1.5 cm x 63 / 34 / 30 / 25 rows)
+FOUR_REGION_PITCH = ((0.75, 63), (1.0, 34), (1.2, 30), (1.5, 25))
 
 
 # ------------------------------------------------------------------- configs
