@@ -310,3 +310,30 @@ def test_non_uniform_pad_row_pitch():
     fit = trk.refit(out.numpy()["n_tracks"])
     assert np.array_equal(fit["par"], o.get("fit_par").astype(np.float32).reshape(-1, 5))
     assert np.array_equal(fit["n_fit"], o.get("fit_n"))
+
+
+@pytest.mark.parametrize("over", [
+    dict(min_chain_len=2, max_gap=0, min_tracklet_hits=3, min_track_hits=2),
+    dict(max_sinphi=np.float32(0.5), pick_chi2_cut=np.float32(4.0)),        # many propagation failures (phase A cut short)
+    dict(min_chain_len=6, max_gap=8, link_T=np.float32(0.2), y_margin=np.float32(0.0)),
+])
+def test_other_cuts_and_rare_paths(over):
+    """Different cuts push the rare branches: chains of two, no gap allowed, propagation failures inside phase A (the
+    chain length is then counted past the failure), tight link cut.  Everything stays bit-exact."""
+    tf = generate_config("cfg2", n_tracks=600, noise=0.2, seed=13)
+    P = default_params(tf)
+    P.update(over)
+    Pg, trk, out = run_gpu(tf, params=P)
+    o = run_oracle(tf, P, last_stage=6)
+    assert trk.counters()["status"] == 0
+    bad = compare_integer_stages(trk, o)
+    assert not bad, bad
+    t = compare_tracklets(trk, o)
+    assert t["hit_mismatch_seeds"] == 0 and t["par_bitexact"] and t["cov_bitexact"] and t["chi2_bitexact"], t
+    res = compare_tracks(out.numpy(), o, tf.n)
+    assert res["cluster_track_equal"] and res["csr_equal"], res
+    T = out.numpy()["n_tracks"]
+    if T:
+        fit = trk.refit(T)
+        assert np.array_equal(fit["n_fit"], o.get("fit_n"))
+        assert np.array_equal(fit["par"], o.get("fit_par").astype(np.float32).reshape(-1, 5))
