@@ -8,7 +8,8 @@
 // Measured and rejected on cfg5 (this version: 6.1 ms): one flat per-lane loop over (query, bin row, candidate) from
 // global memory 14.5 ms and from shared-memory tiles 17.8 ms; a warp-cooperative flattened (slot, candidate) item list
 // 14.1 ms; the five phases (up k=1, up k=2, down k=1, down k=2, scoring) on compacted CTA work lists with the cluster
-// state in shared memory 10.4 ms (twelve CTA barriers per tile cost more than the idle lanes they remove).
+// state in shared memory 10.4 ms (twelve CTA barriers per tile cost more than the idle lanes they remove); the k = 2 up
+// retries (40 % of the clusters, 2 ms of the kernel) deferred to a second, compacted launch 6.5 ms.
 #include "tpc_internal.cuh"
 
 namespace tpc {
