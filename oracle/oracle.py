@@ -57,6 +57,8 @@ def _load():
         lib.orc_kf_fit.restype = C.c_int
         lib.orc_kf_fit.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                    C.c_void_p, C.c_void_p]
+        lib.orc_protect.restype = None
+        lib.orc_protect.argtypes = [C.c_void_p, C.c_float, C.c_float]
         lib.orc_beam_z.restype = C.c_double
         lib.orc_beam_z.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double]
         assert lib.orc_params_size() == C.sizeof(_Params)
@@ -102,6 +104,11 @@ class Oracle:
         if rc != 0:
             raise ValueError(f"oracle rejected the input (rc={rc})")
         return self
+
+    def protect(self, road_y: float, road_z: float) -> np.ndarray:
+        """DESIGN.md section 3.9 on the tracks of the last run: keep flag per INPUT cluster."""
+        self._lib.orc_protect(self._h, float(road_y), float(road_z))
+        return self.get("keep")
 
     def get(self, name: str) -> np.ndarray:
         ptr = C.c_void_p(); n = C.c_int64(); kind = C.c_int()

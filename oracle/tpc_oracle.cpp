@@ -243,6 +243,8 @@ struct Oracle {
   // S7 refit over the owned clusters
   std::vector<double> fit_par, fit_cov, fit_x_ref, fit_z_ref, fit_chi2;
   std::vector<int32_t> fit_ndf, fit_n;
+  // S8 cluster protection, "strategy B"
+  std::vector<int32_t> keep;                                       // [n] by INPUT index: 1 protected, 0 removable
   int s4_prec = 32;
   std::vector<int32_t> trk_cl_start, trk_cl_idx, cluster_track;
   std::vector<double> stage_seconds;                              // [5]
@@ -613,6 +615,21 @@ struct Oracle {
     }
   }
 
+  // ---------------------------------------------------------------------------------------- S8
+  // Cluster protection for hit removal, "strategy B": "runs only the online tracking and removes all hits not in the
+  // vicinity of good tracks".  A cluster is protected iff it is attached to a track or
+  // lies, in its own (sector, row), inside the closed rectangle +-road_y x +-road_z around a cluster some track owns.
+  void stage7_protect(float road_y, float road_z) {
+    keep.assign(n, 0);
+    for (size_t id = 0; id < trk_seed.size(); ++id)
+      for (int32_t q = trk_cl_start[id]; q < trk_cl_start[id + 1]; ++q) {
+        const int o = trk_cl_pos[q];
+        const float y = ys[o], z = zs[o];
+        for_each_in_rect(s_sector[o], s_row[o], y - road_y, y + road_y, z - road_z, z + road_z,
+                         [&](int j) { keep[perm[j]] = 1; });
+      }
+  }
+
   int run(int64_t n_, const uint8_t* sec, const uint8_t* row, const float* y, const float* z, int prec, int last_stage) {
     n = n_; in_sector = sec; in_row = row; in_y = y; in_z = z;
     stage_seconds.assign(5, 0.0);
@@ -726,7 +743,7 @@ int orc_get(void* h, const char* name, const void** ptr, int64_t* n, int* kind) 
   I32(trk_seed); I32(trk_sector); I32(trk_first_row); I32(trk_last_row); I32(trk_n_clusters); I32(trk_ndf);
   F64(trk_par); F64(trk_cov); F64(trk_x_ref); F64(trk_z_ref); F64(trk_chi2); F64(trk_z_beam);
   I32(trk_cl_start); I32(trk_cl_idx); I32(trk_cl_pos); I32(cluster_track); F64(stage_seconds);
-  F64(fit_par); F64(fit_cov); F64(fit_x_ref); F64(fit_z_ref); F64(fit_chi2); I32(fit_ndf); I32(fit_n);
+  I32(keep); F64(fit_par); F64(fit_cov); F64(fit_x_ref); F64(fit_z_ref); F64(fit_chi2); I32(fit_ndf); I32(fit_n);
   F32(up_dx); F32(up_ratio); F32(up_wy); F32(up_wz); F32(dn_dx); F32(dn_ratio); F32(dn_wy); F32(dn_wz);
 #undef I32
 #undef F32
@@ -761,6 +778,9 @@ int orc_kf_fit(const void* params, int prec, int npt, const double* x, const dou
   return prec == 64 ? kf_fit_entry<double>(P, npt, x, y, z, par, cov15, chi2)
                     : kf_fit_entry<float>(P, npt, x, y, z, par, cov15, chi2);
 }
+
+// S8 on the tracks of the last orc_run (last_stage >= 5)
+void orc_protect(void* h, float road_y, float road_z) { reinterpret_cast<Oracle*>(h)->stage7_protect(road_y, road_z); }
 
 // beam-line z of one state, for the pins (prec 32 or 64)
 double orc_beam_z(const void* params, int prec, double x, double y, double z, double tanl, double qpt) {
