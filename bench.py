@@ -301,6 +301,15 @@ def run_ours(args):
     torch.cuda.synchronize(dev)
     refit_ms = ev0.elapsed_time(ev1)
     del fit_buf
+    # ---- cluster protection for hit removal, strategy B (separate call), 1 cm road
+    keep = trk.protect(out, 1.0, 1.0)
+    ev0.record(stream)
+    trk.protect(out, 1.0, 1.0, keep=keep)
+    ev1.record(stream)
+    torch.cuda.synchronize(dev)
+    protect_ms = ev0.elapsed_time(ev1)
+    kept_frac = float(keep[: tf.n].float().mean().item())
+    del keep
 
     # ---- end to end through the host entry points (pinned host buffers in and out).  Time frames arrive one after the
     # other, so the pipelined begin/end pair is the call a user makes: every step still does the H2D
@@ -391,6 +400,8 @@ def run_ours(args):
         "counters": {kk: int(v) for kk, v in k.items()},
         "refit": {"what": "tpc_tracker_refit (separate call, not in the step): all tracks refitted over their owned clusters",
                   "ms": refit_ms},
+        "protect": {"what": "tpc_tracker_protect (separate call, not in the step): strategy-B keep flag per cluster, 1 cm road",
+                    "ms": protect_ms, "kept_fraction": kept_frac},
         "roofline": roofline,
         "cpu_baseline": cpu,
         "gpu_launches": trk.launches_per_call() * args.steps,

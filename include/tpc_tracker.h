@@ -219,6 +219,14 @@ typedef struct {
  * Not part of tpc_track_timeframe (and not of the timed hot path).  CAPACITY if out->max_tracks exceeds the tracker's. */
 TPC_API int tpc_tracker_refit(tpc_tracker_t* t, const tpc_fit_t* out, void* cuda_stream);
 
+/* Cluster protection for hit removal, "strategy B", for the LAST
+ * tpc_track_timeframe call on this handle: keep[i] = 1 iff input cluster i is attached to a track or lies, in its own
+ * (sector, row), within +-road_y (cm) and +-road_z (cm) of a cluster some track owns; else 0.  `cluster_track` is that
+ * call's tpc_tracks_t.cluster_track (DEVICE, [n]); `keep` is DEVICE, [n] bytes.  Enqueued on `cuda_stream`, which must
+ * be ordered after the call; does not synchronise.  INVALID_ARG for null pointers or a negative road. */
+TPC_API int tpc_tracker_protect(tpc_tracker_t* t, const int32_t* cluster_track, float road_y, float road_z, uint8_t* keep,
+                                void* cuda_stream);
+
 /* Pipelined host path (tracker created with host_io = 2 or 3 = number of staging slots; BASELINE.json north_star: whole time frames arrive one
  * after the other).  `begin` enqueues the H2D copy of one frame's HOST (pinned) inputs and its
  * S1..S5 on streams the library owns and returns without waiting; `end` waits for that frame, copies exactly the

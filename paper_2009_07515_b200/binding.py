@@ -68,7 +68,7 @@ STATUS_BITS = {1: "BAD_CLUSTER", 2: "BINS_OVERFLOW", 4: "SEEDS_OVERFLOW", 8: "TR
 
 EXPORTS = [
     "tpc_tracker_workspace_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
-    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit",
+    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit", "tpc_tracker_protect",
     "tpc_tracker_counters", "tpc_tracker_enable_stage_timing", "tpc_tracker_stage_ms", "tpc_tracker_stage_view",
     "tpc_tracker_launches_per_call", "tpc_tracker_destroy", "tpc_error_string",
 ]
@@ -111,6 +111,8 @@ def load_library(build: bool = True) -> C.CDLL:
     lib.tpc_track_timeframe_host_end.argtypes = [C.c_void_p, P(tpc_tracks_t), C.c_int32]
     lib.tpc_tracker_refit.restype = C.c_int
     lib.tpc_tracker_refit.argtypes = [C.c_void_p, P(tpc_fit_t), C.c_void_p]
+    lib.tpc_tracker_protect.restype = C.c_int
+    lib.tpc_tracker_protect.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
     lib.tpc_tracker_counters.restype = C.c_int
     lib.tpc_tracker_counters.argtypes = [C.c_void_p, P(tpc_counters_t)]
     lib.tpc_tracker_enable_stage_timing.restype = C.c_int
@@ -301,6 +303,16 @@ class Tracker:
         return dict(par=out["par"][:, :T].T.copy(), cov=out["cov"][:, :T].T.copy(), x_ref=out["x_ref"][:T].copy(),
                     z_ref=out["z_ref"][:T].copy(), chi2=out["chi2"][:T].copy(), ndf=out["ndf"][:T].copy(),
                     n_fit=out["n_fit"][:T].copy())
+
+    def protect(self, out: Tracks, road_y: float, road_z: float, keep=None, stream=None):
+        """tpc_tracker_protect for the last track_timeframe call (whose outputs are `out`); returns the uint8 device
+        tensor keep[n] (enqueued, not synchronised)."""
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        if keep is None:
+            keep = torch.empty(max(1, out.n_in), dtype=torch.uint8, device=self.device)
+        _check(self.lib, self.lib.tpc_tracker_protect(self._h, out.cluster_track.data_ptr(), float(road_y), float(road_z),
+                                                      keep.data_ptr(), C.c_void_p(st.cuda_stream)), "tpc_tracker_protect")
+        return keep
 
     def counters(self) -> dict:
         k = tpc_counters_t()

@@ -403,6 +403,14 @@ int tpc_tracker_refit(tpc_tracker_t* t, const tpc_fit_t* out, void* cuda_stream)
   return launch_refit(t->ctx, o, st) ? TPC_ERR_CUDA : TPC_OK;
 }
 
+int tpc_tracker_protect(tpc_tracker_t* t, const int32_t* cluster_track, float road_y, float road_z, uint8_t* keep,
+                        void* cuda_stream) {
+  if (!t || !keep || !cluster_track || !(road_y >= 0.f) || !(road_z >= 0.f)) return TPC_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  t->last_stream = st;
+  return launch_protect(t->ctx, cluster_track, road_y, road_z, keep, st) ? TPC_ERR_CUDA : TPC_OK;
+}
+
 int tpc_tracker_counters(tpc_tracker_t* t, tpc_counters_t* out) {
   if (!t || !out) return TPC_ERR_INVALID_ARG;
   Counters k;

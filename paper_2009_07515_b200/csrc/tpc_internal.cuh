@@ -109,6 +109,7 @@ struct FitPtrs {
   int max_tracks;
 };
 int launch_refit(const Ctx& c, const FitPtrs& o, cudaStream_t st);   // S7, separate call
+int launch_protect(const Ctx& c, const int* cluster_track, float road_y, float road_z, unsigned char* keep, cudaStream_t st);   // S8
 
 // In-place inclusive scan of data[0 .. *n_ptr + n_add) (int32), length known only on the device.
 // max_n bounds the grid; tile_sums needs ceil(max_n / kScanTile) + 1 ints.  total_out (nullable)

@@ -167,6 +167,9 @@ def test_full_size_sector_sample():
     row_start = trk.stage_view("row_start")
     link_up = trk.stage_view("link_up"); link_dn = trk.stage_view("link_dn"); perm = trk.stage_view("perm")
     fit = trk.refit(g["n_tracks"])
+    keep = trk.protect(out, 1.0, 1.0)
+    torch.cuda.synchronize()
+    keep = keep.cpu().numpy()
     for s in (0, 23):
         sub, idx = select_sectors(tf, [s])
         o = run_oracle(sub, P)
@@ -194,6 +197,7 @@ def test_full_size_sector_sample():
         assert np.array_equal(fit["n_fit"][first:first + To], o.get("fit_n"))
         assert np.array_equal(fit["par"][first:first + To], o.get("fit_par").astype(np.float32).reshape(-1, 5))
         assert np.array_equal(fit["chi2"][first:first + To], o.get("fit_chi2").astype(np.float32))
+        assert np.array_equal(keep[idx].astype(np.int32), o.protect(1.0, 1.0))
         print(f"sector {s}: {sub.n} clusters, {To} tracks, assignment identical for {same:.6f}, par max rel {rel.max():.2e}")
 
 
@@ -337,3 +341,17 @@ def test_other_cuts_and_rare_paths(over):
         fit = trk.refit(T)
         assert np.array_equal(fit["n_fit"], o.get("fit_n"))
         assert np.array_equal(fit["par"], o.get("fit_par").astype(np.float32).reshape(-1, 5))
+
+
+@pytest.mark.parametrize("which,road", [("cfg1", (2.0, 2.0)), ("mini_event", (1.0, 3.0)), ("mini_tf", (0.5, 0.5)), ("mini_tf", (0.0, 0.0))])
+def test_protect_parity(which, road, cfg1, mini_event, mini_tf):
+    """tpc_tracker_protect (strategy B of PAPER.md:57-61) against the oracle: identical flags."""
+    tf = {"cfg1": cfg1, "mini_event": mini_event, "mini_tf": mini_tf}[which]
+    P, trk, out = run_gpu(tf)
+    o = run_oracle(tf, P, last_stage=5)
+    keep = trk.protect(out, *road)
+    torch.cuda.synchronize()
+    got = keep.cpu().numpy()[: tf.n].astype(np.int32)
+    want = o.protect(*road)
+    assert np.array_equal(got, want)
+    assert np.all(got[out.numpy()["cluster_track"] >= 0] == 1)
