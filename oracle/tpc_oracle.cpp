@@ -243,6 +243,7 @@ struct Oracle {
   // S7 refit over the owned clusters
   std::vector<double> fit_par, fit_cov, fit_x_ref, fit_z_ref, fit_chi2;
   std::vector<int32_t> fit_ndf, fit_n;
+  std::vector<double> fit_res_y, fit_res_z;                        // parallel to trk_cl_idx: residual to the extrapolated track
   // S8 cluster protection, "strategy B"
   std::vector<int32_t> keep;                                       // [n] by INPUT index: 1 protected, 0 removable
   int s4_prec = 32;
@@ -589,6 +590,7 @@ struct Oracle {
     const size_t nt = trk_seed.size();
     fit_par.assign(nt * 5, 0.0); fit_cov.assign(nt * 15, 0.0); fit_x_ref.assign(nt, 0.0); fit_z_ref.assign(nt, 0.0);
     fit_chi2.assign(nt, 0.0); fit_ndf.assign(nt, 0); fit_n.assign(nt, 0);
+    fit_res_y.assign(trk_cl_idx.size(), 0.0); fit_res_z.assign(trk_cl_idx.size(), 0.0);
     const T kbT = T(kb), msp = T(P.max_sinphi), ey2 = T(P.err_y2), ez2 = T(P.err_z2);
     for (size_t id = 0; id < nt; ++id) {
       const int32_t* cl = &trk_cl_pos[trk_cl_start[id]];
@@ -606,6 +608,10 @@ struct Oracle {
       for (int i = m - 2; i >= 0; --i) {
         const int c = cl[i], r = s_row[c];
         if (!kf_propagate<T>(k, kbT, T(P.row_x[r]) - T(P.row_x[cur]), msp, (T*)nullptr)) break;
+        // residual of the cluster to the extrapolated track position: the
+        // innovation of the update that follows
+        fit_res_y[trk_cl_start[id] + i] = (double)(T(ys[c]) - k.p[0]);
+        fit_res_z[trk_cl_start[id] + i] = (double)((T(zs[c]) - zref) - k.p[1]);
         kf_update<T>(k, T(ys[c]), T(zs[c]) - zref, ey2, ez2);
         cur = r; ++nfit;
       }
@@ -743,7 +749,7 @@ int orc_get(void* h, const char* name, const void** ptr, int64_t* n, int* kind) 
   I32(trk_seed); I32(trk_sector); I32(trk_first_row); I32(trk_last_row); I32(trk_n_clusters); I32(trk_ndf);
   F64(trk_par); F64(trk_cov); F64(trk_x_ref); F64(trk_z_ref); F64(trk_chi2); F64(trk_z_beam);
   I32(trk_cl_start); I32(trk_cl_idx); I32(trk_cl_pos); I32(cluster_track); F64(stage_seconds);
-  I32(keep); F64(fit_par); F64(fit_cov); F64(fit_x_ref); F64(fit_z_ref); F64(fit_chi2); I32(fit_ndf); I32(fit_n);
+  I32(keep); F64(fit_res_y); F64(fit_res_z); F64(fit_par); F64(fit_cov); F64(fit_x_ref); F64(fit_z_ref); F64(fit_chi2); I32(fit_ndf); I32(fit_n);
   F32(up_dx); F32(up_ratio); F32(up_wy); F32(up_wz); F32(dn_dx); F32(dn_ratio); F32(dn_wy); F32(dn_wz);
 #undef I32
 #undef F32

@@ -97,3 +97,53 @@ def test_refit_pulls_chi2_and_bookkeeping():
     assert pulls.size > 150
     assert abs(pulls.mean()) < 0.25 and 0.8 < pulls.std() < 1.25, (pulls.mean(), pulls.std())
     assert 0.85 < np.mean(c2) < 1.15, np.mean(c2)
+
+
+def test_residuals_to_the_extrapolated_track():
+    """"Hits attached to tracks are stored as residuals to the extrapolated track position, which have a
+    smaller entropy than absolute hit positions."  The refit reports that residual (the innovation) per owned cluster."""
+    # (i) noise-free: the model predicts the next cluster to a few 10 um (first steps: chord vs tangent direction)
+    tf = generate_config("cfg1", sigma=0.0)
+    P = default_params(tf)
+    o = Oracle(P).run(tf.sector, tf.row, tf.y, tf.z, precision=64, last_stage=6)
+    st = o.get("trk_cl_start"); ry, rz = o.get("fit_res_y"), o.get("fit_res_z")
+    assert ry.shape == o.get("trk_cl_idx").shape
+    for k in range(st.size - 1):
+        if st[k + 1] - st[k] < 40:
+            continue
+        assert ry[st[k + 1] - 1] == 0.0 and rz[st[k + 1] - 1] == 0.0        # the top cluster seeds the fit
+        assert np.abs(ry[st[k]:st[k + 1]]).max() < 1e-2 and np.abs(rz[st[k]:st[k + 1]]).max() < 1e-2
+        assert np.abs(ry[st[k]:st[k + 1] - 10]).max() < 1e-4                  # once the curvature has settled
+    # (ii) the loop recomposed in Python from the single-step entries (pinned above) gives the same residuals and state
+    k = int(np.argmax(np.diff(st)))
+    pos = o.get("trk_cl_pos")[st[k]:st[k + 1]]
+    ys, zs, rows = o.get("ys").astype(np.float64), o.get("zs").astype(np.float64), o.get("s_row")
+    rx = P["row_x"].astype(np.float64)
+    top, nxt = pos[-1], pos[-2]
+    dx, dy, dz = rx[rows[top]] - rx[rows[nxt]], ys[top] - ys[nxt], zs[top] - zs[nxt]
+    dl = math.sqrt(dx * dx + dy * dy)
+    par = np.array([ys[top], 0.0, dy / dl, dz / dl, o.get("trk_par").reshape(-1, 5)[k, 4]])
+    cov = np.zeros(15)
+    for i, v in zip((0, 2, 5, 9, 14), (P["err_y2"], P["err_z2"], P["init_c_ss"], P["init_c_tt"], P["init_c_qq"])):
+        cov[i] = float(v)
+    chi2, cur = 0.0, rows[top]
+    for i in range(pos.size - 2, -1, -1):
+        c = pos[i]
+        ok, par, cov, _ = o.kf_propagate(par, cov, rx[cur], rx[rows[c]])
+        assert ok
+        assert ry[st[k] + i] == ys[c] - par[0] and rz[st[k] + i] == (zs[c] - zs[top]) - par[1]
+        par, cov, chi2 = o.kf_update(par, cov, ys[c], zs[c] - zs[top], chi2)
+        cur = rows[c]
+    assert np.array_equal(par, o.get("fit_par").reshape(-1, 5)[k]) and chi2 == o.get("fit_chi2")[k]
+    # (iii) smeared: residual ~ measurement error + prediction error, centred; far fewer bits than the positions
+    tf = generate_config("cfg3", n_collisions=2)
+    P = default_params(tf)
+    o = Oracle(P).run(tf.sector, tf.row, tf.y, tf.z, last_stage=6)
+    ry, rz, idx = o.get("fit_res_y"), o.get("fit_res_z"), o.get("trk_cl_idx")
+    assert abs(ry.mean()) < 5e-3 and 0.10 < ry.std() < 0.17 and 0.10 < rz.std() < 0.17
+
+    def bits(v, q=0.01):                                     # entropy of the values quantised to 0.1 mm
+        _, cnt = np.unique(np.round(v / q).astype(np.int64), return_counts=True)
+        p = cnt / cnt.sum()
+        return float(-(p * np.log2(p)).sum())
+    assert bits(ry) < bits(tf.y[idx]) - 5 and bits(rz) < bits(tf.z[idx]) - 5
