@@ -211,6 +211,12 @@ typedef struct {
   float* chi2;       /* [max_tracks] */
   int32_t* ndf;      /* [max_tracks] 2*n_fit - 5 */
   int32_t* n_fit;    /* [max_tracks] clusters that entered the fit */
+  /* optional (all three NULL to skip): residual of every owned cluster to the extrapolated track position
+   * (DESIGN.md section 3.7), parallel to tpc_tracks_t.trk_cl_idx of the call; 0 for the top cluster of a
+   * track and for clusters that did not enter the fit */
+  const int32_t* trk_cl_start; /* [n_tracks+1] the call's tpc_tracks_t.trk_cl_start (DEVICE) */
+  float* res_y;      /* [max_track_clusters of the call] cm */
+  float* res_z;      /* [max_track_clusters of the call] cm */
 } tpc_fit_t;
 
 /* Refit of every track of the LAST tpc_track_timeframe call on this handle over the clusters it owns after the

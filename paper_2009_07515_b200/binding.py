@@ -45,7 +45,8 @@ class tpc_tracks_t(C.Structure):
 
 
 class tpc_fit_t(C.Structure):
-    _fields_ = [("max_tracks", C.c_int64)] + [(f, C.c_void_p) for f in ("par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit")]
+    _fields_ = [("max_tracks", C.c_int64)] + [(f, C.c_void_p) for f in ("par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit",
+                                                                       "trk_cl_start", "res_y", "res_z")]
 
 
 class tpc_counters_t(C.Structure):
@@ -277,30 +278,40 @@ class Tracker:
         s = out.struct()
         _check(self.lib, self.lib.tpc_track_timeframe_host_end(self._h, C.byref(s), int(slot)), "tpc_track_timeframe_host_end")
 
-    def new_fit(self) -> dict:
-        """Device buffers for tpc_tracker_refit (layouts as in tpc_fit_t)."""
+    def new_fit(self, residuals: bool = False) -> dict:
+        """Device buffers for tpc_tracker_refit (layouts as in tpc_fit_t); with `residuals` also res_y / res_z."""
         mt, dev = self.caps[3], self.device
         f32 = lambda *s: torch.empty(*s, dtype=torch.float32, device=dev)   # noqa: E731
         i32 = lambda *s: torch.empty(*s, dtype=torch.int32, device=dev)     # noqa: E731
-        return dict(par=f32(5, mt), cov=f32(15, mt), x_ref=f32(mt), z_ref=f32(mt), chi2=f32(mt), ndf=i32(mt), n_fit=i32(mt))
+        d = dict(par=f32(5, mt), cov=f32(15, mt), x_ref=f32(mt), z_ref=f32(mt), chi2=f32(mt), ndf=i32(mt), n_fit=i32(mt))
+        if residuals:
+            d.update(res_y=f32(self.caps[4]), res_z=f32(self.caps[4]))
+        return d
 
-    def refit_into(self, fit: dict, stream=None):
-        """Enqueues tpc_tracker_refit for the tracks of the last track_timeframe call (does not synchronise)."""
+    def refit_into(self, fit: dict, stream=None, out: "Tracks | None" = None):
+        """Enqueues tpc_tracker_refit for the tracks of the last track_timeframe call (does not synchronise).  Residuals
+        (fit has res_y / res_z) need that call's outputs `out` for the CSR offsets."""
         st = stream if stream is not None else torch.cuda.current_stream(self.device)
         f = tpc_fit_t()
         f.max_tracks = self.caps[3]
         for k, v in fit.items():
             setattr(f, k, v.data_ptr())
+        if "res_y" in fit:
+            f.trk_cl_start = out.trk_cl_start.data_ptr()
         _check(self.lib, self.lib.tpc_tracker_refit(self._h, C.byref(f), C.c_void_p(st.cuda_stream)), "tpc_tracker_refit")
 
-    def refit(self, n_tracks: int, stream=None) -> dict:
-        """Convenience: refit + host copies trimmed to n_tracks."""
-        buf = self.new_fit()
-        self.refit_into(buf, stream)
+    def refit(self, n_tracks: int, stream=None, tracks: "Tracks | None" = None) -> dict:
+        """Convenience: refit + host copies trimmed to n_tracks (with `tracks`, the call's outputs, also the residuals)."""
+        buf = self.new_fit(residuals=tracks is not None)
+        self.refit_into(buf, stream, out=tracks)
         torch.cuda.synchronize(self.device)
         T = int(n_tracks)
         out = {k: v.cpu().numpy() for k, v in buf.items()}
-        return dict(par=out["par"][:, :T].T.copy(), cov=out["cov"][:, :T].T.copy(), x_ref=out["x_ref"][:T].copy(),
+        extra = {}
+        if tracks is not None:
+            ntc = int(tracks.trk_cl_start[T].item()) if T else 0
+            extra = dict(res_y=out["res_y"][:ntc].copy(), res_z=out["res_z"][:ntc].copy())
+        return dict(**extra, par=out["par"][:, :T].T.copy(), cov=out["cov"][:, :T].T.copy(), x_ref=out["x_ref"][:T].copy(),
                     z_ref=out["z_ref"][:T].copy(), chi2=out["chi2"][:T].copy(), ndf=out["ndf"][:T].copy(),
                     n_fit=out["n_fit"][:T].copy())
 

@@ -398,6 +398,9 @@ int tpc_tracker_refit(tpc_tracker_t* t, const tpc_fit_t* out, void* cuda_stream)
   FitPtrs o;
   o.par = out->par; o.cov = out->cov; o.x_ref = out->x_ref; o.z_ref = out->z_ref; o.chi2 = out->chi2; o.ndf = out->ndf;
   o.n_fit = out->n_fit; o.max_tracks = (int)out->max_tracks;
+  const int nres = (out->trk_cl_start != nullptr) + (out->res_y != nullptr) + (out->res_z != nullptr);
+  if (nres != 0 && nres != 3) return TPC_ERR_INVALID_ARG;
+  o.trk_cl_start = out->trk_cl_start; o.res_y = out->res_y; o.res_z = out->res_z;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   t->last_stream = st;
   return launch_refit(t->ctx, o, st) ? TPC_ERR_CUDA : TPC_OK;

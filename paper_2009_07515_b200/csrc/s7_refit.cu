@@ -48,6 +48,10 @@ __global__ void __launch_bounds__(kThreads) k_refit(Ctx c, FitPtrs o) {
     const int r_top = rows.next();
     OwnedRows rows2 = rows;                              // positioned after the top cluster
     const int r_nxt = rows.next();
+    // residual slots: the owned clusters of track id sit at trk_cl_start[id] .. in ASCENDING row, the walk is descending
+    const bool want_res = o.res_y != nullptr;
+    int slot = want_res ? o.trk_cl_start[id + 1] - 1 : 0;
+    const int slot0 = want_res ? o.trk_cl_start[id] : 0;
     KF k;
     int cur = r_top, nfit = 0;
     float zref = 0.f;
@@ -65,13 +69,17 @@ __global__ void __launch_bounds__(kThreads) k_refit(Ctx c, FitPtrs o) {
       k.p[0] = pt.x; k.p[1] = 0.0f; k.p[2] = dy / dl; k.p[3] = dz / dl; k.p[4] = c.t_par[(size_t)sd * 5 + 4];
       kf_reset_cov(k, c);
       nfit = 1;
+      if (want_res) { o.res_y[slot] = 0.0f; o.res_z[slot] = 0.0f; --slot; }
       for (int r = rows2.next(); r >= 0; r = rows2.next()) {
         if (!kf_propagate(k, c.kb, tx[r] - tx[cur], c.max_sinphi)) break;
         const float2 v = __ldg(yz + hit[r]);
+        if (want_res) { o.res_y[slot] = v.x - k.p[0]; o.res_z[slot] = (v.y - zref) - k.p[1]; --slot; }
         kf_update(k, v.x, v.y - zref, c.err_y2, c.err_z2);
         cur = r; ++nfit;
       }
     }
+    if (want_res)
+      for (; slot >= slot0; --slot) { o.res_y[slot] = 0.0f; o.res_z[slot] = 0.0f; }   // clusters that did not enter the fit
 #pragma unroll
     for (int i = 0; i < 5; ++i) o.par[i * mt + id] = k.p[i];
 #pragma unroll

@@ -106,6 +106,7 @@ int launch_s5(const Ctx& c, const OutPtrs& o, cudaStream_t st);
 int launch_reset(const Ctx& c, cudaStream_t st);
 struct FitPtrs {
   float* par; float* cov; float* x_ref; float* z_ref; float* chi2; int* ndf; int* n_fit;
+  const int* trk_cl_start; float* res_y; float* res_z;   // optional (null: no residuals)
   int max_tracks;
 };
 int launch_refit(const Ctx& c, const FitPtrs& o, cudaStream_t st);   // S7, separate call

@@ -288,16 +288,20 @@ def test_refit_parity(which, cfg1, mini_event, mini_tf):
     g = out.numpy()
     T = g["n_tracks"]
     assert T == o.get("trk_seed").shape[0] > 0
-    fit = trk.refit(T)
+    fit = trk.refit(T, tracks=out)
     assert np.array_equal(fit["n_fit"], o.get("fit_n")) and np.array_equal(fit["ndf"], o.get("fit_ndf"))
+    # residuals to the extrapolated track, parallel to trk_cl_idx
+    assert fit["res_y"].shape == g["trk_cl_idx"].shape
+    assert np.array_equal(fit["res_y"], o.get("fit_res_y").astype(np.float32))
+    assert np.array_equal(fit["res_z"], o.get("fit_res_z").astype(np.float32))
     ref = o.get("fit_par").reshape(-1, 5)
     assert np.max(np.abs(fit["par"] - ref) / np.maximum(np.abs(ref), [1, 1, .1, .1, .1])) <= PAR_TOL
     for nm, key in (("par", "fit_par"), ("cov", "fit_cov"), ("chi2", "fit_chi2"), ("x_ref", "fit_x_ref"), ("z_ref", "fit_z_ref")):
         want = o.get(key).astype(np.float32).reshape(fit[nm].shape)
         assert np.array_equal(fit[nm], want), nm
     # the refit leaves the tracks of the call untouched and can be repeated
-    again = trk.refit(T)
-    assert all(np.array_equal(fit[k], again[k]) for k in fit)
+    again = trk.refit(T)                                   # without residuals
+    assert all(np.array_equal(fit[k], again[k]) for k in again)
 
 
 def test_non_uniform_pad_row_pitch():
