@@ -272,6 +272,7 @@ int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t
     delete t; return TPC_ERR_CUDA;
   }
   c.n_sms = sms;
+  if (init_s1()) { delete t; return TPC_ERR_CUDA; }
   if (cudaMemcpy(const_cast<RowTab*>(c.rowtab), tab.data(), tab.size() * sizeof(RowTab), cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemset(c.cnt, 0, sizeof(Counters)) != cudaSuccess) {
     delete t; return TPC_ERR_CUDA;

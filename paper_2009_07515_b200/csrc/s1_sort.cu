@@ -450,19 +450,20 @@ int launch_reset(const Ctx& c, cudaStream_t st) {
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 
+// per device, once per tracker (tpc_tracker_create): the bin sort needs more than 48 KB of dynamic shared memory
+int init_s1() {
+  if (cudaFuncSetAttribute(k_binsort<512, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SlabShared)) != cudaSuccess ||
+      cudaFuncSetAttribute(k_binsort<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SlabShared)) != cudaSuccess)
+    return -1;
+  return 0;
+}
+
 int launches_s1() { return 4; }
 int launch_s1(const Ctx& c, cudaStream_t st) {
   const int smem_hist = c.SR <= kHistMaxSR;
   k_zrange_count<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 8), kThreads, smem_hist ? c.SR * sizeof(int) : 0, st>>>(c, smem_hist);
   k_tables<<<1, 1024, 0, st>>>(c);
   k_partition<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 8), kThreads, 0, st>>>(c);
-  static bool attr_set = false;
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(k_binsort<512, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SlabShared)) != cudaSuccess ||
-        cudaFuncSetAttribute(k_binsort<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SlabShared)) != cudaSuccess)
-      return -1;
-    attr_set = true;
-  }
   // big buckets: 512 threads per bucket, four buckets per SM in flight (measured: 1024 x 2 -> 3.4 ms, 512 x 4 -> 3.25,
   // 256 x 6 -> 4.1); small ones: 256 threads, three per SM
   if ((long long)c.n >= 2048LL * c.SR) k_binsort<512, 4><<<grid_for(c.SR, 1, c.n_sms, 4), 512, sizeof(SlabShared), st>>>(c);

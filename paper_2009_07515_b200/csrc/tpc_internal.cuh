@@ -92,6 +92,7 @@ struct Ctx {
 };
 
 // ---- host launchers, one per stage (each only enqueues kernels on `st`)
+int init_s1();                                      // kernel attributes, per device (called at create)
 int launch_s1(const Ctx& c, cudaStream_t st);
 int launch_s2(const Ctx& c, cudaStream_t st);
 int launch_s3(const Ctx& c, cudaStream_t st);
