@@ -68,3 +68,12 @@ def test_workspace_bytes_is_host_only_and_monotone():
     qq, keep2 = tpc.pack_params(Q)
     assert lib.tpc_tracker_workspace_bytes(C.byref(qq), C.c_int64(10), C.c_int64(10), C.c_int64(10), C.c_int64(10),
                                            C.c_int64(10), C.c_int32(0)) == 0
+
+
+def test_header_is_plain_c(tmp_path):
+    """include/tpc_tracker.h compiles as C99 (no C++ or torch types cross the boundary)."""
+    import subprocess
+    src = tmp_path / "t.c"
+    src.write_text('#include "tpc_tracker.h"\nint main(void) { tpc_params_t p; tpc_tracks_t t; tpc_fit_t f; (void)p; (void)t; (void)f; return TPC_OK; }\n')
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-fsyntax-only", "-I", os.path.join(ROOT, "include"), str(src)],
+                   check=True)
