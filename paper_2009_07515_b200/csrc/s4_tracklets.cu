@@ -21,7 +21,9 @@
 // Measured and rejected on cfg5 (this version: 12.8 ms): the searches of a warp laid end to end and tested 32
 // candidates at a time (warp scan, owner lookup, 64-bit shared-memory atomicMin of (d2, position)): 12.9 ms, bit-exact
 // but no faster; the known-cluster loads hoisted above the transport: no change; S5's ownership votes cast by the
-// finishing lane: S4 +4.2 ms for S5 -2.8 ms; 8 CTAs per SM (64 registers, spills): 14.7 ms.
+// finishing lane: S4 +4.2 ms for S5 -2.8 ms; 8 CTAs per SM (64 registers, spills): 14.7 ms; an L2 prefetch of the next
+// row's bin_start entry at the linearly extrapolated position, issued one step ahead: 15.9 ms (20 more instructions
+// in a divergent region cost more than the latency they hide).
 //
 // Arithmetic is written operation by operation in the order of DESIGN.md section 3.4 (compiled with
 // -fmad=false; fused multiply-adds only where the text writes fma(), as __fmaf_rn): the transport J C J^T skips only
