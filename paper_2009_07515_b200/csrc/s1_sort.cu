@@ -200,10 +200,11 @@ __global__ void __launch_bounds__(kThreads) k_partition(Ctx c) {
 // flight the bins + records of all of them (~1 MB each) do not fit L2, and every random access to them was a DRAM
 // sector (19 GB of DRAM traffic for 4 GB of useful bytes, profiles/).  So the CTA first splits its bucket into z-slabs
 // of whole bin rows (a counting sort over <= 64 slab ids, shared-memory counters, records copied rec -> rec2), then
-// bin-sorts one slab at a time ENTIRELY in shared memory: slab histogram (shared atomics), exclusive scan, CSR
+// bin-sorts one slab at a time ENTIRELY in shared memory: the slab's records arrive with one 1-D TMA bulk copy
+// (cp.async.bulk + mbarrier) while the bins are cleared, then slab histogram (shared atomics), exclusive scan, CSR
 // written out once with coalesced stores, stable rank inside multiply-occupied bins from a shared-memory table of
-// input indices.  Global memory sees: rec read twice, rec2 written and read (sequentially, per slab), outputs and
-// bin_start written once.
+// input indices.  Global memory sees: rec read twice, rec2 written and read once, outputs and bin_start written once
+// (7.7 GB of DRAM traffic on cfg5; 10.5 GB when the three sub-steps each re-read rec2, 19 GB before the slab split).
 // Global path (fallback when a slab's bins or clusters do not fit the shared-memory tables): the same steps on
 // the whole bucket with the bins in global memory.
 // Reads of data that atomics or other threads of the CTA wrote go through L2 (__ldcg), never a stale L1 line.
@@ -290,6 +291,8 @@ __device__ void bucket_global(const Ctx& c, const BucketGeom& g, int* s_scan) {
 }
 
 struct SlabShared {
+  float4 recs[kSlabCluCap];           // the records of the slab in flight: one 1-D TMA bulk copy from rec2 (32 KB)
+  unsigned long long mbar;            // mbarrier the bulk copy completes on
   int bins[kSlabBinCap];              // slab histogram, then exclusive offsets inside the slab
   int idx[kSlabCluCap];               // input indices of the clusters of multiply-occupied bins, at offset + arrival rank
   int cnt[kMaxSlabs + 1];             // clusters per slab, then exclusive offsets (cnt[n_slab] = bucket size)
@@ -299,8 +302,30 @@ struct SlabShared {
   int fits;
 };
 
+// ---- 1-D TMA bulk copy global -> shared, completion on an mbarrier (cp.async.bulk; SASS UBLKCP)
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* mbar) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar)) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, unsigned bytes, unsigned long long* mbar) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+               "l"(src_gmem), "r"(bytes), "r"(smem_u32(mbar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* mbar, unsigned parity) {
+  unsigned done;
+  do {
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(done)
+                 : "r"(smem_u32(mbar)), "r"(parity)
+                 : "memory");
+  } while (!done);
+}
+
 template <int kT>
-__device__ void bucket_slabs(const Ctx& c, const BucketGeom& g, SlabShared& sh, int n_slab, int slab_rows) {
+__device__ void bucket_slabs(const Ctx& c, const BucketGeom& g, SlabShared& sh, int n_slab, int slab_rows, unsigned& parity) {
   const int tid = threadIdx.x;
   const int p0 = g.p0, p1 = g.p1, ny = g.ny, nz = g.nzm1 + 1;
   float4* __restrict__ rec2 = c.rec2;
@@ -330,6 +355,7 @@ __device__ void bucket_slabs(const Ctx& c, const BucketGeom& g, SlabShared& sh, 
     const float4 v = __ldcg(c.rec + i);
     rec2[p0 + atomicAdd(&sh.cur[slab_of(v.y)], 1)] = v;
   }
+  asm volatile("fence.proxy.async;" ::: "memory");      // these generic-proxy stores are read back by the TMA engine
   __syncthreads();
 
   // ---- one slab at a time, in shared memory
@@ -337,13 +363,16 @@ __device__ void bucket_slabs(const Ctx& c, const BucketGeom& g, SlabShared& sh, 
     const int q0 = p0 + sh.cnt[k], m = sh.cnt[k + 1] - sh.cnt[k];
     const int rows = min(slab_rows, nz - k * slab_rows);
     const int nbs = rows * ny, bbase = k * slab_rows * ny;
+    // the slab's records come in with one bulk copy while the bins are being cleared
+    if (tid == 0 && m > 0) tma_load_1d(sh.recs, rec2 + q0, (unsigned)m * 16u, &sh.mbar);
     for (int j = tid; j < nbs; j += kT) sh.bins[j] = 0;
     __syncthreads();
-    // histogram: arrival rank inside the bin is the atomic's return value, kept in the record
+    if (m > 0) { mbar_wait(&sh.mbar, parity); parity ^= 1u; }
+    // histogram: arrival rank inside the bin is the atomic's return value, kept in the (shared) record
     for (int i = tid; i < m; i += kT) {
-      const float4 v = __ldcg(rec2 + q0 + i);
+      const float4 v = sh.recs[i];
       const int a = atomicAdd(&sh.bins[local_bin_of(c, g, v.x, v.y) - bbase], 1);
-      reinterpret_cast<int*>(rec2 + q0 + i)[3] = a;
+      reinterpret_cast<int*>(sh.recs + i)[3] = a;
     }
     __syncthreads();
     // exclusive scan in place; the CSR goes out with coalesced stores
@@ -365,7 +394,7 @@ __device__ void bucket_slabs(const Ctx& c, const BucketGeom& g, SlabShared& sh, 
     __syncthreads();
     // alone in its bin -> final place; else park the input index in the shared table
     for (int i = tid; i < m; i += kT) {
-      const float4 v = __ldcg(rec2 + q0 + i);
+      const float4 v = sh.recs[i];
       const int bl = local_bin_of(c, g, v.x, v.y) - bbase;
       const int bs = sh.bins[bl], be = (bl + 1 < nbs) ? sh.bins[bl + 1] : m;
       if (be - bs == 1) {
@@ -379,7 +408,7 @@ __device__ void bucket_slabs(const Ctx& c, const BucketGeom& g, SlabShared& sh, 
     __syncthreads();
     // multiply-occupied bins: stable rank = number of members with a smaller input index
     for (int i = tid; i < m; i += kT) {
-      const float4 v = __ldcg(rec2 + q0 + i);
+      const float4 v = sh.recs[i];
       const int bl = local_bin_of(c, g, v.x, v.y) - bbase;
       const int bs = sh.bins[bl], be = (bl + 1 < nbs) ? sh.bins[bl + 1] : m;
       if (be - bs == 1) continue;
@@ -401,6 +430,8 @@ __global__ void __launch_bounds__(kT, kMinCtas) k_binsort(Ctx c) {
   SlabShared& sh = *reinterpret_cast<SlabShared*>(smem_raw);
   if (c.cnt->status) return;
   const int tid = threadIdx.x;
+  if (tid == 0) mbar_init(&sh.mbar);
+  unsigned parity = 0;                            // phase of sh.mbar the next bulk copy completes (same in every thread)
   for (;;) {
     __syncthreads();                               // everybody is done with the previous bucket's shared state
     if (tid == 0) sh.sr = atomicAdd(&c.cnt->s1_ticket, 1);
@@ -426,7 +457,7 @@ __global__ void __launch_bounds__(kT, kMinCtas) k_binsort(Ctx c) {
     if (n_slab > nz) n_slab = nz;
     const int slab_rows = (nz + n_slab - 1) / n_slab;
     n_slab = (nz + slab_rows - 1) / slab_rows;
-    if ((long long)slab_rows * g.ny <= kSlabBinCap) bucket_slabs<kT>(c, g, sh, n_slab, slab_rows);
+    if ((long long)slab_rows * g.ny <= kSlabBinCap) bucket_slabs<kT>(c, g, sh, n_slab, slab_rows, parity);
     else {
       if (tid == 0) atomicAdd(&c.cnt->s1_global, 1);
       bucket_global<kT>(c, g, sh.scan);
@@ -452,7 +483,7 @@ int launch_reset(const Ctx& c, cudaStream_t st) {
 
 // per device, once per tracker (tpc_tracker_create): the bin sort needs more than 48 KB of dynamic shared memory
 int init_s1() {
-  if (cudaFuncSetAttribute(k_binsort<512, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SlabShared)) != cudaSuccess ||
+  if (cudaFuncSetAttribute(k_binsort<512, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SlabShared)) != cudaSuccess ||
       cudaFuncSetAttribute(k_binsort<256, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SlabShared)) != cudaSuccess)
     return -1;
   return 0;
@@ -464,9 +495,9 @@ int launch_s1(const Ctx& c, cudaStream_t st) {
   k_zrange_count<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 8), kThreads, smem_hist ? c.SR * sizeof(int) : 0, st>>>(c, smem_hist);
   k_tables<<<1, 1024, 0, st>>>(c);
   k_partition<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 8), kThreads, 0, st>>>(c);
-  // big buckets: 512 threads per bucket, four buckets per SM in flight (measured: 1024 x 2 -> 3.4 ms, 512 x 4 -> 3.25,
-  // 256 x 6 -> 4.1); small ones: 256 threads, three per SM
-  if ((long long)c.n >= 2048LL * c.SR) k_binsort<512, 4><<<grid_for(c.SR, 1, c.n_sms, 4), 512, sizeof(SlabShared), st>>>(c);
+  // big buckets: 512 threads per bucket, three buckets per SM in flight (73 KB of shared memory each); small ones: 256
+  // threads, three per SM
+  if ((long long)c.n >= 2048LL * c.SR) k_binsort<512, 3><<<grid_for(c.SR, 1, c.n_sms, 3), 512, sizeof(SlabShared), st>>>(c);
   else k_binsort<256, 3><<<grid_for(c.SR, 1, c.n_sms, 3), 256, sizeof(SlabShared), st>>>(c);
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
