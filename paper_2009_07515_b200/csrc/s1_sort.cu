@@ -453,6 +453,8 @@ __global__ void __launch_bounds__(kT, kMinCtas) k_binsort(Ctx c) {
       continue;
     }
     int n_slab = (m + kSlabTarget - 1) / kSlabTarget;
+    const long long by_bins = ((long long)nz * g.ny + kSlabBinCap - 1) / kSlabBinCap;   // a slab's bins must fit too
+    if (by_bins > n_slab) n_slab = (int)(by_bins < kMaxSlabs ? by_bins : kMaxSlabs);
     if (n_slab > kMaxSlabs) n_slab = kMaxSlabs;
     if (n_slab > nz) n_slab = nz;
     const int slab_rows = (nz + n_slab - 1) / n_slab;
