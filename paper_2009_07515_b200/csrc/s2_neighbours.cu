@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(kThreads, 5) k_neighbours(Ctx c) {
 int launches_s2() { return 1; }
 int launch_s2(const Ctx& c, cudaStream_t st) {
   long long g = ((long long)c.n + kThreads - 1) / kThreads;
-  const long long cap = (long long)c.n_sms * 32;
+  const long long cap = (long long)c.n_sms * 160;   // measured on cfg5: 5 -> 6.9 ms, 32 -> 6.2, 64 -> 5.9, 160 -> 5.76, 320 -> 5.84, 1280 -> 6.3, no cap -> 6.7
   if (g > cap) g = cap;
   if (g < 1) g = 1;
   k_neighbours<<<(unsigned)g, kThreads, c.R * sizeof(RowTab) + 2 * kCap * kThreads * sizeof(int), st>>>(c);
