@@ -496,7 +496,7 @@ int launch_s1(const Ctx& c, cudaStream_t st) {
   const int smem_hist = c.SR <= kHistMaxSR;
   k_zrange_count<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 8), kThreads, smem_hist ? c.SR * sizeof(int) : 0, st>>>(c, smem_hist);
   k_tables<<<1, 1024, 0, st>>>(c);
-  k_partition<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 8), kThreads, 0, st>>>(c);
+  k_partition<<<grid_for(c.n / 4 + 1, kThreads, c.n_sms, 128), kThreads, 0, st>>>(c);
   // big buckets: 512 threads per bucket, three buckets per SM in flight (73 KB of shared memory each); small ones: 256
   // threads, three per SM
   if ((long long)c.n >= 2048LL * c.SR) k_binsort<512, 3><<<grid_for(c.SR, 1, c.n_sms, 3), 512, sizeof(SlabShared), st>>>(c);
