@@ -97,7 +97,7 @@ __global__ void __launch_bounds__(kThreads) k_refit(Ctx c, FitPtrs o) {
 int launches_refit() { return 1; }
 int launch_refit(const Ctx& c, const FitPtrs& o, cudaStream_t st) {
   long long g = ((long long)o.max_tracks + kThreads - 1) / kThreads;
-  const long long cap = (long long)c.n_sms * 16;
+  const long long cap = (long long)c.n_sms * 256;
   if (g > cap) g = cap;
   if (g < 1) g = 1;
   k_refit<<<(unsigned)g, kThreads, c.R * sizeof(float), st>>>(c, o);

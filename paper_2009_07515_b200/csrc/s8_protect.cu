@@ -45,7 +45,7 @@ int launch_protect(const Ctx& c, const int* cluster_track, float road_y, float r
   if (c.n == 0) return 0;
   if (cudaMemsetAsync(mark, 0, (size_t)c.n, st) != cudaSuccess) return -1;
   long long g = ((long long)c.n + kThreads - 1) / kThreads;
-  const long long cap = (long long)c.n_sms * 16;
+  const long long cap = (long long)c.n_sms * 256;
   if (g > cap) g = cap;
   k_mark<<<(unsigned)g, kThreads, 0, st>>>(c, cluster_track, road_y, road_z, mark);
   k_out<<<(unsigned)g, kThreads, 0, st>>>(c, mark, keep);
