@@ -359,3 +359,21 @@ def test_protect_parity(which, road, cfg1, mini_event, mini_tf):
     want = o.protect(*road)
     assert np.array_equal(got, want)
     assert np.all(got[out.numpy()["cluster_track"] >= 0] == 1)
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4"])
+def test_full_size_small_configs(name):
+    """BASELINE.json configs[1..3] at their full sizes (0.8 M, 1.6 M, 3.0 M clusters): every stage, the refit and the
+    protection flags bit-exact against the oracle."""
+    tf = generate_config(name)
+    t, res = _full_parity(tf, exact_assignment=True)
+    assert t["par_bitexact"] and t["cov_bitexact"] and t["chi2_bitexact"], t
+    P, trk, out = run_gpu(tf)
+    o = run_oracle(tf, P, last_stage=6)
+    T = out.numpy()["n_tracks"]
+    fit = trk.refit(T, tracks=out)
+    assert np.array_equal(fit["par"], o.get("fit_par").astype(np.float32).reshape(-1, 5))
+    assert np.array_equal(fit["res_y"], o.get("fit_res_y").astype(np.float32))
+    keep = trk.protect(out, 1.0, 1.0)
+    torch.cuda.synchronize()
+    assert np.array_equal(keep.cpu().numpy()[: tf.n].astype(np.int32), o.protect(1.0, 1.0))
