@@ -59,6 +59,8 @@ def _load():
                                    C.c_void_p, C.c_void_p]
         lib.orc_protect.restype = None
         lib.orc_protect.argtypes = [C.c_void_p, C.c_float, C.c_float]
+        lib.orc_search.restype = C.c_int
+        lib.orc_search.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_int]
         lib.orc_beam_z.restype = C.c_double
         lib.orc_beam_z.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double]
         assert lib.orc_params_size() == C.sizeof(_Params)
@@ -132,6 +134,11 @@ class Oracle:
         self._lib.orc_kf_update(C.byref(self._p), precision, par.ctypes.data, cov.ctypes.data, float(ym), float(zm_rel),
                                 c2.ctypes.data)
         return par, cov, float(c2[0])
+
+    def search(self, par, cov15, zref, sector, row, precision=32) -> int:
+        """DESIGN.md section 3.4.3 on the grid of the last run: sorted position of the nearest gated cluster or -1."""
+        par = np.array(par, dtype=np.float64); cov = np.array(cov15, dtype=np.float64)
+        return int(self._lib.orc_search(self._h, precision, par.ctypes.data, cov.ctypes.data, float(zref), int(sector), int(row)))
 
     def beam_z(self, x, y, z, tanl, qpt, precision=64) -> float:
         """z of the track at the beam line, assuming a primary from the origin."""

@@ -25,10 +25,10 @@
 // generator truth (q/pT 1e-4 rel.) on noise-free helices, pulls on smeared input; S5 vs
 // brute-force ownership; the S4 phase logic (chain, pick-up across holes, gap rule, downward pass) vs
 // generator truth on isolated noise-free helices with rows removed (tests/test_oracle_phases.py);
-// the field constant vs the textbook radius of curvature (tests/golden/helix_radius.txt).
-// "parity unpinned": the S2 pair score and the S4 nearest-candidate choice
-// among several gated clusters are definitions of this reading - only invariants and the
-// end-to-end truth efficiency check them.
+// the field constant vs the textbook radius of curvature (tests/golden/helix_radius.txt); the two CHOICES among
+// several candidates - the S4 search (gate, strict minimum, tie -> lowest position, window, weights) and the S2 pair
+// choice and link cut - on hand-built dyadic constructions whose answers are known by hand, plus a whole-row scan
+// (tests/test_oracle_choice_pins.py; each case lists the mutations it kills).  Nothing is left "parity unpinned".
 // =============================================================================================
 #include <algorithm>
 #include <chrono>
@@ -787,6 +787,18 @@ int orc_kf_fit(const void* params, int prec, int npt, const double* x, const dou
 
 // S8 on the tracks of the last orc_run (last_stage >= 5)
 void orc_protect(void* h, float road_y, float road_z) { reinterpret_cast<Oracle*>(h)->stage7_protect(road_y, road_z); }
+
+// S4 search of one state in row `row` of sector `sector`, on the grid of the last orc_run
+// (last_stage >= 1): sorted position of the nearest gated cluster or -1.  For the pins (tests/test_oracle_search.py).
+int orc_search(void* h, int prec, const double* par, const double* cov15, double zref, int sector, int row) {
+  Oracle& o = *reinterpret_cast<Oracle*>(h);
+  if (prec == 64) {
+    KF<double> k; load_kf(k, par, cov15, 0.0);
+    return o.search<double>(sector, row, k, zref);
+  }
+  KF<float> k; load_kf(k, par, cov15, 0.0);
+  return o.search<float>(sector, row, k, (float)zref);
+}
 
 // beam-line z of one state, for the pins (prec 32 or 64)
 double orc_beam_z(const void* params, int prec, double x, double y, double z, double tanl, double qpt) {
