@@ -13,6 +13,18 @@
  * repository).  All work is enqueued on the caller's CUDA stream; unless stated, calls do not
  * synchronise.  There is no CPU fallback: every stage runs in the library's sm_100a kernels.
  *
+ * Host resources a handle owns (created by tpc_tracker_create, released by tpc_tracker_destroy): the
+ * host struct; 6 CUDA events for the per-stage timing; and, only when created with host_io >= 2,
+ * three non-blocking CUDA streams (upload, compute, download), 4 events per staging slot and one
+ * 48-byte pinned host block the frame counts are copied into.  When built with graph support a handle
+ * also caches one CUDA graph of its launch sequence (tpc_tracker_enable_graph).
+ *
+ * Thread safety: a handle is NOT thread-safe.  Every call on a handle mutates it (the input pointers of
+ * the current frame, the last stream, the slot states), so all calls on one handle must come from one
+ * thread at a time; different handles (each with its own workspace) are independent and may be used
+ * from different threads or streams concurrently.  tpc_error_string and tpc_tracker_workspace_bytes
+ * touch no handle and are thread-safe.
+ *
  * Error behaviour: functions return 0 (TPC_OK) or a negative tpc_error code; device-detected
  * conditions (bad sector/row value, capacity overflow) are reported through the 32-bit status word
  * (tpc_tracks_t.status, tpc_counters_t.status) as a bit set of TPC_STATUS_*; when a status bit is
@@ -42,7 +54,7 @@ enum tpc_error {
 };
 
 enum tpc_status_bits {
-  TPC_STATUS_BAD_CLUSTER = 1,      /* a cluster had sector >= n_sectors or row >= n_rows */
+  TPC_STATUS_BAD_CLUSTER = 1,      /* a cluster had sector >= n_sectors, row >= n_rows, or a non-finite y or z */
   TPC_STATUS_BINS_OVERFLOW = 2,    /* the (y,z) grids need more than max_bins bins (or > INT32_MAX) */
   TPC_STATUS_SEEDS_OVERFLOW = 4,   /* more than max_seeds chain heads qualified as seeds */
   TPC_STATUS_TRACKS_OVERFLOW = 8,  /* more than max_tracks tracks or max_track_clusters attached clusters */
@@ -182,17 +194,26 @@ TPC_API size_t tpc_tracker_workspace_bytes(const tpc_params_t* params, int64_t m
                                    int64_t max_seeds, int64_t max_tracks, int64_t max_track_clusters,
                                    int32_t host_io);
 
-/* Creates a tracker on the current CUDA device.  `d_workspace` (DEVICE, 256-byte aligned, at least
- * workspace_bytes long) stays owned by the caller and must outlive the handle.  Uploads the derived
- * tables (synchronous).  `host_io` as above. */
+/* Creates a tracker on the current CUDA device for the method of DESIGN.md section 3 ("Track Finding",
+ * PAPER.md:137 Table 1; the whole time frame is processed at once in GPU memory that is reused across
+ * consecutive steps, PAPER.md:117-119 - hence ONE caller-owned arena carved once).  `d_workspace`
+ * (DEVICE, 256-byte aligned, at least workspace_bytes long) stays owned by the caller and must outlive
+ * the handle.  Derives the per-row tables on the host and uploads them
+ * (synchronous).  `host_io` as above.  Errors: INVALID_ARG (null / out-of-range parameters, unaligned
+ * workspace), CAPACITY (workspace_bytes too small), CUDA.  On failure *out = NULL and nothing is leaked.
+ * Differs from SURVEY.md section 8(b)'s sketch by two more capacities (max_tracks, max_track_clusters: the
+ * staging buffers of the host path are sized by them) and by host_io. */
 TPC_API int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t max_bins, int64_t max_seeds,
                        int64_t max_tracks, int64_t max_track_clusters, int32_t host_io, void* d_workspace,
                        size_t workspace_bytes, tpc_tracker_t** out);
 
-/* Enqueues stages S1..S5 for one time frame on `cuda_stream` (a cudaStream_t; NULL = default
- * stream).  DEVICE pointers in `in` and `out`.  Does not synchronise; counts and status stay on
- * the device (out->n_tracks, out->status).  out->max_tracks / max_track_clusters must not exceed
- * the capacities given at create. */
+/* The hot path: enqueues stages S1..S5 (DESIGN.md sections 3.1-3.5; BASELINE.json north_star (1)-(5);
+ * "the TPC tracking runs first standalone without such corrections") for one time frame on
+ * `cuda_stream` (a cudaStream_t; NULL = default stream).  DEVICE pointers in `in` and `out`.  Does not
+ * synchronise; counts and status stay on the device (out->n_tracks, out->status).
+ * out->max_tracks / max_track_clusters must not exceed the capacities given at create (CAPACITY);
+ * null or misaligned pointers, n < 0: INVALID_ARG; a failed launch: CUDA.  Device-detected conditions
+ * arrive in out->status (see tpc_status_bits), never as a silently truncated result. */
 TPC_API int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tracks_t* out, void* cuda_stream);
 
 /* Same from/to HOST buffers (tracker created with host_io != 0): copies the SoA input to the device,
@@ -252,12 +273,18 @@ TPC_API int tpc_tracker_counters(tpc_tracker_t* t, tpc_counters_t* out);
 TPC_API int tpc_tracker_enable_stage_timing(tpc_tracker_t* t, int32_t enable);
 TPC_API int tpc_tracker_stage_ms(tpc_tracker_t* t, float* out_ms5);
 
-/* Debug view of one workspace array (enum tpc_stage_array).  Synchronises. */
+/* Debug view of one workspace array (enum tpc_stage_array): the intermediate result of one stage of
+ * DESIGN.md sections 3.1-3.5, for the stage-by-stage parity tests.  The pointer is a
+ * DEVICE pointer into the caller's workspace, valid until the next track call on the handle.
+ * Synchronises the stream of the last call (it reads the device counters for the lengths). */
 TPC_API int tpc_tracker_stage_view(tpc_tracker_t* t, int32_t which, tpc_stage_view_t* out);
 
 /* Number of kernel launches tpc_track_timeframe enqueues per call (for bench.py's gpu_launches). */
 TPC_API int tpc_tracker_launches_per_call(const tpc_tracker_t* t);
 
+/* Releases the host resources listed at the top (synchronises the library-owned streams first).  The
+ * workspace is the caller's and is not touched; frames still in flight on a caller's stream must have
+ * finished (memory belongs to the framework around the tracker, not to the tracker). */
 TPC_API int tpc_tracker_destroy(tpc_tracker_t* t);
 
 TPC_API const char* tpc_error_string(int code);

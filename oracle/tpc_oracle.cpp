@@ -293,12 +293,17 @@ struct Oracle {
     zmin.assign(P.n_sectors, INFINITY); zmax.assign(P.n_sectors, -INFINITY); nz.assign(P.n_sectors, 0);
     for (int64_t i = 0; i < n; ++i) {
       if (in_sector[i] >= P.n_sectors || in_row[i] >= P.n_rows) return -1;
+      if (!std::isfinite(in_y[i]) || !std::isfinite(in_z[i])) return -1;      // precondition: finite coordinates
       const int s = in_sector[i];
       zmin[s] = std::min(zmin[s], in_z[i]);
       zmax[s] = std::max(zmax[s], in_z[i]);
     }
-    for (int s = 0; s < P.n_sectors; ++s)
-      nz[s] = (zmin[s] <= zmax[s]) ? (int)std::floor((zmax[s] - zmin[s]) * inv_cz) + 1 : 0;
+    for (int s = 0; s < P.n_sectors; ++s) {
+      if (!(zmin[s] <= zmax[s])) continue;
+      const float rows = std::floor((zmax[s] - zmin[s]) * inv_cz);
+      if (!(rows < 2147483646.0f)) return -2;                                   // more bin rows than an int32 holds: N_b > INT32_MAX
+      nz[s] = (int)rows + 1;
+    }
     bin_base.assign(n_sr + 1, 0);
     int64_t acc = 0;
     for (int s = 0; s < P.n_sectors; ++s)

@@ -203,7 +203,7 @@ class Tracker:
     """tpc_tracker_create / tpc_track_timeframe / tpc_tracker_destroy with torch-owned memory."""
 
     def __init__(self, params: dict, max_clusters: int, max_bins: int, max_seeds: int, max_tracks: int,
-                 max_track_clusters: int, host_io: int = 0, device="cuda:0"):
+                 max_track_clusters: int, host_io: int = 0, device="cuda:0", guard_bytes: int = 0):
         if not torch.cuda.is_available():
             raise RuntimeError("tpc tracker needs a CUDA device: there is no CPU fallback")
         self.lib = load_library()
@@ -217,11 +217,21 @@ class Tracker:
             raise ValueError("tpc_tracker_workspace_bytes rejected the parameters / capacities")
         self.workspace_bytes = int(nbytes)
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            # guard_bytes > 0 (tests): canary bytes on both sides of the arena, see guards_intact()
+            g = (int(guard_bytes) + 255) // 256 * 256
+            self._arena = torch.full((nbytes + 2 * g,), 0xA5, dtype=torch.uint8, device=self.device)
+            self._guard = g
+            self.workspace = self._arena[g: g + nbytes]
             h = C.c_void_p()
             _check(self.lib, self.lib.tpc_tracker_create(C.byref(self._p), *caps, int(host_io), self.workspace.data_ptr(),
                                                          nbytes, C.byref(h)), "tpc_tracker_create")
         self._h = h
+
+    def guards_intact(self) -> bool:
+        """True iff no kernel wrote outside the workspace arena (only meaningful with guard_bytes > 0)."""
+        torch.cuda.synchronize(self.device)
+        g = self._guard
+        return bool((self._arena[:g] == 0xA5).all().item() and (self._arena[self._arena.numel() - g:] == 0xA5).all().item())
 
     # -- lifetime
     def destroy(self):

@@ -260,7 +260,7 @@ int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t
   t->max_tracks = max_tracks; t->max_track_clusters = max_track_clusters; t->host_io = host_io;
   size_t total = 0;
   layout(t, static_cast<char*>(d_workspace), &total);
-  if (total > workspace_bytes) { delete t; return TPC_ERR_CAPACITY; }
+  if (total > workspace_bytes) { delete t; return TPC_ERR_CAPACITY; }   // nothing but the host struct exists yet
   std::vector<RowTab> tab;
   fill_ctx_constants(t, tab);
   t->params.row_x = nullptr;
@@ -277,8 +277,9 @@ int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t
       cudaMemset(c.cnt, 0, sizeof(Counters)) != cudaSuccess) {
     delete t; return TPC_ERR_CUDA;
   }
+  // from here on a failure goes through tpc_tracker_destroy, which releases whatever was created so far
   for (auto& e : t->ev)
-    if (cudaEventCreate(&e) != cudaSuccess) { delete t; return TPC_ERR_CUDA; }
+    if (cudaEventCreate(&e) != cudaSuccess) { tpc_tracker_destroy(t); return TPC_ERR_CUDA; }
   if (host_io >= 2) {
     bool ok = cudaStreamCreateWithFlags(&t->s_in, cudaStreamNonBlocking) == cudaSuccess &&
               cudaStreamCreateWithFlags(&t->s_compute, cudaStreamNonBlocking) == cudaSuccess &&
@@ -351,28 +352,34 @@ int tpc_track_timeframe_host_begin(tpc_tracker_t* t, const tpc_clusters_t* in, i
   if (sl.busy) return TPC_ERR_INVALID_ARG;          // begin / end must alternate per slot
   const size_t n = (size_t)in->n;
   sl.n = in->n;
+  // A failure after something was enqueued must not leave copies or kernels in flight on a slot the caller believes
+  // free (a retry would overwrite staging that is still being read): drain the library's streams before returning.
+  auto fail = [&](int code) {
+    cudaStreamSynchronize(t->s_in); cudaStreamSynchronize(t->s_compute);
+    return code;
+  };
   if (cudaStreamWaitEvent(t->s_in, sl.in_free, 0) != cudaSuccess) return TPC_ERR_CUDA;
   if (n) {
     if (cudaMemcpyAsync(sl.sector, in->sector, n, cudaMemcpyHostToDevice, t->s_in) != cudaSuccess ||
         cudaMemcpyAsync(sl.row, in->row, n, cudaMemcpyHostToDevice, t->s_in) != cudaSuccess ||
         cudaMemcpyAsync(sl.y, in->y, n * 4, cudaMemcpyHostToDevice, t->s_in) != cudaSuccess ||
         cudaMemcpyAsync(sl.z, in->z, n * 4, cudaMemcpyHostToDevice, t->s_in) != cudaSuccess)
-      return TPC_ERR_CUDA;
+      return fail(TPC_ERR_CUDA);
   }
   if (cudaEventRecord(sl.h2d_done, t->s_in) != cudaSuccess ||
       cudaStreamWaitEvent(t->s_compute, sl.h2d_done, 0) != cudaSuccess ||
       cudaStreamWaitEvent(t->s_compute, sl.out_free, 0) != cudaSuccess)
-    return TPC_ERR_CUDA;
+    return fail(TPC_ERR_CUDA);
   tpc_clusters_t d = *in;
   d.sector = sl.sector; d.row = sl.row; d.y = sl.y; d.z = sl.z; d.x = nullptr;
   const int rc = run_device(t, &d, sl.out, t->s_compute, sl.in_free);
-  if (rc != TPC_OK) return rc;
+  if (rc != TPC_OK) return fail(rc);
   int* hc = t->h_counts + 4 * slot;
   if (cudaMemcpyAsync(hc + 0, sl.out.n_tracks, 4, cudaMemcpyDeviceToHost, t->s_compute) != cudaSuccess ||
       cudaMemcpyAsync(hc + 1, sl.out.status, 4, cudaMemcpyDeviceToHost, t->s_compute) != cudaSuccess ||
       cudaMemcpyAsync(hc + 2, &t->ctx.cnt->n_track_clusters, 4, cudaMemcpyDeviceToHost, t->s_compute) != cudaSuccess ||
       cudaEventRecord(sl.done, t->s_compute) != cudaSuccess)
-    return TPC_ERR_CUDA;
+    return fail(TPC_ERR_CUDA);
   sl.busy = true;
   return TPC_OK;
 }

@@ -21,7 +21,8 @@ namespace tpc {
 namespace {
 
 constexpr int kThreads = 256;
-constexpr int kHistMaxSR = 12288;   // (sector,row) histogram kept in shared memory up to this many buckets (48 KB)
+constexpr int kHistMaxSR = 11776;   // (sector,row) histogram kept in shared memory up to this many buckets: 46 KB dynamic + the 2 KB
+                                    // of static smin/smax stay inside the 48 KB a kernel gets without opting in
 
 __global__ void __launch_bounds__(256) k_reset(Ctx c) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -44,7 +45,8 @@ __global__ void __launch_bounds__(kThreads) k_zrange_count(Ctx c, int use_smem_h
   bool bad = false;
   const long long n = c.n;
   auto one = [&](int s, int r, float z) {
-    if (s >= c.S || r >= c.R) { bad = true; return; }
+    // a non-finite z has no bin (and an infinite one would make the z range, hence the bin count, meaningless)
+    if (s >= c.S || r >= c.R || !(fabsf(z) < INFINITY)) { bad = true; return; }
     const int key = float_key(z);
     if (key < smin[s]) atomicMin(&smin[s], key);
     if (key > smax[s]) atomicMax(&smax[s], key);
@@ -117,13 +119,18 @@ __global__ void __launch_bounds__(1024) k_tables(Ctx c) {
   __shared__ int sscan[33];
   if (threadIdx.x == 0) {
     long long acc = 0;
+    bool too_many = false;
     for (int s = 0; s < c.S; ++s) {
       const int kmin = c.zmin_key[s], kmax = c.zmax_key[s];
       int nz = 0;
       float zmin = 0.f, zmax = 0.f;
       if (kmin <= kmax) {
         zmin = key_float(kmin); zmax = key_float(kmax);
-        nz = (int)floorf((zmax - zmin) * c.inv_cz) + 1;
+        // the row count stays a float until it is known to fit: a huge |z| (1e30) would saturate the conversion and the
+        // "+ 1" would wrap; such a grid is a BINS_OVERFLOW like any other grid that is too large
+        const float rows = floorf((zmax - zmin) * c.inv_cz);
+        if (!(rows < 2147483646.0f)) { too_many = true; nz = 0; }
+        else nz = (int)rows + 1;
       }
       c.zmin[s] = zmin; c.zmax[s] = zmax; c.nz[s] = nz; snz[s] = nz;
       sbase[s] = acc;
@@ -131,6 +138,7 @@ __global__ void __launch_bounds__(1024) k_tables(Ctx c) {
     }
     sbase[c.S] = acc;
     int st = 0;
+    if (too_many) sbase[c.S] = acc = 2147483647LL;             // every thread sees "not ok" below
     if (acc > 2147483647LL - 2 || acc > (long long)c.max_bins) { st = TPC_STATUS_BINS_OVERFLOW; acc = 0; }
     if (st) atomicOr(&c.cnt->status, st);
     c.cnt->n_bins = (int)acc;
@@ -169,7 +177,9 @@ __global__ void __launch_bounds__(1024) k_tables(Ctx c) {
 __global__ void __launch_bounds__(kThreads) k_partition(Ctx c) {
   if (c.cnt->status) return;
   const long long n = c.n;
+  bool bad = false;
   auto one = [&](int s, int r, float y, float z, long long i) {
+    if (!(fabsf(y) < INFINITY)) bad = true;             // precondition: finite coordinates (z was checked by k_zrange_count)
     const int pos = atomicAdd(c.sr_cursor + s * c.R + r, 1);
     c.rec[pos] = make_float4(y, z, __int_as_float((int)i), 0.0f);
   };
@@ -191,6 +201,7 @@ __global__ void __launch_bounds__(kThreads) k_partition(Ctx c) {
     const long long i = (n4 << 2) + threadIdx.x;
     one(c.in_sector[i], c.in_row[i], c.in_y[i], c.in_z[i], i);
   }
+  if (bad) atomicOr(&c.cnt->status, (int)TPC_STATUS_BAD_CLUSTER);
 }
 
 // ---------------------------------------------------------------------------------- bin sort inside a (sector,row) bucket

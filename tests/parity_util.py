@@ -12,7 +12,7 @@ INT_STAGES = ["perm", "bin_start", "row_start", "bin_base", "nz", "link_up_raw",
               "seed_head", "seed_len"]
 
 
-def run_gpu(tf, params=None, host=False, caps=None, timing=False):
+def run_gpu(tf, params=None, host=False, caps=None, timing=False, guard_bytes=0):
     import paper_2009_07515_b200 as tpc
     P = params or default_params(tf)
     c = tpc.suggest_capacities(tf.n, P)
@@ -20,7 +20,7 @@ def run_gpu(tf, params=None, host=False, caps=None, timing=False):
     if caps:
         c.update(caps)
     trk = tpc.Tracker(P, c["max_clusters"], c["max_bins"], c["max_seeds"], c["max_tracks"], c["max_track_clusters"],
-                      host_io=host)
+                      host_io=host, guard_bytes=guard_bytes)
     if timing:
         trk.enable_stage_timing(True)
     th = lambda a: torch.from_numpy(np.ascontiguousarray(a))  # noqa: E731
@@ -132,3 +132,133 @@ def compare_tracks(out_np: dict, o, n_in: int):
                 matched += 1
     res["matched_frac"] = matched / To if To else 1.0
     return res
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# Whole-frame parity, sector by sector.  Sectors are independent (section 3.1: one z range per sector;
+# S2..S5 never leave a sector), so the oracle run on the clusters of ONE sector must reproduce, array by array and bit for
+# bit, the slice of the CUDA result that belongs to that sector.  The sectors are checked in a fork()ed process pool:
+# the children inherit the host copies of the CUDA arrays (module global _FRAME), run the plain oracle and compare; they
+# never touch CUDA.
+_FRAME = None
+
+
+def collect_gpu_frame(tf, P, trk, out, road=(1.0, 1.0)):
+    """Host copies of every stage array, the outputs, the refit (with residuals) and the keep flags of one CUDA run."""
+    g = out.numpy()
+    fit = trk.refit(g["n_tracks"], tracks=out)
+    keep = trk.protect(out, *road)
+    torch.cuda.synchronize()
+    views = {nm: trk.stage_view(nm) for nm in (
+        "perm", "yz", "srow", "bin_start", "row_start", "bin_base", "zmin", "zmax", "nz", "link_up_raw", "link_dn_raw",
+        "link_up", "link_dn", "seed_head", "seed_len", "t_hit", "t_first_row", "t_last_row", "t_n_hits", "t_par", "t_cov",
+        "t_chi2", "t_zref", "tracklet_of_seed", "k_owned")}
+    return dict(tf=tf, P=P, out=g, fit=fit, keep=keep.cpu().numpy()[: tf.n].astype(np.int32), road=road, **views)
+
+
+def _eq(bad, name, a, b):
+    a = np.asarray(a); b = np.asarray(b)
+    if a.shape != b.shape:
+        bad.append(f"{name}: shape {a.shape} vs {b.shape}")
+    elif not np.array_equal(a, b):
+        bad.append(f"{name}: {int((a != b).sum())} of {a.size} differ")
+
+
+def check_sector(s: int):
+    """Oracle on sector `s` of _FRAME['tf'] against the CUDA arrays restricted to that sector: list of mismatches."""
+    from tpc_synth import select_sectors
+    F = _FRAME
+    tf, P, g, fit = F["tf"], F["P"], F["out"], F["fit"]
+    R = P["n_rows"]
+    sub, idx = select_sectors(tf, [s])
+    o = Oracle(P).run(sub.sector, sub.row, sub.y, sub.z, precision=32, last_stage=6)
+    bad = []
+    f32 = np.float32
+    a, b = int(F["row_start"][s * R]), int(F["row_start"][(s + 1) * R])
+    if b - a != sub.n:
+        return s, [f"row_start: sector holds {b - a} positions, {sub.n} clusters"], {}
+    off = lambda v: np.where(v >= 0, v.astype(np.int64) + a, -1)   # noqa: E731  oracle positions -> frame positions
+    # ---- S1
+    _eq(bad, "perm", F["perm"][a:b], idx[o.get("perm")])
+    yz = F["yz"].reshape(-1, 2)[a:b]
+    _eq(bad, "ys", yz[:, 0], o.get("ys")); _eq(bad, "zs", yz[:, 1], o.get("zs"))
+    _eq(bad, "srow", F["srow"][a:b].astype(np.int64), o.get("s_sector").astype(np.int64) * 256 + o.get("s_row"))
+    bb0, bb1 = int(F["bin_base"][s * R]), int(F["bin_base"][(s + 1) * R])
+    _eq(bad, "bin_base", F["bin_base"][s * R:(s + 1) * R + 1].astype(np.int64) - bb0, o.get("bin_base")[s * R:(s + 1) * R + 1])
+    _eq(bad, "bin_start", F["bin_start"][bb0:bb1 + 1].astype(np.int64) - a, o.get("bin_start"))
+    _eq(bad, "row_start", F["row_start"][s * R:(s + 1) * R + 1].astype(np.int64) - a, o.get("row_start")[s * R:(s + 1) * R + 1])
+    _eq(bad, "nz", F["nz"][s], o.get("nz")[s]); _eq(bad, "zmin", F["zmin"][s], o.get("zmin")[s]); _eq(bad, "zmax", F["zmax"][s], o.get("zmax")[s])
+    # ---- S2 / S3
+    for nm in ("link_up_raw", "link_dn_raw", "link_up", "link_dn"):
+        _eq(bad, nm, F[nm][a:b], off(o.get(nm)))
+    k0, k1 = int(np.searchsorted(F["seed_head"], a)), int(np.searchsorted(F["seed_head"], b))
+    _eq(bad, "seed_head", F["seed_head"][k0:k1], off(o.get("seed_head")))
+    _eq(bad, "seed_len", F["seed_len"][k0:k1], o.get("seed_len"))
+    K = k1 - k0
+    # ---- S4 (the CUDA hit table is defined on [t_first_row, t_last_row] only; the oracle's holds -1 outside)
+    if K == o.get("seed_head").shape[0]:
+        hit = F["t_hit"].reshape(-1, R)[k0:k1].copy()
+        rows = np.arange(R)[None, :]
+        hit[(rows < F["t_first_row"][k0:k1, None]) | (rows > F["t_last_row"][k0:k1, None])] = -1
+        _eq(bad, "t_hit", hit, off(o.get("t_hit").reshape(-1, R)))
+        for nm in ("t_first_row", "t_last_row", "t_n_hits"):
+            _eq(bad, nm, F[nm][k0:k1], o.get(nm))
+        _eq(bad, "t_par", F["t_par"].reshape(-1, 5)[k0:k1], o.get("t_par").astype(f32).reshape(-1, 5))
+        _eq(bad, "t_cov", F["t_cov"].reshape(-1, 15)[k0:k1], o.get("t_cov").astype(f32).reshape(-1, 15))
+        _eq(bad, "t_chi2", F["t_chi2"][k0:k1], o.get("t_chi2").astype(f32))
+        _eq(bad, "t_zref", F["t_zref"][k0:k1], o.get("t_z_ref").astype(f32))
+        tos_g = F["tracklet_of_seed"][k0:k1].astype(np.int64); tos_o = o.get("tracklet_of_seed")
+        first_kept = tos_g[tos_g >= 0].min() if (tos_g >= 0).any() else 0
+        _eq(bad, "tracklet_of_seed", np.where(tos_g >= 0, tos_g - first_kept, -1), tos_o)
+        _eq(bad, "k_owned", F["k_owned"][k0:k1], o.get("k_owned"))
+    # ---- S5: tracks of a sector have consecutive ids (seed order is sector-major)
+    mine = np.nonzero(g["sector"] == s)[0]
+    t0, t1 = (int(mine[0]), int(mine[-1]) + 1) if mine.size else (0, 0)
+    To = int(o.get("trk_seed").shape[0])
+    if t1 - t0 != To or (mine.size and not np.array_equal(mine, np.arange(t0, t1))):
+        bad.append(f"tracks: {t1 - t0} vs oracle {To}")
+    else:
+        ct = g["cluster_track"][idx].astype(np.int64)
+        _eq(bad, "cluster_track", np.where(ct >= 0, ct - t0, -1), o.get("cluster_track"))
+        st = g["trk_cl_start"][t0:t1 + 1].astype(np.int64)
+        c0, c1 = (int(st[0]), int(st[-1])) if To else (0, 0)
+        _eq(bad, "trk_cl_start", st - c0 if To else np.zeros(1, np.int64), o.get("trk_cl_start"))
+        _eq(bad, "trk_cl_idx", g["trk_cl_idx"][c0:c1], idx[o.get("trk_cl_idx")] if To else np.empty(0, np.int64))
+        for nm in ("first_row", "last_row", "n_clusters", "ndf"):
+            _eq(bad, nm, g[nm][t0:t1], o.get("trk_" + nm))
+        _eq(bad, "par", g["par"][t0:t1], o.get("trk_par").astype(f32).reshape(-1, 5))
+        _eq(bad, "cov", g["cov"][t0:t1], o.get("trk_cov").astype(f32).reshape(-1, 15))
+        for nm in ("x_ref", "z_ref", "chi2", "z_beam"):
+            _eq(bad, nm, g[nm][t0:t1], o.get("trk_" + nm).astype(f32))
+        # ---- refit + residuals (DESIGN.md section 3.7)
+        _eq(bad, "fit_par", fit["par"][t0:t1], o.get("fit_par").astype(f32).reshape(-1, 5))
+        _eq(bad, "fit_cov", fit["cov"][t0:t1], o.get("fit_cov").astype(f32).reshape(-1, 15))
+        for nm in ("x_ref", "z_ref", "chi2"):
+            _eq(bad, "fit_" + nm, fit[nm][t0:t1], o.get("fit_" + nm).astype(f32))
+        _eq(bad, "fit_n", fit["n_fit"][t0:t1], o.get("fit_n")); _eq(bad, "fit_ndf", fit["ndf"][t0:t1], o.get("fit_ndf"))
+        _eq(bad, "res_y", fit["res_y"][c0:c1], o.get("fit_res_y").astype(f32))
+        _eq(bad, "res_z", fit["res_z"][c0:c1], o.get("fit_res_z").astype(f32))
+    # ---- protection flags (DESIGN.md section 3.8)
+    _eq(bad, "keep", F["keep"][idx], o.protect(*F["road"]))
+    stats = dict(n=sub.n, seeds=K, tracks=To, attached=int((o.get("cluster_track") >= 0).sum()))
+    return s, bad, stats
+
+
+def check_sectors_parallel(frame: dict, sectors, procs=None):
+    """Runs check_sector over `sectors` in a fork()ed pool (children: numpy + the CPU oracle only).  Returns
+    ({sector: [mismatch, ...]}, {sector: stats}, processes used)."""
+    import multiprocessing as mp
+    import os
+    global _FRAME
+    _FRAME = frame
+    sectors = list(sectors)
+    procs = max(1, min(len(sectors), procs or (os.cpu_count() or 1)))
+    try:
+        if procs == 1:
+            res = [check_sector(s) for s in sectors]
+        else:
+            with mp.get_context("fork").Pool(procs) as pool:
+                res = pool.map(check_sector, sectors, chunksize=1)
+    finally:
+        _FRAME = None
+    return {s: b for s, b, _ in res}, {s: st for s, _, st in res}, procs
