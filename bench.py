@@ -35,7 +35,7 @@ FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg5", help="cfg1..cfg5 (BASELINE.json configs[0..4]); cfg5 = the metric's")
@@ -43,6 +43,9 @@ def parse():
     ap.add_argument("--cell-y", type=float, default=0.0, help="override the grid cell along y, cm (debug; 0 = tpc_synth.choose_cell)")
     ap.add_argument("--cell-z", type=float, default=0.0, help="override the grid cell along z, cm (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--parity-sectors", type=int, default=2,
+                    help="sectors of the timed frame checked against the oracle before timing (0: skip)")
+    ap.add_argument("--repeats", type=int, default=10, help="separately-evented steps for median / best (>= 10)")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
 
@@ -117,6 +120,151 @@ class ClockSampler:
                     reasons.add(nm)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# The two legs that execute oracle/ (test infrastructure, never on the product path): the pre-timing parity check of
+# the timed configuration ("each config is also run once through the parity checker before it is
+# timed") and the CPU baseline.  Both run the oracle on whole sectors (sectors are independent) in
+# fork()ed children that inherit the host arrays through _SHARED and never touch CUDA.
+_SHARED = None
+
+
+def _sector_slices(tf):
+    """Input indices of every sector, in input order: one stable argsort instead of 36 masks."""
+    order = np.argsort(tf.sector, kind="stable")
+    counts = np.bincount(tf.sector, minlength=tf.geometry.n_sectors)
+    ends = np.cumsum(counts)
+    return order, ends - counts, ends
+
+
+def _oracle_sector(s: int):
+    """Child: the oracle, as it stands, on sector s; returns (clusters, seconds)."""
+    from oracle import Oracle
+    F = _SHARED
+    tf, idx = F["tf"], F["order"][F["lo"][s]:F["hi"][s]]
+    sec, row, y, z = tf.sector[idx], tf.row[idx], tf.y[idx], tf.z[idx]
+    t0 = time.perf_counter()
+    Oracle(F["P"]).run(sec, row, y, z)
+    return int(idx.size), time.perf_counter() - t0
+
+
+def _parity_sector(s: int):
+    """Child: oracle on sector s against the CUDA result restricted to that sector; list of mismatching arrays."""
+    from oracle import Oracle
+    F = _SHARED
+    tf, P, g = F["tf"], F["P"], F["out"]
+    R = int(P["n_rows"])
+    idx = F["order"][F["lo"][s]:F["hi"][s]]
+    o = Oracle(P).run(tf.sector[idx], tf.row[idx], tf.y[idx], tf.z[idx])
+    a, b = int(F["row_start"][s * R]), int(F["row_start"][(s + 1) * R])
+    bad = []
+
+    def eq(name, x, y_):
+        x = np.asarray(x); y_ = np.asarray(y_)
+        if x.shape != y_.shape or not np.array_equal(x, y_):
+            bad.append(name)
+
+    off = lambda v: np.where(v >= 0, v.astype(np.int64) + a, -1)   # noqa: E731  oracle positions -> frame positions
+    eq("perm", F["perm"][a:b], idx[o.get("perm")])
+    for nm in ("link_up_raw", "link_dn_raw", "link_up", "link_dn"):
+        eq(nm, F[nm][a:b], off(o.get(nm)))
+    mine = np.nonzero(g["sector"] == s)[0]
+    t0, t1 = (int(mine[0]), int(mine[-1]) + 1) if mine.size else (0, 0)
+    To = int(o.get("trk_seed").shape[0])
+    if t1 - t0 != To:
+        bad.append(f"n_tracks {t1 - t0} vs {To}")
+    else:
+        ct = g["cluster_track"][idx].astype(np.int64)
+        eq("cluster_track", np.where(ct >= 0, ct - t0, -1), o.get("cluster_track"))
+        st = g["trk_cl_start"][t0:t1 + 1].astype(np.int64)
+        c0, c1 = (int(st[0]), int(st[-1])) if To else (0, 0)
+        eq("trk_cl_idx", g["trk_cl_idx"][c0:c1], idx[o.get("trk_cl_idx")] if To else np.empty(0, np.int64))
+        eq("par", g["par"][t0:t1], o.get("trk_par").astype(np.float32).reshape(-1, 5))
+        eq("cov", g["cov"][t0:t1], o.get("trk_cov").astype(np.float32).reshape(-1, 15))
+        eq("chi2", g["chi2"][t0:t1], o.get("trk_chi2").astype(np.float32))
+    return s, bad, int(idx.size), To
+
+
+def _fork_map(fn, items, procs):
+    import multiprocessing as mp
+    if procs <= 1 or len(items) <= 1:
+        return [fn(i) for i in items]
+    with mp.get_context("fork").Pool(procs) as pool:
+        return pool.map(fn, items, chunksize=1)
+
+
+def parity_precheck(tf, P, trk, out, n_sectors: int) -> dict:
+    """The timed configuration through the parity checker before it is timed: `n_sectors` whole sectors of the frame,
+    S1 order, raw and cleaned links, assignment, CSR and track parameters, all compared exactly."""
+    global _SHARED
+    S = tf.geometry.n_sectors
+    counts = np.bincount(tf.sector, minlength=S)
+    filled = [s for s in range(S) if counts[s] > 0]
+    # spread over both sides of the TPC
+    pick = sorted({filled[int((i + 0.5) * len(filled) / n_sectors)] for i in range(n_sectors)}) if filled else []
+    order, lo, hi = _sector_slices(tf)
+    shared = dict(tf=tf, P=P, out=out.numpy(), order=order, lo=lo, hi=hi)
+    for nm in ("perm", "row_start", "link_up_raw", "link_dn_raw", "link_up", "link_dn"):
+        shared[nm] = trk.stage_view(nm)
+    _SHARED = shared
+    t0 = time.perf_counter()
+    try:
+        res = _fork_map(_parity_sector, pick, min(len(pick), os.cpu_count() or 1))
+    finally:
+        _SHARED = None
+    bad = {int(s): b for s, b, _, _ in res if b}
+    return {"checked": "oracle vs CUDA, exact: perm, raw + cleaned links, cluster_track, trk_cl_idx, par, cov, chi2",
+            "sectors": [int(s) for s in pick], "clusters": int(sum(n for _, _, n, _ in res)),
+            "tracks": int(sum(t for _, _, _, t in res)), "ok": not bad, "mismatches": bad,
+            "seconds": round(time.perf_counter() - t0, 1)}
+
+
+def cpu_baseline(tf, P, one_thread_clusters=8_000_000) -> dict:
+    """The oracle as it stands on this box's host cores: (i) one thread on a bounded sample of whole
+    sectors, (ii) sector-parallel over P = os.cpu_count() processes on all sectors of the frame (36 independent units;
+    cf. PAPER.md:129).  The headline `value` / `cores` is (ii)."""
+    from oracle import Oracle
+    global _SHARED
+    S = tf.geometry.n_sectors
+    order, lo, hi = _sector_slices(tf)
+    counts = hi - lo
+    take, tot = [], 0
+    for s in range(S):
+        if take and tot + counts[s] > one_thread_clusters:
+            break
+        take.append(s); tot += int(counts[s])
+    idx = np.sort(order[lo[take[0]]:hi[take[-1]]])
+    sub = [a[idx] for a in (tf.sector, tf.row, tf.y, tf.z)]
+    t0 = time.perf_counter()
+    o = Oracle(P).run(*sub)
+    dt1 = time.perf_counter() - t0
+    one = {"value": idx.size / dt1, "unit": UNIT, "cores": 1,
+           "sample": f"sectors {take[0]}..{take[-1]} of {tf.name} ({idx.size} of {tf.n} clusters), all five stages, fp32, {dt1:.1f} s",
+           "stage_seconds": [float(v) for v in o.get("stage_seconds")]}
+    filled = [s for s in range(S) if counts[s] > 0]
+    procs = max(1, min(os.cpu_count() or 1, len(filled)))
+    # bounded: all sectors if that is <= ~30 s of wall at the measured one-thread rate, else the first sectors that fit
+    budget_clusters = one["value"] * procs * 30.0
+    sectors, tot = [], 0
+    for s in filled:
+        if sectors and tot + counts[s] > budget_clusters:
+            break
+        sectors.append(s); tot += int(counts[s])
+    procs = min(procs, len(sectors))
+    _SHARED = dict(tf=tf, P=P, order=order, lo=lo, hi=hi)
+    t0 = time.perf_counter()
+    try:
+        res = _fork_map(_oracle_sector, sectors, procs)
+    finally:
+        _SHARED = None
+    dtp = time.perf_counter() - t0
+    n_par = sum(n for n, _ in res)
+    return {"value": n_par / dtp, "unit": UNIT, "cores": procs, "kind": "oracle",
+            "sample": f"sectors {sectors[0]}..{sectors[-1]} of {tf.name} ({n_par} of {tf.n} clusters), one oracle process per sector over "
+                      f"{procs} processes (os.cpu_count() = {os.cpu_count()}), all five stages, fp32, {dtp:.1f} s wall, "
+                      f"{sum(t for _, t in res):.1f} core-seconds",
+            "one_thread": one}
 
 
 def make_timeframe(args, rank: int):
@@ -264,6 +412,15 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
+    # ---- the timed configuration through the parity checker before it is timed (rank 0, a few whole sectors)
+    parity = None
+    if args.parity_sectors > 0 and rank == 0:
+        trk.track_timeframe(*d_in, out)
+        torch.cuda.synchronize(dev)
+        parity = parity_precheck(tf, P, trk, out, args.parity_sectors)
+        if not parity["ok"]:
+            raise RuntimeError(f"parity check failed before timing: {parity['mismatches']}")
+
     # ---- device-timed: K steps back to back, inputs resident
     for _ in range(args.warmup):
         trk.track_timeframe(*d_in, out)
@@ -281,6 +438,16 @@ def run_ours(args):
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop() if rank == 0 else None
     k = trk.counters()
+
+    # ---- the same step, separately evented (>= 10 repeats): median and best next to the mean
+    reps = max(10, args.repeats)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(reps + 1)]
+    evs[0].record(stream)
+    for i in range(reps):
+        trk.track_timeframe(*d_in, out)
+        evs[i + 1].record(stream)
+    torch.cuda.synchronize(dev)
+    per_step = np.array([evs[i].elapsed_time(evs[i + 1]) for i in range(reps)])
 
     # ---- per-stage device times (events recorded inside the library, separate untimed-by-value runs)
     trk.enable_stage_timing(True)
@@ -370,27 +537,12 @@ def run_ours(args):
                 "stage_ms": {n: float(v) for n, v in zip(names, stage)},
                 "stage_bytes": {n: int(bytes_[n]) for n in names}}
 
-    cpu = None
-    if not args.no_cpu_baseline:
-        from oracle import Oracle
-        # bounded sample: whole sectors, ~15 s of single-threaded oracle work
-        counts = np.bincount(tf.sector, minlength=tf.geometry.n_sectors)
-        take, tot = [], 0
-        for s in range(tf.geometry.n_sectors):
-            if take and tot + counts[s] > 8_000_000:
-                break
-            take.append(s); tot += int(counts[s])
-        sub, _ = select_sectors(tf, take)
-        t0 = time.perf_counter()
-        o = Oracle(P).run(sub.sector, sub.row, sub.y, sub.z)
-        dt = time.perf_counter() - t0
-        cpu = {"value": sub.n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"sectors {take[0]}..{take[-1]} of {tf.name} ({sub.n} of {tf.n} clusters), all five stages, fp32, {dt:.1f} s",
-               "stage_seconds": [float(v) for v in o.get("stage_seconds")]}
+    cpu = None if args.no_cpu_baseline else cpu_baseline(tf, P)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "ms_per_step": ms_step, "ms_per_step_median": float(np.median(per_step)), "ms_per_step_best": float(per_step.min()),
+        "repeats": int(per_step.size), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": tf.name, "n_clusters_per_gpu": tf.n, "n_clusters_total": n_total,
                    "parallelism": "replicas (one time frame per GPU, no collective)" if world > 1 else "single GPU",
@@ -398,6 +550,7 @@ def run_ours(args):
                    "cell_cm": [float(P["cell_y"]), float(P["cell_z"])], "generate_s": round(t_gen, 1),
                    "workspace_GB": round(trk.workspace_bytes / 1e9, 2)},
         "counters": {kk: int(v) for kk, v in k.items()},
+        "parity_before_timing": parity,
         "refit": {"what": "tpc_tracker_refit (separate call, not in the step): all tracks refitted over their owned clusters",
                   "ms": refit_ms},
         "protect": {"what": "tpc_tracker_protect (separate call, not in the step): strategy-B keep flag per cluster, 1 cm road",

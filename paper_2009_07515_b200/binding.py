@@ -372,13 +372,15 @@ def max_bins_bound(sector, z, params: dict) -> int:
     S = int(params["n_sectors"])
     if sector.size == 0:
         return 1
+    ok = np.isfinite(z) & (sector < S)          # non-finite / out-of-range clusters are rejected on the device (status bit)
+    sector, z = sector[ok], z[ok]
     zmin = np.full(S, np.inf); zmax = np.full(S, -np.inf)
     np.minimum.at(zmin, sector, z); np.maximum.at(zmax, sector, z)
     span = np.where(np.isfinite(zmin), zmax - zmin, 0.0)
     nz = np.where(np.isfinite(zmin), np.floor(span / float(params["cell_z"])) + 3, 0)
     rx = np.asarray(params["row_x"], dtype=np.float64)
     ny = np.floor(2.0 * rx * float(params["tan_half_sector"]) / float(params["cell_y"])) + 2
-    return int(nz.sum() * ny.sum()) + 1
+    return int(min(nz.sum() * ny.sum(), float(2**31 - 3))) + 1   # the device raises BINS_OVERFLOW beyond int32
 
 
 def suggest_capacities(n_clusters: int, params: dict) -> dict:

@@ -28,7 +28,10 @@ def test_bench_line_has_the_contract_keys():
         assert k in r, k
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
     c = d["cpu_baseline"]
-    assert c["kind"] == "oracle" and c["cores"] == 1 and c["value"] > 0 and c["unit"] == "clusters/s" and c["sample"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["unit"] == "clusters/s" and c["sample"]
+    assert c["one_thread"]["cores"] == 1 and c["one_thread"]["value"] > 0            # (i) one thread, (ii) sector-parallel
+    assert d["parity_before_timing"]["ok"] is True and d["parity_before_timing"]["sectors"]
+    assert d["repeats"] >= 10 and d["ms_per_step_best"] <= d["ms_per_step_median"]
     e = d["e2e"]
     assert e["value"] > 0 and e["h2d_bytes_per_step"] == d["config"]["n_clusters_per_gpu"] * 10 and e["d2h_bytes_per_step"] > 0
     assert d["gpu_launches"] >= 20 * d["steps"]
