@@ -16,8 +16,7 @@
  * Host resources a handle owns (created by tpc_tracker_create, released by tpc_tracker_destroy): the
  * host struct; 6 CUDA events for the per-stage timing; and, only when created with host_io >= 2,
  * three non-blocking CUDA streams (upload, compute, download), 4 events per staging slot and one
- * 48-byte pinned host block the frame counts are copied into.  When built with graph support a handle
- * also caches one CUDA graph of its launch sequence (tpc_tracker_enable_graph).
+ * 48-byte pinned host block the frame counts are copied into.
  *
  * Thread safety: a handle is NOT thread-safe.  Every call on a handle mutates it (the input pointers of
  * the current frame, the last stream, the slot states), so all calls on one handle must come from one
@@ -85,12 +84,22 @@ typedef struct {
   float max_sinphi;         /* S4 propagation limit */
   float y_margin;           /* S4 sector-exit margin, cm */
   float init_c_ss, init_c_tt, init_c_qq; /* S4 initial variances of sin(phi), tan(lambda), q/pT */
+  /* Native time input ("the TPC hits cannot be converted from native pad, row, and time coordinates
+   * into x, y, and z coordinates ahead of time").  z_is_time = 0: tpc_clusters_t.z is the pseudo-z
+   * in cm and the two values below are ignored.  z_is_time != 0: tpc_clusters_t.z holds the cluster TIME in time units
+   * counted from the start of the time frame, and S1 computes the pseudo-z itself, in fp32, while it reads the input
+   * (no extra pass): zc = drift_length - t * cm_per_time_unit (two roundings), z = zc on the A side (sector <
+   * n_sectors / 2) and 0 - zc on the C side.  cm_per_time_unit = drift velocity x length of a time unit (> 0, finite). */
+  int32_t z_is_time;
+  float cm_per_time_unit;
+  float drift_length;       /* cm, full drift length of one side (250) */
 } tpc_params_t;
 
 /* Input clusters of one time frame, SoA.  DEVICE pointers for tpc_track_timeframe, HOST pointers
  * (ideally pinned) for tpc_track_timeframe_host.  Read-only; must stay valid until the stream has
  * finished the call.  `x` may be NULL and is not read: the tracker uses row_x[row] (pad-row centre).
- * `z` is the pseudo-z in cm computed with vertex time 0 (continuous readout).
+ * `z` is the pseudo-z in cm computed with vertex time 0 (continuous readout) - or, when
+ * tpc_params_t.z_is_time is set, the cluster time in time units (the tracker converts it, see there).
  * Preconditions: coordinates finite; 0 <= n <= max_clusters; DEVICE arrays aligned like fresh
  * allocations (sector and row to 4 bytes, y and z to 16 bytes - the kernels use vector loads), else
  * INVALID_ARG. */
@@ -100,7 +109,7 @@ typedef struct {
   const uint8_t* row;    /* [n] */
   const float* x;        /* [n] or NULL (unused) */
   const float* y;        /* [n] sector-local y, cm */
-  const float* z;        /* [n] pseudo-z, cm */
+  const float* z;        /* [n] pseudo-z, cm (z_is_time = 0) or time, time units (z_is_time != 0) */
 } tpc_clusters_t;
 
 /* Output tracks, SoA, caller-allocated with the stated capacities.  DEVICE pointers for

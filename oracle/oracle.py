@@ -24,7 +24,11 @@ class _Params(C.Structure):
         ("min_track_hits", C.c_int32),
         ("pick_chi2_cut", C.c_float), ("max_sinphi", C.c_float), ("y_margin", C.c_float),
         ("init_c_ss", C.c_float), ("init_c_tt", C.c_float), ("init_c_qq", C.c_float),
+        ("z_is_time", C.c_int32), ("cm_per_time_unit", C.c_float), ("drift_length", C.c_float),
     ]
+
+
+_DEFAULTS = {"z_is_time": 0, "cm_per_time_unit": 0.0, "drift_length": 0.0}
 
 
 _KINDS = {0: np.int32, 1: np.float32, 2: np.float64, 3: np.uint64, 4: np.int64}
@@ -77,7 +81,8 @@ def _pack(params: dict) -> _Params:
             for i, v in enumerate(rx):
                 p.row_x[i] = float(v)
         else:
-            setattr(p, name, params[name].item() if hasattr(params[name], "item") else params[name])
+            v = params[name] if name in params else _DEFAULTS[name]
+            setattr(p, name, v.item() if hasattr(v, "item") else v)
     return p
 
 

@@ -51,6 +51,7 @@ struct Params {             // mirrors the ctypes Structure in oracle/oracle.py 
   float link_ay, link_az, link_b, link_T;
   int32_t min_chain_len, max_gap, min_tracklet_hits, min_track_hits;
   float pick_chi2_cut, max_sinphi, y_margin, init_c_ss, init_c_tt, init_c_qq;
+  int32_t z_is_time; float cm_per_time_unit, drift_length;   // native time input, DESIGN.md section 3.0a
 };
 
 // floor(v) clamped to [0, hi]; defined for every v (NaN and negatives -> 0), DESIGN.md section 3.1 (3)
@@ -214,6 +215,7 @@ struct Oracle {
   int64_t n = 0;
   const uint8_t* in_sector = nullptr; const uint8_t* in_row = nullptr;
   const float* in_y = nullptr; const float* in_z = nullptr;
+  std::vector<float> z_from_time;      // pseudo-z computed from the native time, when z_is_time
 
   // S1
   std::vector<float> zmin, zmax; std::vector<int32_t> nz;         // per sector
@@ -643,6 +645,17 @@ struct Oracle {
 
   int run(int64_t n_, const uint8_t* sec, const uint8_t* row, const float* y, const float* z, int prec, int last_stage) {
     n = n_; in_sector = sec; in_row = row; in_y = y; in_z = z;
+    if (P.z_is_time) {
+      // the input holds the cluster time t in time units; its pseudo-z (vertex
+      // time 0) is the drift distance left at time t, positive on the A side (sectors < n_sectors / 2), negative on the C
+      // side.  fp32, the product and the difference rounded separately.
+      z_from_time.resize(n);
+      for (int64_t i = 0; i < n; ++i) {
+        const float zc = P.drift_length - z[i] * P.cm_per_time_unit;
+        z_from_time[i] = (int)sec[i] < P.n_sectors / 2 ? zc : 0.0f - zc;
+      }
+      in_z = z_from_time.data();
+    }
     stage_seconds.assign(5, 0.0);
     auto now = [] { return std::chrono::steady_clock::now(); };
     auto secs = [](auto a, auto b) { return std::chrono::duration<double>(b - a).count(); };

@@ -28,7 +28,11 @@ class tpc_params_t(C.Structure):
         ("min_track_hits", C.c_int32),
         ("pick_chi2_cut", C.c_float), ("max_sinphi", C.c_float), ("y_margin", C.c_float),
         ("init_c_ss", C.c_float), ("init_c_tt", C.c_float), ("init_c_qq", C.c_float),
+        ("z_is_time", C.c_int32), ("cm_per_time_unit", C.c_float), ("drift_length", C.c_float),
     ]
+
+
+_PARAM_DEFAULTS = {"z_is_time": 0, "cm_per_time_unit": 0.0, "drift_length": 0.0}   # pseudo-z input unless asked otherwise
 
 
 class tpc_clusters_t(C.Structure):
@@ -145,7 +149,7 @@ def pack_params(params: dict):
         if name == "row_x":
             p.row_x = rx.ctypes.data
         else:
-            v = params[name]
+            v = params[name] if name in params else _PARAM_DEFAULTS[name]
             setattr(p, name, v.item() if hasattr(v, "item") else v)
     return p, rx
 
@@ -370,6 +374,9 @@ def max_bins_bound(sector, z, params: dict) -> int:
     sector; the tracker computes the exact grids itself on the device)."""
     sector = np.asarray(sector); z = np.asarray(z, dtype=np.float64)
     S = int(params["n_sectors"])
+    if params.get("z_is_time", 0):              # native time input: the span of the pseudo-z the device will compute
+        zc = float(params["drift_length"]) - z * float(params["cm_per_time_unit"])
+        z = np.where(sector < S // 2, zc, -zc)
     if sector.size == 0:
         return 1
     ok = np.isfinite(z) & (sector < S)          # non-finite / out-of-range clusters are rejected on the device (status bit)

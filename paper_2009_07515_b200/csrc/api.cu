@@ -56,6 +56,8 @@ bool params_ok(const tpc_params_t* p) {
   if ((int64_t)p->n_sectors * p->n_rows > 65535) return false;
   if (!(p->cell_y > 0.f) || !(p->cell_z > 0.f) || !(p->tan_half_sector > 0.f)) return false;
   if (p->min_chain_len < 2 || p->max_gap < 0) return false;
+  if (p->z_is_time && (!(p->cm_per_time_unit > 0.f) || !(p->cm_per_time_unit < INFINITY) || !(std::fabs(p->drift_length) < INFINITY)))
+    return false;
   for (int r = 0; r < p->n_rows; ++r) {
     if (!(p->row_x[r] > 0.f)) return false;
     if (r && !(p->row_x[r] > p->row_x[r - 1])) return false;
@@ -136,6 +138,7 @@ void fill_ctx_constants(tpc_tracker* t, std::vector<RowTab>& tab) {
   c.min_tracklet_hits = p.min_tracklet_hits; c.min_track_hits = p.min_track_hits;
   c.pick_chi2_cut = p.pick_chi2_cut; c.max_sinphi = p.max_sinphi; c.y_margin = p.y_margin;
   c.init_c_ss = p.init_c_ss; c.init_c_tt = p.init_c_tt; c.init_c_qq = p.init_c_qq;
+  c.z_is_time = p.z_is_time != 0; c.cm_per_time_unit = p.cm_per_time_unit; c.drift_length = p.drift_length;
   tab.assign(R, RowTab{});
   int acc = 0;
   for (int r = 0; r < R; ++r) {

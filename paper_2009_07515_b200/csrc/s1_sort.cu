@@ -44,7 +44,8 @@ __global__ void __launch_bounds__(kThreads) k_zrange_count(Ctx c, int use_smem_h
   __syncthreads();
   bool bad = false;
   const long long n = c.n;
-  auto one = [&](int s, int r, float z) {
+  auto one = [&](int s, int r, float zin) {
+    const float z = input_z(c, s, zin);                  // cm as given, or converted from the native time (section 3.0a)
     // a non-finite z has no bin (and an infinite one would make the z range, hence the bin count, meaningless)
     if (s >= c.S || r >= c.R || !(fabsf(z) < INFINITY)) { bad = true; return; }
     const int key = float_key(z);
@@ -178,7 +179,8 @@ __global__ void __launch_bounds__(kThreads) k_partition(Ctx c) {
   if (c.cnt->status) return;
   const long long n = c.n;
   bool bad = false;
-  auto one = [&](int s, int r, float y, float z, long long i) {
+  auto one = [&](int s, int r, float y, float zin, long long i) {
+    const float z = input_z(c, s, zin);
     if (!(fabsf(y) < INFINITY)) bad = true;             // precondition: finite coordinates (z was checked by k_zrange_count)
     const int pos = atomicAdd(c.sr_cursor + s * c.R + r, 1);
     c.rec[pos] = make_float4(y, z, __int_as_float((int)i), 0.0f);

@@ -52,6 +52,7 @@ struct Ctx {
   float err_y2, err_z2, link_T;
   int min_chain_len, max_gap, min_tracklet_hits, min_track_hits;
   float pick_chi2_cut, max_sinphi, y_margin, init_c_ss, init_c_tt, init_c_qq;
+  int z_is_time; float cm_per_time_unit, drift_length;   // native time input
   const RowTab* rowtab;               // [R]
   // capacities
   int max_clusters; int max_bins; int max_seeds; int max_tracks; int max_track_clusters;
@@ -130,6 +131,14 @@ __device__ __forceinline__ int floor_clamp(float v, int hi) {
   //   f = floorf(v); !(f >= 0) ? 0 : f >= (float)hi ? hi : (int)f      (hi >= 0)
   // in three instructions
   return min(max(__float2int_rd(v), 0), hi);
+}
+
+// the pseudo-z of an input cluster of sector s whose z entry is v (cm, or time units when
+// z_is_time).  -fmad=false: the product and the difference are rounded separately, like the oracle's.
+__device__ __forceinline__ float input_z(const Ctx& c, int s, float v) {
+  if (!c.z_is_time) return v;
+  const float zc = c.drift_length - v * c.cm_per_time_unit;
+  return s < (c.S >> 1) ? zc : 0.0f - zc;
 }
 
 // order-preserving float <-> int key (signed compare)

@@ -69,6 +69,50 @@ def test_mini_timeframe_pileup(mini_tf):
     print(t, res)
 
 
+def test_native_time_input_bit_exact(mini_tf):
+    """the z array holds native cluster times; S1 converts while it reads.  Every
+    stage, the refit and z_beam bit-exact against the oracle on the same times; the sorted z the tracker works on is
+    within the fp32 rounding of the time of the frame's own pseudo-z."""
+    from tpc_synth import to_native_time
+    tft, tp = to_native_time(mini_tf)
+    P = default_params(mini_tf); P.update(tp)
+    _, trk, out = run_gpu(tft, params=P)
+    o = run_oracle(tft, P)
+    assert trk.counters()["status"] == 0
+    assert not compare_integer_stages(trk, o)
+    t = compare_tracklets(trk, o)
+    assert t["hit_mismatch_seeds"] == 0 and t["par_bitexact"] and t["cov_bitexact"] and t["chi2_bitexact"], t
+    res = compare_tracks(out.numpy(), o, tft.n)
+    assert res["cluster_track_equal"] and res["csr_equal"] and res["n_tracks"][0] > 1000, res
+    g = out.numpy()
+    assert np.array_equal(g["z_beam"], o.get("trk_z_beam").astype(np.float32))
+    assert np.array_equal(g["z_ref"], o.get("trk_z_ref").astype(np.float32))
+    z_in = np.empty(tft.n, np.float32); z_in[trk.stage_view("perm")] = trk.stage_view("yz").reshape(-1, 2)[:, 1]
+    assert np.abs(z_in.astype(np.float64) - mini_tf.z).max() < 1e-3
+    # the host path converts the same way
+    _, trk_h, out_h = run_gpu(tft, params=P, host=True)
+    assert np.array_equal(out_h.numpy()["cluster_track"], g["cluster_track"])
+
+
+def test_native_time_input_rejects_bad_parameters_and_flags_overflowing_times(cfg1):
+    import paper_2009_07515_b200 as tpc
+    from tpc_synth import to_native_time
+    tft, tp = to_native_time(cfg1)
+    for bad in (dict(cm_per_time_unit=np.float32(0.0)), dict(cm_per_time_unit=np.float32(np.inf)),
+                dict(drift_length=np.float32(np.nan))):
+        P = default_params(cfg1); P.update(tp); P.update(bad)
+        with pytest.raises((RuntimeError, ValueError)):
+            tpc.Tracker(P, 1024, 1024, 64, 64, 1024)
+    # a time so large that the z grid would need more rows than an int32 holds (or whose pseudo-z is not finite): a status
+    # bit, nothing written out of bounds
+    P = default_params(cfg1); P.update(tp)
+    t = tft.z.copy(); t[17] = np.float32(3e38)
+    import copy
+    tfb = copy.copy(tft); tfb.z = t
+    _, trk, out = run_gpu(tfb, params=P, caps=dict(max_bins=1 << 22), guard_bytes=1 << 20)
+    assert out.numpy()["status"] & 3 and out.numpy()["n_tracks"] == 0 and trk.guards_intact()
+
+
 def test_reports_bit_exactness(mini_event):
     """Not a requirement of north_star, but the design goal: identical op order => identical bits."""
     P, trk, out = run_gpu(mini_event)

@@ -17,4 +17,5 @@ from .generator import (  # noqa: F401
     choose_cell,
     default_params,
     select_sectors,
+    to_native_time,
 )

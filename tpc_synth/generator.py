@@ -310,6 +310,20 @@ def default_params(tf: TimeFrame, cell: float | None = None) -> dict:
     )
 
 
+def to_native_time(tf: TimeFrame, time_unit_us: float = 0.2) -> tuple[TimeFrame, dict]:
+    """The same time frame with the NATIVE time coordinate in place of the pseudo-z: a cluster is read
+    out at t = t_coll + (L - |z_true|) / v_d after the start of the frame, i.e. t = (L -+ z') / v_d for the pseudo-z z'
+    on the A / C side; here in units of `time_unit_us` (0.2 us = one TPC time bin), evaluated in double from the frame's
+    own z', cast to fp32 last.  Returns (frame whose `z` holds t, the three tpc_params_t entries that describe it)."""
+    g = tf.geometry
+    side = np.where(tf.sector < g.n_azimuthal, 1.0, -1.0)
+    t = (g.drift_length - side * tf.z.astype(np.float64)) / (g.v_drift * float(time_unit_us))
+    out = TimeFrame(sector=tf.sector, row=tf.row, x=tf.x, y=tf.y, z=t.astype(np.float32), track_id=tf.track_id,
+                    truth=tf.truth, geometry=g, tf_length_us=tf.tf_length_us, sigma=tf.sigma, name=tf.name + "+time")
+    return out, dict(z_is_time=1, cm_per_time_unit=np.float32(g.v_drift * float(time_unit_us)),
+                     drift_length=np.float32(g.drift_length))
+
+
 def select_sectors(tf: TimeFrame, sectors) -> tuple[TimeFrame, np.ndarray]:
     """Sub-frame holding only the clusters of ``sectors`` (order kept) + their input indices."""
     keep = np.isin(tf.sector, np.asarray(list(sectors), dtype=np.uint8))
