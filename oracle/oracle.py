@@ -63,6 +63,10 @@ def _load():
                                    C.c_void_p, C.c_void_p]
         lib.orc_protect.restype = None
         lib.orc_protect.argtypes = [C.c_void_p, C.c_float, C.c_float]
+        lib.orc_merge.restype = None
+        lib.orc_merge.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float]
+        lib.orc_kf_rotate.restype = C.c_double
+        lib.orc_kf_rotate.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double]
         lib.orc_search.restype = C.c_int
         lib.orc_search.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_int]
         lib.orc_beam_z.restype = C.c_double
@@ -113,9 +117,20 @@ class Oracle:
         return self
 
     def protect(self, road_y: float, road_z: float) -> np.ndarray:
-        """DESIGN.md section 3.9 on the tracks of the last run: keep flag per INPUT cluster."""
+        """DESIGN.md section 3.8 on the tracks of the last run: keep flag per INPUT cluster."""
         self._lib.orc_protect(self._h, float(road_y), float(road_z))
         return self.get("keep")
+
+    def merge(self, max_rows: int = 30, back_rows: int = 1, edge: float = 6.0, dz_win: float = 100.0,
+              chi2_cut: float = 100.0) -> "Oracle":
+        """DESIGN.md section 3.9 on the tracks and the refit of the last run (last_stage = 6): results under mrg_*."""
+        self._lib.orc_merge(self._h, int(max_rows), int(back_rows), float(edge), float(dz_win), float(chi2_cut))
+        return self
+
+    def kf_rotate(self, par, cov15, x, sa, ca, precision=64):
+        par = np.array(par, dtype=np.float64); cov = np.array(cov15, dtype=np.float64)
+        xn = self._lib.orc_kf_rotate(C.byref(self._p), precision, par.ctypes.data, cov.ctypes.data, float(x), float(sa), float(ca))
+        return (not np.isnan(xn)), par, cov, float(xn)
 
     def get(self, name: str) -> np.ndarray:
         ptr = C.c_void_p(); n = C.c_int64(); kind = C.c_int()

@@ -200,6 +200,49 @@ void kf_reset_cov(KF<T>& k, const Params& P) {
   k.chi2 = T(0);
 }
 
+
+// Rotation of the state into the sector frame turned by alpha about the beam axis (sa = sin(alpha), ca = cos(alpha)),
+// DESIGN.md section 3.9.2.  The point and the direction turn rigidly; the state is then given at the plane
+// x' = x*ca + y*sa of the new frame (returned in *x_new), so the covariance moves with the Jacobian of "turn, then
+// slide along the track back onto that plane".  Plain operations, one rounding each (no fma).  Returns false and leaves
+// the state untouched if the track is too steep in either frame.
+template <class T>
+bool kf_rotate(KF<T>& k, T kb, T x, T sa, T ca, T max_sinphi, T* x_new) {
+  const T y = k.p[0], s = k.p[2], t = k.p[3], q = k.p[4];
+  if (!(std::fabs(s) < max_sinphi)) return false;
+  const T c = std::sqrt(T(1) - s * s);
+  const T s1 = s * ca - c * sa;
+  const T c1 = c * ca + s * sa;
+  if (!(std::fabs(s1) < max_sinphi) || !(c1 > T(0))) return false;
+  const T xn = x * ca + y * sa;
+  const T yn = y * ca - x * sa;
+  T J[5][5];
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j < 5; ++j) J[i][j] = (i == j) ? T(1) : T(0);
+  J[0][0] = c / c1;                           // d y'/d y: the slide along the track back to the plane x' = const
+  J[1][0] = ((T(0) - sa) * t) / c1;           // d z'/d y
+  J[2][0] = (T(0) - kb * q) * sa;             // d s'/d y: the curvature acts over the slide
+  J[2][2] = c1 / c;                           // d sin(phi - alpha)/d sin(phi)
+  T M[5][5], C1[5][5];
+  for (int i = 0; i < 5; ++i)
+    for (int l = 0; l < 5; ++l) {
+      T acc = T(0);
+      for (int kk = 0; kk < 5; ++kk) acc = acc + J[i][kk] * k.C[kk][l];
+      M[i][l] = acc;
+    }
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j <= i; ++j) {
+      T acc = T(0);
+      for (int l = 0; l < 5; ++l) acc = acc + M[i][l] * J[j][l];
+      C1[i][j] = acc; C1[j][i] = acc;
+    }
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j < 5; ++j) k.C[i][j] = C1[i][j];
+  k.p[0] = yn; k.p[2] = s1;
+  *x_new = xn;
+  return true;
+}
+
 // ------------------------------------------------------------------------------------------
 struct Oracle {
   Params P;
@@ -248,6 +291,15 @@ struct Oracle {
   std::vector<double> fit_res_y, fit_res_z;                        // parallel to trk_cl_idx: residual to the extrapolated track
   // S8 cluster protection, "strategy B"
   std::vector<int32_t> keep;                                       // [n] by INPUT index: 1 protected, 0 removable
+  // S9 track merger
+  std::vector<int32_t> fit_row;                                    // [n_tracks] row of the state of the downward refit
+  std::vector<double> up_par, up_cov, up_x_ref, up_z_ref, up_chi2; // upward refit: state at the highest fitted row
+  std::vector<int32_t> up_row, up_n;
+  std::vector<int32_t> mrg_best_b, mrg_best_a, mrg_next, mrg_prev, mrg_dir;   // [n_tracks]
+  std::vector<double> mrg_chi2_b;                                  // [n_tracks] score of best_b (or -1)
+  std::vector<int32_t> mrg_of_track, mrg_seg_start, mrg_seg_idx;   // merged id of every track; CSR merged -> tracks, inner to outer
+  std::vector<double> mrg_par, mrg_cov, mrg_x_ref, mrg_z_ref, mrg_chi2;
+  std::vector<int32_t> mrg_n_fit, mrg_ndf, mrg_sector, mrg_n_clusters;
   int s4_prec = 32;
   std::vector<int32_t> trk_cl_start, trk_cl_idx, cluster_track;
   std::vector<double> stage_seconds;                              // [5]
@@ -596,7 +648,7 @@ struct Oracle {
   void stage6() {
     const size_t nt = trk_seed.size();
     fit_par.assign(nt * 5, 0.0); fit_cov.assign(nt * 15, 0.0); fit_x_ref.assign(nt, 0.0); fit_z_ref.assign(nt, 0.0);
-    fit_chi2.assign(nt, 0.0); fit_ndf.assign(nt, 0); fit_n.assign(nt, 0);
+    fit_chi2.assign(nt, 0.0); fit_ndf.assign(nt, 0); fit_n.assign(nt, 0); fit_row.assign(nt, 0);
     fit_res_y.assign(trk_cl_idx.size(), 0.0); fit_res_z.assign(trk_cl_idx.size(), 0.0);
     const T kbT = T(kb), msp = T(P.max_sinphi), ey2 = T(P.err_y2), ez2 = T(P.err_z2);
     for (size_t id = 0; id < nt; ++id) {
@@ -623,8 +675,185 @@ struct Oracle {
         cur = r; ++nfit;
       }
       store_kf(k, &fit_par[id * 5], &fit_cov[id * 15], &fit_chi2[id]);
-      fit_x_ref[id] = (double)P.row_x[cur]; fit_z_ref[id] = (double)zref;
+      fit_x_ref[id] = (double)P.row_x[cur]; fit_z_ref[id] = (double)zref; fit_row[id] = cur;
       fit_n[id] = nfit; fit_ndf[id] = 2 * nfit - 5;
+    }
+  }
+
+
+  // ---------------------------------------------------------------------------------------- S9
+  // Track merger ("Track Fit" of PAPER.md:99, 131, 138: the segments a track was found in - one per
+  // sector it crosses, and one per stretch between holes longer than max_gap - are joined and refitted).  Runs after
+  // stage6 (the downward refit gives every segment's state at its INNER end).
+  //   9.1 upward refit: the state at the OUTER end;  9.2-9.4 candidates and score;  9.5 mutual best;  9.6 chains;
+  //   9.7 downward refit of every merged track through all its segments, turning the frame at sector changes.
+  struct MergeCuts { int32_t max_rows, back_rows; float edge, dz_win, chi2_cut; };
+
+  template <class T>
+  void stage9(const MergeCuts& mc) {
+    const int nt = (int)trk_seed.size(), n_az = P.n_sectors / 2;
+    const T kbT = T(kb), msp = T(P.max_sinphi), ey2 = T(P.err_y2), ez2 = T(P.err_z2);
+    // sin and cos of the sector angle (twice the half-sector angle) from tan_half_sector alone: no libm (section 3.0)
+    const T th = T(P.tan_half_sector);
+    const T den = T(1) + th * th;
+    const T sin_a = (T(2) * th) / den, cos_a = (T(1) - th * th) / den;
+
+    // ---- 9.1 upward refit: seed at the lowest owned cluster from the direction to the next one, q/pT of the downward
+    // refit as the starting value, then propagate + update (no gate) through the owned clusters in ascending row
+    up_par.assign((size_t)nt * 5, 0.0); up_cov.assign((size_t)nt * 15, 0.0); up_x_ref.assign(nt, 0.0); up_z_ref.assign(nt, 0.0);
+    up_chi2.assign(nt, 0.0); up_row.assign(nt, 0); up_n.assign(nt, 0);
+    for (int id = 0; id < nt; ++id) {
+      const int32_t* cl = &trk_cl_pos[trk_cl_start[id]];
+      const int m = trk_cl_start[id + 1] - trk_cl_start[id];
+      if (m < 2) continue;
+      const int bot = cl[0], nxt = cl[1];
+      const T zref = T(zs[bot]);
+      const T dx = T(P.row_x[s_row[nxt]]) - T(P.row_x[s_row[bot]]);
+      const T dy = T(ys[nxt]) - T(ys[bot]), dz = T(zs[nxt]) - T(zs[bot]);
+      const T dl = std::sqrt(dx * dx + dy * dy);
+      KF<T> k;
+      k.p[0] = T(ys[bot]); k.p[1] = T(0); k.p[2] = dy / dl; k.p[3] = dz / dl; k.p[4] = T(fit_par[(size_t)id * 5 + 4]);
+      kf_reset_cov(k, P);
+      int cur = s_row[bot], nfit = 1;
+      for (int i = 1; i < m; ++i) {
+        const int c = cl[i], r = s_row[c];
+        if (!kf_propagate<T>(k, kbT, T(P.row_x[r]) - T(P.row_x[cur]), msp, (T*)nullptr)) break;
+        kf_update<T>(k, T(ys[c]), T(zs[c]) - zref, ey2, ez2);
+        cur = r; ++nfit;
+      }
+      store_kf(k, &up_par[(size_t)id * 5], &up_cov[(size_t)id * 15], &up_chi2[id]);
+      up_x_ref[id] = (double)P.row_x[cur]; up_z_ref[id] = (double)zref; up_row[id] = cur; up_n[id] = nfit;
+    }
+
+    // ---- 9.2 absolute z of the two ends (one rounding each)
+    std::vector<T> z_in(nt), z_out(nt);
+    for (int id = 0; id < nt; ++id) {
+      z_in[id] = T(fit_z_ref[id]) + T(fit_par[(size_t)id * 5 + 1]);
+      z_out[id] = T(up_z_ref[id]) + T(up_par[(size_t)id * 5 + 1]);
+    }
+    // tracks of a sector ordered by z_in (a library sort as a step: it only speeds the window scan up, the candidate set
+    // is defined by the predicate of 9.3)
+    std::vector<std::vector<int32_t>> by_sector(P.n_sectors);
+    for (int id = 0; id < nt; ++id) by_sector[trk_sector[id]].push_back(id);
+    for (auto& v : by_sector) std::sort(v.begin(), v.end(), [&](int32_t a, int32_t b) { return z_in[a] < z_in[b] || (z_in[a] == z_in[b] && a < b); });
+
+    // ---- 9.3 / 9.4 / 9.5: score of every candidate pair; best partner of every outer end and of every inner end
+    mrg_best_b.assign(nt, -1); mrg_best_a.assign(nt, -1); mrg_chi2_b.assign(nt, -1.0); mrg_dir.assign(nt, 0);
+    std::vector<T> best_a_chi2(nt, T(0));
+    std::vector<int32_t> best_b_dir(nt, 0), best_a_dir(nt, 0);
+    const T dzw = T(mc.dz_win), cut = T(mc.chi2_cut);
+    for (int a = 0; a < nt; ++a) {
+      if (up_n[a] < 2 || fit_n[a] < 2) continue;
+      const int sa_ = trk_sector[a], ra = up_row[a];
+      const T ya = T(up_par[(size_t)a * 5 + 0]);
+      T best = T(0); int bb = -1, bdir = 0;
+      for (int pass = 0; pass < 2; ++pass) {
+        int dir = 0, sb = sa_;
+        if (pass == 1) {
+          // the neighbour the outer end is heading for: only if that end lies within `edge` of the sector boundary
+          if (!(std::fabs(ya) >= T(ymax[ra]) - T(mc.edge))) continue;
+          dir = ya >= T(0) ? 1 : -1;
+          sb = (sa_ / n_az) * n_az + ((sa_ % n_az) + dir + n_az) % n_az;
+          if (sb == sa_) continue;                        // a one-sector geometry has no neighbour
+        }
+        const auto& lst = by_sector[sb];
+        const T zlo = z_out[a] - dzw, zhi = z_out[a] + dzw;
+        auto it = std::lower_bound(lst.begin(), lst.end(), zlo, [&](int32_t b, T v) { return z_in[b] < v; });
+        for (; it != lst.end() && z_in[*it] <= zhi; ++it) {
+          const int b = *it;
+          if (b == a || up_n[b] < 2 || fit_n[b] < 2) continue;
+          const int rb = fit_row[b];
+          if (dir == 0 ? (rb < ra + 1 || rb > ra + mc.max_rows) : (rb < ra - mc.back_rows || rb > ra + mc.max_rows)) continue;
+          // 9.4 the outer state of a, turned into b's frame if that is another sector, moved to b's inner plane
+          KF<T> k; load_kf(k, &up_par[(size_t)a * 5], &up_cov[(size_t)a * 15], 0.0);
+          T x = T(up_x_ref[a]);
+          if (dir != 0 && !kf_rotate<T>(k, kbT, x, dir > 0 ? sin_a : T(0) - sin_a, cos_a, msp, &x)) continue;
+          if (!kf_propagate<T>(k, kbT, T(fit_x_ref[b]) - x, msp, (T*)nullptr)) continue;
+          const double* pb = &fit_par[(size_t)b * 5]; const double* cb = &fit_cov[(size_t)b * 15];
+          T d[5];
+          d[0] = T(pb[0]) - k.p[0];
+          d[1] = z_in[b] - (T(up_z_ref[a]) + k.p[1]);
+          d[2] = T(pb[2]) - k.p[2]; d[3] = T(pb[3]) - k.p[3]; d[4] = T(pb[4]) - k.p[4];
+          T chi = T(0);
+          for (int i = 0; i < 5; ++i) chi = chi + (d[i] * d[i]) / (k.C[i][i] + T(cb[i * (i + 1) / 2 + i]));
+          if (!(chi <= cut)) continue;
+          // 9.5 the best partner of a's outer end (ties -> lowest b) and of b's inner end (ties -> lowest a)
+          if (bb < 0 || chi < best || (chi == best && b < bb)) { best = chi; bb = b; bdir = dir; }
+          if (mrg_best_a[b] < 0 || chi < best_a_chi2[b] || (chi == best_a_chi2[b] && a < mrg_best_a[b])) {
+            best_a_chi2[b] = chi; mrg_best_a[b] = a; best_a_dir[b] = dir;
+          }
+        }
+      }
+      mrg_best_b[a] = bb; best_b_dir[a] = bdir; mrg_chi2_b[a] = bb >= 0 ? (double)best : -1.0;
+    }
+    // ---- 9.6 mutual links and chains
+    mrg_next.assign(nt, -1); mrg_prev.assign(nt, -1);
+    for (int a = 0; a < nt; ++a) {
+      const int b = mrg_best_b[a];
+      if (b >= 0 && mrg_best_a[b] == a) { mrg_next[a] = b; mrg_prev[b] = a; mrg_dir[a] = best_b_dir[a]; }
+    }
+    mrg_of_track.assign(nt, -1); mrg_seg_start.assign(1, 0); mrg_seg_idx.clear();
+    for (int h = 0; h < nt; ++h) {
+      if (mrg_prev[h] >= 0) continue;                     // heads in ascending track id
+      const int32_t id = (int32_t)mrg_seg_start.size() - 1;
+      int len = 0;
+      for (int k2 = h; k2 >= 0 && len < nt; k2 = mrg_next[k2], ++len) { mrg_of_track[k2] = id; mrg_seg_idx.push_back(k2); }
+      mrg_seg_start.push_back((int32_t)mrg_seg_idx.size());
+    }
+    // ---- 9.7 downward refit of every merged track: from the top cluster of the outermost segment through all owned
+    // clusters of all segments in turn, the frame turned back at every sector change
+    const int nm = (int)mrg_seg_start.size() - 1;
+    mrg_par.assign((size_t)nm * 5, 0.0); mrg_cov.assign((size_t)nm * 15, 0.0); mrg_x_ref.assign(nm, 0.0); mrg_z_ref.assign(nm, 0.0);
+    mrg_chi2.assign(nm, 0.0); mrg_n_fit.assign(nm, 0); mrg_ndf.assign(nm, 0); mrg_sector.assign(nm, 0); mrg_n_clusters.assign(nm, 0);
+    for (int mId = 0; mId < nm; ++mId) {
+      const int s0 = mrg_seg_start[mId], s1 = mrg_seg_start[mId + 1];
+      int ncl = 0;
+      for (int q = s0; q < s1; ++q) ncl += trk_cl_start[mrg_seg_idx[q] + 1] - trk_cl_start[mrg_seg_idx[q]];
+      mrg_n_clusters[mId] = ncl;
+      const int last = mrg_seg_idx[s1 - 1];
+      const int32_t* cl = &trk_cl_pos[trk_cl_start[last]];
+      const int m = trk_cl_start[last + 1] - trk_cl_start[last];
+      if (m < 2) continue;
+      const int top = cl[m - 1], nxt = cl[m - 2];
+      const T zref = T(zs[top]);
+      const T dx = T(P.row_x[s_row[top]]) - T(P.row_x[s_row[nxt]]);
+      const T dy = T(ys[top]) - T(ys[nxt]), dz = T(zs[top]) - T(zs[nxt]);
+      const T dl = std::sqrt(dx * dx + dy * dy);
+      KF<T> k;
+      k.p[0] = T(ys[top]); k.p[1] = T(0); k.p[2] = dy / dl; k.p[3] = dz / dl; k.p[4] = T(trk_par[(size_t)last * 5 + 4]);   // as section 3.7
+      kf_reset_cov(k, P);
+      T x = T(P.row_x[s_row[top]]);
+      int nfit = 1, sector = trk_sector[last];
+      bool ok = true;
+      for (int q = s1 - 1; q >= s0 && ok; --q) {
+        const int seg = mrg_seg_idx[q];
+        const int32_t* c2 = &trk_cl_pos[trk_cl_start[seg]];
+        const int m2 = trk_cl_start[seg + 1] - trk_cl_start[seg];
+        if (q < s1 - 1) {                                 // coming down from segment q+1 into segment q
+          const int dir = mrg_dir[seg];                   // the link seg -> next went `dir` sectors up; go back
+          if (dir != 0) {
+            // first, still in the upper segment's frame, to the plane through the top cluster of segment q (its x in
+            // that frame: the point turned by +dir), where the track is no steeper than the finder saw it; then turn
+            const int ct = c2[m2 - 1];
+            const T sd = dir > 0 ? sin_a : T(0) - sin_a;
+            const T xt = T(P.row_x[s_row[ct]]) * cos_a + T(ys[ct]) * sd;
+            if (!kf_propagate<T>(k, kbT, xt - x, msp, (T*)nullptr)) break;
+            x = xt;
+            if (!kf_rotate<T>(k, kbT, x, T(0) - sd, cos_a, msp, &x)) break;
+          }
+          sector = trk_sector[seg];
+        }
+        for (int i = (q == s1 - 1 ? m2 - 2 : m2 - 1); i >= 0; --i) {
+          const int c = c2[i], r = s_row[c];
+          if (!kf_propagate<T>(k, kbT, T(P.row_x[r]) - x, msp, (T*)nullptr)) { ok = false; break; }
+          x = T(P.row_x[r]);
+          kf_update<T>(k, T(ys[c]), T(zs[c]) - zref, ey2, ez2);
+          ++nfit;
+        }
+      }
+      store_kf(k, &mrg_par[(size_t)mId * 5], &mrg_cov[(size_t)mId * 15], &mrg_chi2[mId]);
+      mrg_x_ref[mId] = (double)x; mrg_z_ref[mId] = (double)zref; mrg_n_fit[mId] = nfit; mrg_ndf[mId] = 2 * nfit - 5;
+      mrg_sector[mId] = sector;
     }
   }
 
@@ -768,6 +997,10 @@ int orc_get(void* h, const char* name, const void** ptr, int64_t* n, int* kind) 
   F64(trk_par); F64(trk_cov); F64(trk_x_ref); F64(trk_z_ref); F64(trk_chi2); F64(trk_z_beam);
   I32(trk_cl_start); I32(trk_cl_idx); I32(trk_cl_pos); I32(cluster_track); F64(stage_seconds);
   I32(keep); F64(fit_res_y); F64(fit_res_z); F64(fit_par); F64(fit_cov); F64(fit_x_ref); F64(fit_z_ref); F64(fit_chi2); I32(fit_ndf); I32(fit_n);
+  I32(fit_row); F64(up_par); F64(up_cov); F64(up_x_ref); F64(up_z_ref); F64(up_chi2); I32(up_row); I32(up_n);
+  I32(mrg_best_b); I32(mrg_best_a); I32(mrg_next); I32(mrg_prev); I32(mrg_dir); F64(mrg_chi2_b);
+  I32(mrg_of_track); I32(mrg_seg_start); I32(mrg_seg_idx);
+  F64(mrg_par); F64(mrg_cov); F64(mrg_x_ref); F64(mrg_z_ref); F64(mrg_chi2); I32(mrg_n_fit); I32(mrg_ndf); I32(mrg_sector); I32(mrg_n_clusters);
   F32(up_dx); F32(up_ratio); F32(up_wy); F32(up_wz); F32(dn_dx); F32(dn_ratio); F32(dn_wy); F32(dn_wz);
 #undef I32
 #undef F32
@@ -805,6 +1038,27 @@ int orc_kf_fit(const void* params, int prec, int npt, const double* x, const dou
 
 // S8 on the tracks of the last orc_run (last_stage >= 5)
 void orc_protect(void* h, float road_y, float road_z) { reinterpret_cast<Oracle*>(h)->stage7_protect(road_y, road_z); }
+
+// S9 on the tracks and the refit of the last orc_run (last_stage >= 6)
+void orc_merge(void* h, int max_rows, int back_rows, float edge, float dz_win, float chi2_cut) {
+  Oracle* o = reinterpret_cast<Oracle*>(h);
+  const Oracle::MergeCuts mc{max_rows, back_rows, edge, dz_win, chi2_cut};
+  if (o->s4_prec == 64) o->stage9<double>(mc); else o->stage9<float>(mc);
+}
+
+// one rotation of DESIGN.md section 3.9.2 (for the pins): par / cov15 in place, returns the new x or NaN on failure
+double orc_kf_rotate(const void* params, int prec, double* par, double* cov15, double x, double sa, double ca) {
+  const Params& P = *reinterpret_cast<const Params*>(params);
+  const float kbf = -0.00299792458f * P.bz_tesla;
+  if (prec == 64) {
+    KF<double> k; load_kf(k, par, cov15, 0.0); double xn = 0;
+    if (!kf_rotate<double>(k, (double)kbf, x, sa, ca, (double)P.max_sinphi, &xn)) return NAN;
+    store_kf(k, par, cov15, nullptr); return xn;
+  }
+  KF<float> k; load_kf(k, par, cov15, 0.0); float xn = 0;
+  if (!kf_rotate<float>(k, kbf, (float)x, (float)sa, (float)ca, P.max_sinphi, &xn)) return NAN;
+  store_kf(k, par, cov15, nullptr); return (double)xn;
+}
 
 // S4 search of one state in row `row` of sector `sector`, on the grid of the last orc_run
 // (last_stage >= 1): sorted position of the nearest gated cluster or -1.  For the pins (tests/test_oracle_search.py).
