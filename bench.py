@@ -467,7 +467,16 @@ def run_ours(args):
     ev1.record(stream)
     torch.cuda.synchronize(dev)
     refit_ms = ev0.elapsed_time(ev1)
-    del fit_buf
+    # ---- the track merger of DESIGN.md section 3.9 (separate call after the refit): device time of the merge alone
+    mg_buf = trk.new_merged()
+    trk.merge_into(fit_buf, mg_buf)
+    ev0.record(stream)
+    trk.merge_into(fit_buf, mg_buf)
+    ev1.record(stream)
+    torch.cuda.synchronize(dev)
+    merge_ms = ev0.elapsed_time(ev1)
+    n_merged = int(mg_buf["n_merged"].item())
+    del mg_buf
     # ---- cluster protection for hit removal, strategy B (separate call), 1 cm road
     keep = trk.protect(out, 1.0, 1.0)
     ev0.record(stream)
@@ -476,7 +485,7 @@ def run_ours(args):
     torch.cuda.synchronize(dev)
     protect_ms = ev0.elapsed_time(ev1)
     kept_frac = float(keep[: tf.n].float().mean().item())
-    del keep
+    del keep, fit_buf
 
     # ---- end to end through the host entry points (pinned host buffers in and out).  Time frames arrive one after the
     # other, so the pipelined begin/end pair is the call a user makes: every step still does the H2D
@@ -553,6 +562,8 @@ def run_ours(args):
         "parity_before_timing": parity,
         "refit": {"what": "tpc_tracker_refit (separate call, not in the step): all tracks refitted over their owned clusters",
                   "ms": refit_ms},
+        "merge": {"what": "tpc_tracker_merge (separate call after the refit, not in the step): segments joined across sector "
+                          "borders and long holes, upward + merged downward refit", "ms": merge_ms, "n_merged": n_merged},
         "protect": {"what": "tpc_tracker_protect (separate call, not in the step): strategy-B keep flag per cluster, 1 cm road",
                     "ms": protect_ms, "kept_fraction": kept_frac},
         "roofline": roofline,

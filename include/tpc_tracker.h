@@ -186,7 +186,21 @@ enum tpc_stage_array {
   TPC_VIEW_T_ZREF = 22,     /* float [n_seeds] */
   TPC_VIEW_TRACKLET_OF_SEED = 23, /* int32 [n_seeds] rank among kept tracklets or -1 (S5) */
   TPC_VIEW_OWNED = 24,      /* int32 [n_seeds] clusters owned (S5) */
-  TPC_VIEW_COUNT_ = 25
+  /* S7 / S9 (valid after tpc_tracker_refit / tpc_tracker_merge; per track) */
+  TPC_VIEW_FIT_ROW = 25,    /* int32 [n_tracks] row of the state of the downward refit */
+  TPC_VIEW_UP_PAR = 26,     /* float [5][max_tracks] state at the outer end (upward refit) */
+  TPC_VIEW_UP_COV = 27,     /* float [15][max_tracks] */
+  TPC_VIEW_UP_X = 28,       /* float [n_tracks] */
+  TPC_VIEW_UP_ZREF = 29,    /* float [n_tracks] */
+  TPC_VIEW_UP_ROW = 30,     /* int32 [n_tracks] */
+  TPC_VIEW_UP_N = 31,       /* int32 [n_tracks] */
+  TPC_VIEW_MRG_BEST_B = 32, /* int32 [n_tracks] best partner of the outer end or -1 (3.9.5) */
+  TPC_VIEW_MRG_BEST_A = 33, /* uint64 [n_tracks] (ordered key of chi2 << 32) | best partner of the inner end; all ones = none */
+  TPC_VIEW_MRG_CHI_B = 34,  /* float [n_tracks] chi2 of best_b or -1 */
+  TPC_VIEW_MRG_NEXT = 35,   /* int32 [n_tracks] link to the next segment outwards or -1 (3.9.6) */
+  TPC_VIEW_MRG_PREV = 36,   /* int32 [n_tracks] */
+  TPC_VIEW_MRG_DIR = 37,    /* int32 [n_tracks] 0 same sector, +-1 the neighbour the link goes to */
+  TPC_VIEW_COUNT_ = 38
 };
 
 typedef struct {
@@ -254,6 +268,44 @@ typedef struct {
  * `cuda_stream`, which must be ordered after that call; does not synchronise; entries [0, n_tracks) are written.
  * Not part of tpc_track_timeframe (and not of the timed hot path).  CAPACITY if out->max_tracks exceeds the tracker's. */
 TPC_API int tpc_tracker_refit(tpc_tracker_t* t, const tpc_fit_t* out, void* cuda_stream);
+
+/* Cuts of the track merger. */
+typedef struct {
+  int32_t max_rows;   /* a continuation starts at most this many rows above the outer end (30) */
+  int32_t back_rows;  /* ... and, in a neighbouring sector, at most this many rows below it (1) */
+  float edge;         /* cm: a neighbour is tried only if the outer end lies within `edge` of the sector boundary (6) */
+  float dz_win;       /* cm: |z_in(B) - z_out(A)| window of the candidates (50); > 0 */
+  float chi2_cut;     /* candidates need chi2 <= chi2_cut over the five parameters (100) */
+} tpc_merge_cuts_t;
+
+/* Merged tracks (DEVICE pointers, caller-allocated for max_tracks entries each; layouts as in tpc_tracks_t).
+ * Tracks = the segments found by tpc_track_timeframe; a merged track is a chain of them, inner to outer. */
+typedef struct {
+  int64_t max_tracks;
+  int32_t* n_merged;         /* [1] */
+  int32_t* merged_of_track;  /* [max_tracks] merged id of every track */
+  int32_t* seg_start;        /* [max_tracks+1] CSR merged track -> its tracks */
+  int32_t* seg_idx;          /* [max_tracks] track ids, inner to outer */
+  float* par;                /* [5][max_tracks] merged refit, state at x_ref in the frame of `sector` */
+  float* cov;                /* [15][max_tracks] */
+  float* x_ref;              /* [max_tracks] */
+  float* z_ref;              /* [max_tracks] z of the outermost cluster: absolute z = par[1] + z_ref */
+  float* chi2;               /* [max_tracks] */
+  int32_t* ndf;              /* [max_tracks] 2*n_fit - 5 */
+  int32_t* n_fit;            /* [max_tracks] clusters that entered the merged fit */
+  int32_t* sector;           /* [max_tracks] sector whose frame the state is given in (the innermost one reached) */
+  int32_t* n_clusters;       /* [max_tracks] clusters of all segments */
+} tpc_merged_t;
+
+/* Track merger (the second slice of "Track Fit"): joins the tracks of the
+ * LAST tpc_track_timeframe call on this handle that continue each other - across a sector border or across a hole of
+ * more than max_gap rows - and refits every merged track over all its clusters (upward pass for the outer-end states,
+ * downward pass through all segments with the frame turned at sector changes).  `fit` is the output of the
+ * tpc_tracker_refit call that followed that tpc_track_timeframe (DEVICE; its residual fields are not used).  Enqueued on
+ * `cuda_stream`, which must be ordered after both; does not synchronise; entries [0, n_merged) / [0, n_tracks) are written.
+ * INVALID_ARG for null pointers or cuts out of range, CAPACITY if a max_tracks exceeds the tracker's. */
+TPC_API int tpc_tracker_merge(tpc_tracker_t* t, const tpc_fit_t* fit, const tpc_merge_cuts_t* cuts, const tpc_merged_t* out,
+                              void* cuda_stream);
 
 /* Cluster protection for hit removal, "strategy B", for the LAST
  * tpc_track_timeframe call on this handle: keep[i] = 1 iff input cluster i is attached to a track or lies, in its own

@@ -53,6 +53,22 @@ class tpc_fit_t(C.Structure):
                                                                        "trk_cl_start", "res_y", "res_z")]
 
 
+class tpc_merge_cuts_t(C.Structure):
+    _fields_ = [("max_rows", C.c_int32), ("back_rows", C.c_int32), ("edge", C.c_float), ("dz_win", C.c_float),
+                ("chi2_cut", C.c_float)]
+
+
+_MERGED_FIELDS = ["n_merged", "merged_of_track", "seg_start", "seg_idx", "par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit",
+                  "sector", "n_clusters"]
+
+
+class tpc_merged_t(C.Structure):
+    _fields_ = [("max_tracks", C.c_int64)] + [(f, C.c_void_p) for f in _MERGED_FIELDS]
+
+
+MERGE_CUTS = dict(max_rows=30, back_rows=1, edge=6.0, dz_win=50.0, chi2_cut=100.0)
+
+
 class tpc_counters_t(C.Structure):
     _fields_ = [("n_clusters", C.c_int64), ("n_bins", C.c_int64), ("n_seeds", C.c_int64), ("n_tracklets", C.c_int64),
                 ("n_tracks", C.c_int64), ("n_track_clusters", C.c_int64), ("n_linked", C.c_int64),
@@ -67,13 +83,15 @@ VIEWS = {name: i for i, name in enumerate([
     "perm", "yz", "srow", "bin_start", "row_start", "bin_base", "zmin", "zmax", "nz",
     "link_up_raw", "link_dn_raw", "link_up", "link_dn", "seed_head", "seed_len",
     "t_hit", "t_first_row", "t_last_row", "t_n_hits", "t_par", "t_cov", "t_chi2", "t_zref",
-    "tracklet_of_seed", "k_owned"])}
+    "tracklet_of_seed", "k_owned",
+    "fit_row", "up_par", "up_cov", "up_x", "up_zref", "up_row", "up_n",
+    "mrg_best_b", "mrg_best_a", "mrg_chi_b", "mrg_next", "mrg_prev", "mrg_dir"])}
 
 STATUS_BITS = {1: "BAD_CLUSTER", 2: "BINS_OVERFLOW", 4: "SEEDS_OVERFLOW", 8: "TRACKS_OVERFLOW", 16: "CHAIN_CYCLE"}
 
 EXPORTS = [
     "tpc_tracker_workspace_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
-    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit", "tpc_tracker_protect",
+    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit", "tpc_tracker_merge", "tpc_tracker_protect",
     "tpc_tracker_counters", "tpc_tracker_enable_stage_timing", "tpc_tracker_stage_ms", "tpc_tracker_stage_view",
     "tpc_tracker_launches_per_call", "tpc_tracker_destroy", "tpc_error_string",
 ]
@@ -116,6 +134,8 @@ def load_library(build: bool = True) -> C.CDLL:
     lib.tpc_track_timeframe_host_end.argtypes = [C.c_void_p, P(tpc_tracks_t), C.c_int32]
     lib.tpc_tracker_refit.restype = C.c_int
     lib.tpc_tracker_refit.argtypes = [C.c_void_p, P(tpc_fit_t), C.c_void_p]
+    lib.tpc_tracker_merge.restype = C.c_int
+    lib.tpc_tracker_merge.argtypes = [C.c_void_p, P(tpc_fit_t), P(tpc_merge_cuts_t), P(tpc_merged_t), C.c_void_p]
     lib.tpc_tracker_protect.restype = C.c_int
     lib.tpc_tracker_protect.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
     lib.tpc_tracker_counters.restype = C.c_int
@@ -329,6 +349,44 @@ class Tracker:
                     z_ref=out["z_ref"][:T].copy(), chi2=out["chi2"][:T].copy(), ndf=out["ndf"][:T].copy(),
                     n_fit=out["n_fit"][:T].copy())
 
+    def new_merged(self) -> dict:
+        """Device buffers for tpc_tracker_merge (layouts as in tpc_merged_t)."""
+        mt, dev = self.caps[3], self.device
+        f32 = lambda *s: torch.empty(*s, dtype=torch.float32, device=dev)   # noqa: E731
+        i32 = lambda *s: torch.zeros(*s, dtype=torch.int32, device=dev)     # noqa: E731
+        return dict(n_merged=i32(1), merged_of_track=i32(mt), seg_start=i32(mt + 1), seg_idx=i32(mt), par=f32(5, mt),
+                    cov=f32(15, mt), x_ref=f32(mt), z_ref=f32(mt), chi2=f32(mt), ndf=i32(mt), n_fit=i32(mt), sector=i32(mt),
+                    n_clusters=i32(mt))
+
+    def merge_into(self, fit: dict, merged: dict, cuts: dict | None = None, stream=None):
+        """Enqueues tpc_tracker_merge for the tracks of the last track_timeframe call, whose refit (refit_into) is `fit`
+        (does not synchronise)."""
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        f = tpc_fit_t()
+        f.max_tracks = self.caps[3]
+        for k in ("par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit"):
+            setattr(f, k, fit[k].data_ptr())
+        kw = dict(MERGE_CUTS); kw.update(cuts or {})
+        c = tpc_merge_cuts_t(int(kw["max_rows"]), int(kw["back_rows"]), float(kw["edge"]), float(kw["dz_win"]), float(kw["chi2_cut"]))
+        m = tpc_merged_t()
+        m.max_tracks = self.caps[3]
+        for k in _MERGED_FIELDS:
+            setattr(m, k, merged[k].data_ptr())
+        _check(self.lib, self.lib.tpc_tracker_merge(self._h, C.byref(f), C.byref(c), C.byref(m), C.c_void_p(st.cuda_stream)),
+               "tpc_tracker_merge")
+
+    def merge(self, n_tracks: int, cuts: dict | None = None) -> dict:
+        """Convenience: refit + merge + host copies trimmed to the tracks / merged tracks found."""
+        fit = self.new_fit(); mg = self.new_merged()
+        self.refit_into(fit)
+        self.merge_into(fit, mg, cuts)
+        torch.cuda.synchronize(self.device)
+        T = int(n_tracks); M = int(mg["n_merged"].item())
+        h = {k: v.cpu().numpy() for k, v in mg.items()}
+        return dict(n_merged=M, merged_of_track=h["merged_of_track"][:T].copy(), seg_start=h["seg_start"][:M + 1].copy(),
+                    seg_idx=h["seg_idx"][:T].copy(), par=h["par"][:, :M].T.copy(), cov=h["cov"][:, :M].T.copy(),
+                    **{k: h[k][:M].copy() for k in ("x_ref", "z_ref", "chi2", "ndf", "n_fit", "sector", "n_clusters")})
+
     def protect(self, out: Tracks, road_y: float, road_z: float, keep=None, stream=None):
         """tpc_tracker_protect for the last track_timeframe call (whose outputs are `out`); returns the uint8 device
         tensor keep[n] (enqueued, not synchronised)."""
@@ -359,7 +417,7 @@ class Tracker:
         """Host copy of one workspace array (debug / parity tests)."""
         v = tpc_stage_view_t()
         _check(self.lib, self.lib.tpc_tracker_stage_view(self._h, VIEWS[name], C.byref(v)), "tpc_tracker_stage_view")
-        dt = {(4, 0): np.int32, (4, 1): np.float32, (2, 0): np.uint16}[(v.elem_bytes, v.is_float)]
+        dt = {(4, 0): np.int32, (4, 1): np.float32, (2, 0): np.uint16, (8, 0): np.uint64}[(v.elem_bytes, v.is_float)]
         out = np.empty(v.n, dtype=dt)
         if v.n:
             # plain byte copy device -> host of a workspace slice

@@ -79,8 +79,12 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   c.rec = cv.take<float4>(N);
   c.bins = cv.take<int>(NB + 2 + 8);
   c.perm = cv.take<int>(N); c.yz = cv.take<float2>(N); c.srow = cv.take<uint16_t>(N);
+  const size_t T = (size_t)t->max_tracks;
+  c.max_merge_bins = 1 << 18;                       // (sector, z) bins of the merger's inner ends (S9)
   size_t max_scan = N > NB + 2 ? N : NB + 2;
   if (K > max_scan) max_scan = K;
+  if (T > max_scan) max_scan = T;
+  if ((size_t)c.max_merge_bins + 2 > max_scan) max_scan = (size_t)c.max_merge_bins + 2;
   c.tile_sums = cv.take<int>(max_scan / kScanTile + 2);
   // S1's second record buffer and the four link arrays of S2/S3 are never live together: one 16 N byte slice serves both
   c.rec2 = cv.take<float4>(N);
@@ -101,8 +105,21 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   c.track_seed = cv.take<int>(K);
   c.mask_words = (R + 31) / 32;
   c.own_mask = cv.take<unsigned>(K * (size_t)c.mask_words);
+  // S7 / S9: per track
+  c.fit_row = cv.take<int>(T);
+  c.up_par = cv.take<float>(5 * T); c.up_cov = cv.take<float>(15 * T); c.up_chi2 = cv.take<float>(T);
+  c.up_x = cv.take<float>(T); c.up_zref = cv.take<float>(T); c.up_row = cv.take<int>(T); c.up_n = cv.take<int>(T);
+  c.m_sector = cv.take<int>(T); c.m_zin = cv.take<float>(T); c.m_zout = cv.take<float>(T);
+  c.m_bin_base = cv.take<int>(S + 1); c.m_nzb = cv.take<int>(S);
+  c.m_bin_start = cv.take<int>((size_t)c.max_merge_bins + 2); c.m_bin_fill = cv.take<int>((size_t)c.max_merge_bins);
+  c.m_bin_of = cv.take<int>(T); c.m_rec = cv.take<float4>(T); c.m_srec = cv.take<float4>(T);
+  c.m_best_b = cv.take<int>(T); c.m_chi_b = cv.take<float>(T); c.m_dir_b = cv.take<int>(T);
+  c.m_best_a = cv.take<unsigned long long>(T);
+  c.m_next = cv.take<int>(T); c.m_prev = cv.take<int>(T); c.m_dir = cv.take<int>(T);
+  c.m_head_scan = cv.take<int>(T); c.m_seg_scan = cv.take<int>(T); c.m_head_of = cv.take<int>(T);
+  c.mcnt = cv.take<MergeCounters>(1);
   for (int k = 0; k < t->host_io; ++k) {
-    const size_t T = (size_t)t->max_tracks, TC = (size_t)t->max_track_clusters;
+    const size_t TC = (size_t)t->max_track_clusters;
     tpc_tracker::Slot& sl = t->slot[k];
     sl.sector = cv.take<uint8_t>(N); sl.row = cv.take<uint8_t>(N);
     sl.y = cv.take<float>(N); sl.z = cv.take<float>(N);
@@ -417,6 +434,35 @@ int tpc_tracker_refit(tpc_tracker_t* t, const tpc_fit_t* out, void* cuda_stream)
   return launch_refit(t->ctx, o, st) ? TPC_ERR_CUDA : TPC_OK;
 }
 
+int tpc_tracker_merge(tpc_tracker_t* t, const tpc_fit_t* fit, const tpc_merge_cuts_t* cuts, const tpc_merged_t* out,
+                      void* cuda_stream) {
+  if (!t || !fit || !cuts || !out) return TPC_ERR_INVALID_ARG;
+  if (!fit->par || !fit->cov || !fit->x_ref || !fit->z_ref || !fit->n_fit) return TPC_ERR_INVALID_ARG;
+  if (!out->n_merged || !out->merged_of_track || !out->seg_start || !out->seg_idx || !out->par || !out->cov || !out->x_ref ||
+      !out->z_ref || !out->chi2 || !out->ndf || !out->n_fit || !out->sector || !out->n_clusters)
+    return TPC_ERR_INVALID_ARG;
+  if (cuts->max_rows < 0 || cuts->back_rows < 0 || !(cuts->edge >= 0.f) || !(cuts->dz_win > 0.f) || !(cuts->dz_win < INFINITY) ||
+      !(cuts->chi2_cut >= 0.f))
+    return TPC_ERR_INVALID_ARG;
+  if (fit->max_tracks < 1 || fit->max_tracks > t->max_tracks || out->max_tracks < 1 || out->max_tracks > t->max_tracks)
+    return TPC_ERR_CAPACITY;
+  FitPtrs f{};
+  f.par = fit->par; f.cov = fit->cov; f.x_ref = fit->x_ref; f.z_ref = fit->z_ref; f.chi2 = fit->chi2; f.ndf = fit->ndf;
+  f.n_fit = fit->n_fit; f.max_tracks = (int)fit->max_tracks;
+  MergePtrs o{};
+  o.max_rows = cuts->max_rows; o.back_rows = cuts->back_rows; o.edge = cuts->edge; o.dz_win = cuts->dz_win; o.chi2_cut = cuts->chi2_cut;
+  // sine and cosine of the sector angle from tan_half_sector alone, fp32, one rounding per operation
+  const float th = t->params.tan_half_sector;
+  const float den = 1.0f + th * th;
+  o.sin_a = (2.0f * th) / den; o.cos_a = (1.0f - th * th) / den;
+  o.n_merged = out->n_merged; o.merged_of_track = out->merged_of_track; o.seg_start = out->seg_start; o.seg_idx = out->seg_idx;
+  o.par = out->par; o.cov = out->cov; o.x_ref = out->x_ref; o.z_ref = out->z_ref; o.chi2 = out->chi2; o.ndf = out->ndf;
+  o.n_fit = out->n_fit; o.sector = out->sector; o.n_clusters = out->n_clusters; o.max_tracks = (int)out->max_tracks;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  t->last_stream = st;
+  return launch_merge(t->ctx, f, o, st) ? TPC_ERR_CUDA : TPC_OK;
+}
+
 int tpc_tracker_protect(tpc_tracker_t* t, const int32_t* cluster_track, float road_y, float road_z, uint8_t* keep,
                         void* cuda_stream) {
   if (!t || !keep || !cluster_track || !(road_y >= 0.f) || !(road_z >= 0.f)) return TPC_ERR_INVALID_ARG;
@@ -486,6 +532,19 @@ int tpc_tracker_stage_view(tpc_tracker_t* t, int32_t which, tpc_stage_view_t* ou
     case TPC_VIEW_T_ZREF: set(c.t_zref, ns, 4, 1); break;
     case TPC_VIEW_TRACKLET_OF_SEED: set(c.tracklet_of_seed, ns, 4, 0); break;
     case TPC_VIEW_OWNED: set(c.k_owned, ns, 4, 0); break;
+    case TPC_VIEW_FIT_ROW: set(c.fit_row, k.n_tracks, 4, 0); break;
+    case TPC_VIEW_UP_PAR: set(c.up_par, 5 * (int64_t)c.max_tracks, 4, 1); break;
+    case TPC_VIEW_UP_COV: set(c.up_cov, 15 * (int64_t)c.max_tracks, 4, 1); break;
+    case TPC_VIEW_UP_X: set(c.up_x, k.n_tracks, 4, 1); break;
+    case TPC_VIEW_UP_ZREF: set(c.up_zref, k.n_tracks, 4, 1); break;
+    case TPC_VIEW_UP_ROW: set(c.up_row, k.n_tracks, 4, 0); break;
+    case TPC_VIEW_UP_N: set(c.up_n, k.n_tracks, 4, 0); break;
+    case TPC_VIEW_MRG_BEST_B: set(c.m_best_b, k.n_tracks, 4, 0); break;
+    case TPC_VIEW_MRG_BEST_A: set(c.m_best_a, k.n_tracks, 8, 0); break;
+    case TPC_VIEW_MRG_CHI_B: set(c.m_chi_b, k.n_tracks, 4, 1); break;
+    case TPC_VIEW_MRG_NEXT: set(c.m_next, k.n_tracks, 4, 0); break;
+    case TPC_VIEW_MRG_PREV: set(c.m_prev, k.n_tracks, 4, 0); break;
+    case TPC_VIEW_MRG_DIR: set(c.m_dir, k.n_tracks, 4, 0); break;
     default: return TPC_ERR_INVALID_ARG;
   }
   return TPC_OK;

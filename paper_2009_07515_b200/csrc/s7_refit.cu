@@ -89,6 +89,7 @@ __global__ void __launch_bounds__(kThreads) k_refit(Ctx c, FitPtrs o) {
     o.z_ref[id] = zref;
     o.n_fit[id] = nfit;
     o.ndf[id] = nfit ? 2 * nfit - 5 : 0;
+    c.fit_row[id] = nfit ? cur : 0;                     // for the merger (S9)
   }
 }
 

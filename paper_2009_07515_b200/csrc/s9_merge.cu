@@ -1,0 +1,456 @@
+// S9 - track merger (the second slice of "Track Fit"): the segments a
+// physical track was found in - one per sector it crosses, one per stretch between holes longer than max_gap - are
+// joined by comparing the state at the outer end of one with the state at the inner end of the other, and every
+// joined track is refitted over all its clusters.  A separate call (tpc_tracker_merge) after tpc_track_timeframe and
+// tpc_tracker_refit; it reads what those left in the workspace and the refit's output.
+//
+//   k_merge_tables   one thread: a z grid per sector for the inner ends (bin width = dz_win, doubled until the bins fit)
+//   k_refit_up       thread per track: upward refit (3.9.1) -> state at the outer end; z of both ends, sector; counts the
+//                    inner end into its (sector, z) bin
+//   scan + k_merge_fill   counting sort of 16-byte inner-end records by (sector, z bin): "extensive use of sort" - here
+//                    a hand-written counting sort (no Thrust / CUB), the window of 3.9.3 is then a contiguous run of bins
+//   k_merge_match    thread per outer end: candidates of 3.9.3 from the bins around z_out, score 3.9.4 (rotation +
+//                    helix step + chi2), best partner of the outer end in registers (ties -> lowest id), best partner of
+//                    every inner end by a 64-bit atomicMin of (chi2 bits, id) - both independent of the visiting order
+//   k_merge_link     mutual best -> links (3.9.5);  flags + scan -> merged ids (3.9.6)
+//   k_chain_len / scan / k_chain_fill   chains followed from their heads: merged_of_track, CSR merged -> segments
+//   k_refit_merged   thread per merged track: downward refit through all segments, the frame turned at sector changes (3.9.7)
+//
+// Arithmetic: fp32, -fmad=false, the operations of DESIGN.md section 3.9 in the order written (the helix step and the
+// update are those of S4, kf.cuh); bit-identical to the oracle.
+#include "kf.cuh"
+#include "tpc_internal.cuh"
+
+namespace tpc {
+namespace {
+
+constexpr int kThreads = 128;
+
+// the state turned into the frame rotated by the angle with sine sa and cosine ca
+__device__ __forceinline__ bool kf_rotate(KF& k, float kb, float x, float sa, float ca, float max_sinphi, float* x_new) {
+  const float y = k.p[0], s = k.p[2], t = k.p[3], q = k.p[4];
+  if (!(fabsf(s) < max_sinphi)) return false;
+  const float c = sqrtf(1.0f - s * s);
+  const float s1 = s * ca - c * sa;
+  const float c1 = c * ca + s * sa;
+  if (!(fabsf(s1) < max_sinphi) || !(c1 > 0.0f)) return false;
+  const float xn = x * ca + y * sa;
+  const float yn = y * ca - x * sa;
+  const float j00 = c / c1;
+  const float j10 = ((0.0f - sa) * t) / c1;
+  const float j20 = (0.0f - kb * q) * sa;
+  const float j22 = c1 / c;
+  // M = J C: rows 3 and 4 of J are unit rows; M0 = j00 C0, M1 = j10 C0 + C1, M2 = j20 C0 + j22 C2
+  float m0[5], m1[5], m2[5];
+#pragma unroll
+  for (int l = 0; l < 5; ++l) {
+    m0[l] = j00 * k.c[CI(0, l)];
+    m1[l] = j10 * k.c[CI(0, l)] + k.c[CI(1, l)];
+    m2[l] = j20 * k.c[CI(0, l)] + j22 * k.c[CI(2, l)];
+  }
+  // C'[i][0] = M[i][0] j00;  C'[i][1] = M[i][0] j10 + M[i][1];  C'[i][2] = M[i][0] j20 + M[i][2] j22;  C'[i][3,4] = M[i][3,4]
+  float n[15];
+  n[CI(0, 0)] = m0[0] * j00;
+  n[CI(1, 0)] = m1[0] * j00;
+  n[CI(2, 0)] = m2[0] * j00;
+  n[CI(3, 0)] = k.c[CI(3, 0)] * j00;
+  n[CI(4, 0)] = k.c[CI(4, 0)] * j00;
+  n[CI(1, 1)] = m1[0] * j10 + m1[1];
+  n[CI(2, 1)] = m2[0] * j10 + m2[1];
+  n[CI(3, 1)] = k.c[CI(3, 0)] * j10 + k.c[CI(3, 1)];
+  n[CI(4, 1)] = k.c[CI(4, 0)] * j10 + k.c[CI(4, 1)];
+  n[CI(2, 2)] = m2[0] * j20 + m2[2] * j22;
+  n[CI(3, 2)] = k.c[CI(3, 0)] * j20 + k.c[CI(3, 2)] * j22;
+  n[CI(4, 2)] = k.c[CI(4, 0)] * j20 + k.c[CI(4, 2)] * j22;
+  n[CI(3, 3)] = k.c[CI(3, 3)];
+  n[CI(4, 3)] = k.c[CI(4, 3)];
+  n[CI(4, 4)] = k.c[CI(4, 4)];
+#pragma unroll
+  for (int i = 0; i < 15; ++i) k.c[i] = n[i];
+  k.p[0] = yn; k.p[2] = s1;
+  *x_new = xn;
+  return true;
+}
+
+// owned rows of a tracklet in ASCENDING order
+struct OwnedRowsUp {
+  const unsigned* mask;
+  int first, w, words;
+  unsigned m;
+  __device__ __forceinline__ OwnedRowsUp(const unsigned* mask_, int first_, int words_) : mask(mask_), first(first_), w(0), words(words_) {
+    m = mask[0];
+  }
+  __device__ __forceinline__ int next() {
+    while (m == 0) {
+      if (++w >= words) return -1;
+      m = mask[w];
+    }
+    const int bit = __ffs(m) - 1;
+    m &= m - 1;
+    return first + 32 * w + bit;
+  }
+};
+// ... and in DESCENDING order
+struct OwnedRowsDown {
+  const unsigned* mask;
+  int first, w;
+  unsigned m;
+  __device__ __forceinline__ OwnedRowsDown(const unsigned* mask_, int first_, int words) : mask(mask_), first(first_), w(words - 1) {
+    m = mask[w];
+  }
+  __device__ __forceinline__ int next() {
+    while (m == 0) {
+      if (--w < 0) return -1;
+      m = mask[w];
+    }
+    const int bit = 31 - __clz(m);
+    m &= ~(1u << bit);
+    return first + 32 * w + bit;
+  }
+};
+
+__device__ __forceinline__ int n_tracks_of(const Ctx& c, const MergePtrs& o) { return min(c.cnt->n_tracks, o.max_tracks); }
+
+// ---------------------------------------------------------------------------------- z grid of the inner ends
+__global__ void k_merge_tables(Ctx c, MergePtrs o) {
+  if (threadIdx.x || blockIdx.x) return;
+  MergeCounters& mc = *c.mcnt;
+  mc.n_merged = 0; mc.status = 0;
+  // bins a quarter of the window wide: a query reads 9-10 bins, 1.25 x the window instead of 3 x with bins of dz_win
+  float w = o.dz_win * 0.25f;
+  for (int it = 0; it < 64; ++it, w = w * 2.0f) {
+    const float inv_w = 1.0f / w;
+    long long acc = 0;
+    for (int s = 0; s < c.S; ++s) {
+      c.m_bin_base[s] = (int)acc;
+      int nzb = 0;
+      if (c.nz[s] > 0) {
+        const float rows = floorf((c.zmax[s] - c.zmin[s]) * inv_w);
+        nzb = rows < 1.0e9f ? (int)rows + 1 : 2000000000;
+      }
+      c.m_nzb[s] = nzb;
+      acc += nzb;
+      if (acc > c.max_merge_bins) break;
+    }
+    if (acc <= c.max_merge_bins) {
+      c.m_bin_base[c.S] = (int)acc;
+      mc.n_bins = (int)acc; mc.inv_w = inv_w;
+      return;
+    }
+  }
+  mc.n_bins = 0; mc.inv_w = 0.0f; mc.status = 1;      // cannot happen for finite z ranges: 2^64 * dz_win covers everything
+}
+
+__global__ void __launch_bounds__(kThreads) k_merge_clear(Ctx c, MergePtrs o) {
+  const int nb = c.mcnt->n_bins;
+  const int nt = n_tracks_of(c, o);
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i <= nb; i += gridDim.x * blockDim.x) c.m_bin_start[i] = 0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nt; i += gridDim.x * blockDim.x) {
+    c.m_best_b[i] = -1; c.m_chi_b[i] = -1.0f; c.m_dir_b[i] = 0;
+    c.m_best_a[i] = ~0ull;
+    c.m_next[i] = -1; c.m_prev[i] = -1; c.m_dir[i] = 0;
+  }
+}
+
+__device__ __forceinline__ int merge_bin(const Ctx& c, int s, float z, float inv_w) {
+  return c.m_bin_base[s] + floor_clamp((z - c.zmin[s]) * inv_w, c.m_nzb[s] - 1);
+}
+
+// ---------------------------------------------------------------------------------- 3.9.1 upward refit + end bookkeeping
+__global__ void __launch_bounds__(kThreads) k_refit_up(Ctx c, FitPtrs f, MergePtrs o) {
+  extern __shared__ float tx[];
+  for (int i = threadIdx.x; i < c.R; i += blockDim.x) tx[i] = c.rowtab[i].x;
+  __syncthreads();
+  if (c.cnt->status || c.mcnt->status) return;
+  const int nt = n_tracks_of(c, o), R = c.R;
+  const size_t mt = (size_t)c.max_tracks, ft = (size_t)f.max_tracks;
+  const float inv_w = c.mcnt->inv_w;
+  const float2* __restrict__ yz = c.yz;
+  for (int id = blockIdx.x * blockDim.x + threadIdx.x; id < nt; id += gridDim.x * blockDim.x) {
+    const int sd = c.track_seed[id];
+    const int* hit = c.t_hit + (size_t)sd * R;
+    const int first = c.t_first_row[sd], last = c.t_last_row[sd];
+    const int words = (last - first) / 32 + 1;
+    OwnedRowsUp rows(c.own_mask + (size_t)sd * c.mask_words, first, words);
+    const int r_bot = rows.next();
+    const int r_nxt = rows.next();
+    KF k;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) k.p[i] = 0.f;
+#pragma unroll
+    for (int i = 0; i < 15; ++i) k.c[i] = 0.f;
+    k.chi2 = 0.f;
+    int cur = max(r_bot, 0), nfit = 0, sector = 0;
+    float zref = 0.f;
+    if (r_bot >= 0) sector = c.srow[hit[r_bot]] >> 8;
+    if (r_bot >= 0 && r_nxt >= 0) {
+      const float2 pb = __ldg(yz + hit[r_bot]), pn = __ldg(yz + hit[r_nxt]);
+      zref = pb.y;
+      const float dx = tx[r_nxt] - tx[r_bot];
+      const float dy = pn.x - pb.x, dz = pn.y - pb.y;
+      const float dl = sqrtf(dx * dx + dy * dy);
+      k.p[0] = pb.x; k.p[1] = 0.0f; k.p[2] = dy / dl; k.p[3] = dz / dl; k.p[4] = f.par[4 * ft + id];
+      kf_reset_cov(k, c);
+      nfit = 1;
+      for (int r = r_nxt; r >= 0; r = rows.next()) {
+        if (!kf_propagate(k, c.kb, tx[r] - tx[cur], c.max_sinphi)) break;
+        const float2 v = __ldg(yz + hit[r]);
+        kf_update(k, v.x, v.y - zref, c.err_y2, c.err_z2);
+        cur = r; ++nfit;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 5; ++i) c.up_par[i * mt + id] = k.p[i];
+#pragma unroll
+    for (int i = 0; i < 15; ++i) c.up_cov[i * mt + id] = k.c[i];
+    c.up_chi2[id] = k.chi2;
+    c.up_x[id] = nfit ? tx[cur] : 0.f;
+    c.up_zref[id] = zref;
+    c.up_row[id] = nfit ? cur : 0;
+    c.up_n[id] = nfit;
+    c.m_sector[id] = sector;
+    const float z_in = f.z_ref[id] + f.par[1 * ft + id];
+    c.m_zin[id] = z_in;
+    c.m_zout[id] = zref + k.p[1];
+    // the inner end goes into its (sector, z) bin (every track: those that take no part are skipped when read)
+    const int b = merge_bin(c, sector, z_in, inv_w);
+    c.m_bin_of[id] = b;
+    // the record the candidate scan reads: z_in, the row of the inner state (-1: takes no part), the id
+    c.m_rec[id] = make_float4(z_in, __int_as_float(nfit >= 2 && f.n_fit[id] >= 2 ? c.fit_row[id] : -1), __int_as_float(id), 0.0f);
+    atomicAdd(c.m_bin_start + b + 1, 1);              // counts at b + 1: the inclusive scan leaves the CSR starts in place
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_merge_fill(Ctx c, MergePtrs o) {
+  if (c.cnt->status || c.mcnt->status) return;
+  const int nt = n_tracks_of(c, o);
+  for (int id = blockIdx.x * blockDim.x + threadIdx.x; id < nt; id += gridDim.x * blockDim.x) {
+    const int b = c.m_bin_of[id];
+    const int pos = c.m_bin_start[b] + atomicAdd(c.m_bin_fill + b, 1);
+    c.m_srec[pos] = c.m_rec[id];
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_merge_zero_fill(Ctx c) {
+  const int nb = c.mcnt->n_bins;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nb; i += gridDim.x * blockDim.x) c.m_bin_fill[i] = 0;
+}
+
+// ---------------------------------------------------------------------------------- 3.9.3 - 3.9.5 candidates, score, choice
+__global__ void __launch_bounds__(kThreads) k_merge_match(Ctx c, FitPtrs f, MergePtrs o) {
+  extern __shared__ float sm[];
+  float* tymax = sm;
+  for (int i = threadIdx.x; i < c.R; i += blockDim.x) tymax[i] = c.rowtab[i].ymax;
+  __syncthreads();
+  if (c.cnt->status || c.mcnt->status) return;
+  const int nt = n_tracks_of(c, o), n_az = c.S >> 1;
+  const size_t mt = (size_t)c.max_tracks, ft = (size_t)f.max_tracks;
+  const float inv_w = c.mcnt->inv_w;
+  for (int a = blockIdx.x * blockDim.x + threadIdx.x; a < nt; a += gridDim.x * blockDim.x) {
+    if (c.up_n[a] < 2 || f.n_fit[a] < 2) continue;
+    const int s_a = c.m_sector[a], r_a = c.up_row[a];
+    KF ka;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) ka.p[i] = c.up_par[i * mt + a];
+#pragma unroll
+    for (int i = 0; i < 15; ++i) ka.c[i] = c.up_cov[i * mt + a];
+    ka.chi2 = 0.f;
+    const float x_a = c.up_x[a], zref_a = c.up_zref[a], z_out = c.m_zout[a];
+    const float zlo = z_out - o.dz_win, zhi = z_out + o.dz_win;
+    float best = 0.f;
+    int bb = -1, bdir = 0;
+    for (int pass = 0; pass < 2; ++pass) {
+      int dir = 0, s_b = s_a;
+      if (pass == 1) {
+        if (!(fabsf(ka.p[0]) >= tymax[r_a] - o.edge)) continue;
+        dir = ka.p[0] >= 0.0f ? 1 : -1;
+        s_b = (s_a / n_az) * n_az + ((s_a % n_az) + dir + n_az) % n_az;
+        if (s_b == s_a) continue;
+      }
+      if (c.m_nzb[s_b] == 0) continue;
+      const int b0 = merge_bin(c, s_b, zlo, inv_w), b1 = merge_bin(c, s_b, zhi, inv_w);
+      const int j0 = c.m_bin_start[b0], j1 = c.m_bin_start[b1 + 1];
+      for (int j = j0; j < j1; ++j) {
+        const float4 rec = __ldg(c.m_srec + j);         // contiguous run of 16-byte records: no gather before the cheap cuts
+        const int b = __float_as_int(rec.z), r_b = __float_as_int(rec.y);
+        const float z_b = rec.x;
+        if (b == a || r_b < 0) continue;
+        if (!(z_b >= zlo && z_b <= zhi)) continue;
+        if (dir == 0 ? (r_b < r_a + 1 || r_b > r_a + o.max_rows) : (r_b < r_a - o.back_rows || r_b > r_a + o.max_rows)) continue;
+        KF k = ka;
+        float x = x_a;
+        if (dir != 0 && !kf_rotate(k, c.kb, x, dir > 0 ? o.sin_a : 0.0f - o.sin_a, o.cos_a, c.max_sinphi, &x)) continue;
+        if (!kf_propagate(k, c.kb, f.x_ref[b] - x, c.max_sinphi)) continue;
+        float d[5];
+        d[0] = f.par[0 * ft + b] - k.p[0];
+        d[1] = z_b - (zref_a + k.p[1]);
+        d[2] = f.par[2 * ft + b] - k.p[2];
+        d[3] = f.par[3 * ft + b] - k.p[3];
+        d[4] = f.par[4 * ft + b] - k.p[4];
+        float chi = 0.0f;
+#pragma unroll
+        for (int i = 0; i < 5; ++i) chi = chi + (d[i] * d[i]) / (k.c[CI(i, i)] + f.cov[(size_t)CI(i, i) * ft + b]);
+        if (!(chi <= o.chi2_cut)) continue;
+        if (bb < 0 || chi < best || (chi == best && b < bb)) { best = chi; bb = b; bdir = dir; }
+        // high word: order-preserving unsigned key of chi (fp32 variances can come out slightly negative, and then so
+        // does chi); low word = id -> ties go to the lowest a
+        const unsigned cb = __float_as_uint(chi);
+        const unsigned ck = (cb & 0x80000000u) ? ~cb : (cb | 0x80000000u);
+        atomicMin(c.m_best_a + b, ((unsigned long long)ck << 32) | (unsigned)a);
+      }
+    }
+    c.m_best_b[a] = bb; c.m_dir_b[a] = bdir; c.m_chi_b[a] = bb >= 0 ? best : -1.0f;
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_merge_link(Ctx c, MergePtrs o) {
+  if (c.cnt->status || c.mcnt->status) return;
+  const int nt = n_tracks_of(c, o);
+  for (int a = blockIdx.x * blockDim.x + threadIdx.x; a < nt; a += gridDim.x * blockDim.x) {
+    const int b = c.m_best_b[a];
+    if (b >= 0 && (int)(c.m_best_a[b] & 0xFFFFFFFFull) == a) { c.m_next[a] = b; c.m_prev[b] = a; c.m_dir[a] = c.m_dir_b[a]; }
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_merge_heads(Ctx c, MergePtrs o) {
+  const int nt = (c.cnt->status || c.mcnt->status) ? 0 : n_tracks_of(c, o);
+  if (blockIdx.x == 0 && threadIdx.x == 0) c.mcnt->n_scan = nt;
+  for (int a = blockIdx.x * blockDim.x + threadIdx.x; a < nt; a += gridDim.x * blockDim.x) c.m_head_scan[a] = c.m_prev[a] < 0;
+}
+
+// merged id of a head = its rank; the chain is followed once for the length and the members' ids ...
+__global__ void __launch_bounds__(kThreads) k_chain_len(Ctx c, MergePtrs o) {
+  const int nt = c.mcnt->n_scan;
+  if (blockIdx.x == 0 && threadIdx.x == 0) { *o.n_merged = nt ? c.m_head_scan[nt - 1] : 0; c.mcnt->n_merged = nt ? c.m_head_scan[nt - 1] : 0; }
+  for (int h = blockIdx.x * blockDim.x + threadIdx.x; h < nt; h += gridDim.x * blockDim.x) {
+    if (c.m_prev[h] >= 0) continue;
+    const int m = c.m_head_scan[h] - 1;
+    int len = 0;
+    for (int k = h; k >= 0 && len < nt; k = c.m_next[k], ++len) o.merged_of_track[k] = m;
+    c.m_seg_scan[m] = len;
+    c.m_head_of[m] = h;
+  }
+}
+
+// ... and once more to write the CSR (seg_scan is now the inclusive scan of the lengths)
+__global__ void __launch_bounds__(kThreads) k_chain_fill(Ctx c, MergePtrs o) {
+  const int nm = c.mcnt->n_merged, nt = c.mcnt->n_scan;
+  if (blockIdx.x == 0 && threadIdx.x == 0) o.seg_start[0] = 0;
+  for (int m = blockIdx.x * blockDim.x + threadIdx.x; m < nm; m += gridDim.x * blockDim.x) {
+    const int end = c.m_seg_scan[m];
+    o.seg_start[m + 1] = end;
+    int pos = m ? c.m_seg_scan[m - 1] : 0;
+    int len = 0;
+    for (int k = c.m_head_of[m]; k >= 0 && len < nt; k = c.m_next[k], ++len) o.seg_idx[pos++] = k;
+  }
+}
+
+// ---------------------------------------------------------------------------------- 3.9.7 merged refit
+__global__ void __launch_bounds__(kThreads) k_refit_merged(Ctx c, MergePtrs o) {
+  extern __shared__ float tx[];
+  for (int i = threadIdx.x; i < c.R; i += blockDim.x) tx[i] = c.rowtab[i].x;
+  __syncthreads();
+  const int nm = c.mcnt->n_merged, R = c.R;
+  const size_t mo = (size_t)o.max_tracks;
+  const float2* __restrict__ yz = c.yz;
+  for (int m = blockIdx.x * blockDim.x + threadIdx.x; m < nm; m += gridDim.x * blockDim.x) {
+    const int s0 = o.seg_start[m], s1 = o.seg_start[m + 1];
+    KF k;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) k.p[i] = 0.f;
+#pragma unroll
+    for (int i = 0; i < 15; ++i) k.c[i] = 0.f;
+    k.chi2 = 0.f;
+    float x = 0.f, zref = 0.f;
+    int nfit = 0, ncl = 0, sector = 0;
+    bool ok = true, started = false;
+    for (int q = s1 - 1; q >= s0; --q) {
+      const int seg = o.seg_idx[q];
+      const int sd = c.track_seed[seg];
+      ncl += c.k_owned[sd];
+      if (!ok) continue;                                // only the cluster count goes on
+      const int* hit = c.t_hit + (size_t)sd * R;
+      const int first = c.t_first_row[sd], last = c.t_last_row[sd];
+      OwnedRowsDown rows(c.own_mask + (size_t)sd * c.mask_words, first, (last - first) / 32 + 1);
+      int r = rows.next();
+      if (q == s1 - 1) {
+        OwnedRowsDown peek = rows;
+        const int r_nxt = peek.next();
+        if (r < 0 || r_nxt < 0) { ok = false; continue; }
+        sector = c.m_sector[seg];
+        const float2 pt = __ldg(yz + hit[r]), pn = __ldg(yz + hit[r_nxt]);
+        zref = pt.y;
+        const float dx = tx[r] - tx[r_nxt];
+        const float dy = pt.x - pn.x, dz = pt.y - pn.y;
+        const float dl = sqrtf(dx * dx + dy * dy);
+        k.p[0] = pt.x; k.p[1] = 0.0f; k.p[2] = dy / dl; k.p[3] = dz / dl; k.p[4] = c.t_par[(size_t)sd * 5 + 4];
+        kf_reset_cov(k, c);
+        x = tx[r]; nfit = 1; started = true;
+        r = rows.next();
+      } else {
+        const int dir = c.m_dir[seg];
+        if (dir != 0) {
+          const float sd_ = dir > 0 ? o.sin_a : 0.0f - o.sin_a;
+          const float2 pc = __ldg(yz + hit[r]);
+          const float xt = tx[r] * o.cos_a + pc.x * sd_;
+          if (!kf_propagate(k, c.kb, xt - x, c.max_sinphi)) { ok = false; continue; }
+          x = xt;
+          if (!kf_rotate(k, c.kb, x, 0.0f - sd_, o.cos_a, c.max_sinphi, &x)) { ok = false; continue; }
+        }
+        sector = c.m_sector[seg];
+      }
+      for (; r >= 0; r = rows.next()) {
+        if (!kf_propagate(k, c.kb, tx[r] - x, c.max_sinphi)) { ok = false; break; }
+        x = tx[r];
+        const float2 v = __ldg(yz + hit[r]);
+        kf_update(k, v.x, v.y - zref, c.err_y2, c.err_z2);
+        ++nfit;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 5; ++i) o.par[i * mo + m] = k.p[i];
+#pragma unroll
+    for (int i = 0; i < 15; ++i) o.cov[i * mo + m] = k.c[i];
+    o.chi2[m] = k.chi2;
+    o.x_ref[m] = started ? x : 0.f;
+    o.z_ref[m] = zref;
+    o.n_fit[m] = nfit;
+    o.ndf[m] = nfit ? 2 * nfit - 5 : 0;
+    o.sector[m] = sector;
+    o.n_clusters[m] = ncl;
+  }
+}
+
+unsigned grid_for(long long n, const Ctx& c, int per_sm) {
+  long long g = (n + kThreads - 1) / kThreads;
+  const long long cap = (long long)c.n_sms * per_sm;
+  if (g > cap) g = cap;
+  if (g < 1) g = 1;
+  return (unsigned)g;
+}
+
+}  // namespace
+
+int launches_merge() { return 12 + 6; }
+int launch_merge(const Ctx& c, const FitPtrs& f, const MergePtrs& o, cudaStream_t st) {
+  const unsigned gt = grid_for(c.max_tracks, c, 64), gb = grid_for(c.max_merge_bins, c, 16);
+  const size_t sh = c.R * sizeof(float);
+  k_merge_tables<<<1, 32, 0, st>>>(c, o);
+  k_merge_clear<<<gt > gb ? gt : gb, kThreads, 0, st>>>(c, o);
+  k_refit_up<<<gt, kThreads, sh, st>>>(c, f, o);
+  // CSR starts of the (sector, z) bins: inclusive scan of the counts written at b + 1 (entry 0 stays 0)
+  if (launch_scan_inclusive(c.m_bin_start, &c.mcnt->n_bins, 1, (long long)c.max_merge_bins + 1, c.tile_sums, nullptr, c.n_sms, st)) return -1;
+  k_merge_zero_fill<<<gb, kThreads, 0, st>>>(c);
+  k_merge_fill<<<gt, kThreads, 0, st>>>(c, o);
+  k_merge_match<<<gt, kThreads, sh, st>>>(c, f, o);
+  k_merge_link<<<gt, kThreads, 0, st>>>(c, o);
+  k_merge_heads<<<gt, kThreads, 0, st>>>(c, o);
+  if (launch_scan_inclusive(c.m_head_scan, &c.mcnt->n_scan, 0, c.max_tracks, c.tile_sums, nullptr, c.n_sms, st)) return -1;
+  k_chain_len<<<gt, kThreads, 0, st>>>(c, o);
+  if (launch_scan_inclusive(c.m_seg_scan, &c.mcnt->n_merged, 0, c.max_tracks, c.tile_sums, nullptr, c.n_sms, st)) return -1;
+  k_chain_fill<<<gt, kThreads, 0, st>>>(c, o);
+  k_refit_merged<<<gt, kThreads, sh, st>>>(c, o);
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+}  // namespace tpc

@@ -43,6 +43,16 @@ struct Counters {
   int pad[1];
 };
 
+// Device counter block of the merger (S9).
+struct MergeCounters {
+  int n_bins;             // (sector, z) bins of the inner ends
+  float inv_w;            // 1 / bin width
+  int n_merged;
+  int n_scan;             // n_tracks of the call (device-resident scan length)
+  int status;             // != 0: the z grid could not be built
+  int pad[3];
+};
+
 // Everything a kernel needs, passed by value (a few hundred bytes).
 struct Ctx {
   // geometry / cuts
@@ -88,6 +98,18 @@ struct Ctx {
   int* surv_scan; int* owned_scan;    // [max_seeds] inclusive scans
   int* track_seed;                    // [max_seeds] seed of track id (S5 k_write; read by k_params and the refit)
   unsigned* own_mask; int mask_words; // [max_seeds][mask_words] bit k of word w: row first_row + 32 w + k is owned
+  // S7 / S9 (per track, [max_tracks]; SoA [component][max_tracks] for par / cov)
+  int* fit_row;                       // row of the state the downward refit (S7) ended on
+  float* up_par; float* up_cov; float* up_chi2; float* up_x; float* up_zref; int* up_row; int* up_n;   // upward refit (3.9.1)
+  int* m_sector; float* m_zin; float* m_zout;
+  int max_merge_bins;
+  int* m_bin_base; int* m_nzb;        // [S+1], [S]
+  int* m_bin_start; int* m_bin_fill;  // [max_merge_bins+2], [max_merge_bins]
+  int* m_bin_of; float4* m_rec; float4* m_srec;   // [max_tracks]: bin, inner-end record (z_in, row or -1, id), records sorted by bin
+  int* m_best_b; float* m_chi_b; int* m_dir_b; unsigned long long* m_best_a;
+  int* m_next; int* m_prev; int* m_dir;
+  int* m_head_scan; int* m_seg_scan; int* m_head_of;
+  MergeCounters* mcnt;
   Counters* cnt;
   int n_sms;
 };
@@ -112,6 +134,15 @@ struct FitPtrs {
   int max_tracks;
 };
 int launch_refit(const Ctx& c, const FitPtrs& o, cudaStream_t st);   // S7, separate call
+struct MergePtrs {                    // S9: cuts + the caller's outputs
+  int max_rows, back_rows; float edge, dz_win, chi2_cut;
+  float sin_a, cos_a;                 // sine / cosine of the sector angle, host-computed in fp32
+  int* n_merged; int* merged_of_track; int* seg_start; int* seg_idx;
+  float* par; float* cov; float* x_ref; float* z_ref; float* chi2; int* ndf; int* n_fit; int* sector; int* n_clusters;
+  int max_tracks;
+};
+int launch_merge(const Ctx& c, const FitPtrs& f, const MergePtrs& o, cudaStream_t st);   // S9, separate call
+int launches_merge();
 int launch_protect(const Ctx& c, const int* cluster_track, float road_y, float road_z, unsigned char* keep, cudaStream_t st);   // S8
 
 // In-place inclusive scan of data[0 .. *n_ptr + n_add) (int32), length known only on the device.

@@ -1,0 +1,140 @@
+"""GPU parity of the track merger (tpc_tracker_merge) against the oracle: every intermediate array
+(upward refit, best partners with their chi2, links) and every output (merged ids, CSR of segments, merged refit)
+bit-exact, on a central event, a piled-up slice, the 4-region pitch, with other cuts, and at the full size of cfg2-cfg4."""
+import numpy as np
+import pytest
+import torch
+
+from tests.parity_util import run_gpu, run_oracle
+from tpc_synth import default_params, generate_config
+
+pytestmark = pytest.mark.gpu
+
+CUTS = dict(max_rows=30, back_rows=1, edge=6.0, dz_win=50.0, chi2_cut=100.0)
+
+
+def _merge_parity(tf, P=None, cuts=None, min_links=1):
+    kw = dict(CUTS); kw.update(cuts or {})
+    P, trk, out = run_gpu(tf, params=P)
+    g = out.numpy()
+    T = g["n_tracks"]
+    m = trk.merge(T, kw)
+    o = run_oracle(tf, P, last_stage=6).merge(**kw)
+    f32 = np.float32
+    mt = trk.caps[3]
+    bad = []
+
+    def eq(name, a, b):
+        a = np.asarray(a); b = np.asarray(b)
+        if a.shape != b.shape or not np.array_equal(a, b):
+            bad.append(f"{name}: {a.shape} vs {b.shape}" if a.shape != b.shape else f"{name}: {int((a != b).sum())} of {a.size} differ")
+
+    assert T == o.get("trk_seed").size
+    # 3.9.1 upward refit
+    eq("fit_row", trk.stage_view("fit_row"), o.get("fit_row"))
+    eq("up_par", trk.stage_view("up_par").reshape(5, mt)[:, :T].T, o.get("up_par").astype(f32).reshape(-1, 5))
+    eq("up_cov", trk.stage_view("up_cov").reshape(15, mt)[:, :T].T, o.get("up_cov").astype(f32).reshape(-1, 15))
+    eq("up_x", trk.stage_view("up_x"), o.get("up_x_ref").astype(f32))
+    eq("up_zref", trk.stage_view("up_zref"), o.get("up_z_ref").astype(f32))
+    eq("up_row", trk.stage_view("up_row"), o.get("up_row"))
+    eq("up_n", trk.stage_view("up_n"), o.get("up_n"))
+    # 3.9.3 - 3.9.5 choice
+    eq("best_b", trk.stage_view("mrg_best_b"), o.get("mrg_best_b"))
+    eq("chi_b", trk.stage_view("mrg_chi_b"), o.get("mrg_chi2_b").astype(f32))
+    key = trk.stage_view("mrg_best_a")
+    eq("best_a", np.where(key == np.uint64(0xFFFFFFFFFFFFFFFF), -1, (key & np.uint64(0xFFFFFFFF)).astype(np.int64)), o.get("mrg_best_a"))
+    for nm in ("next", "prev", "dir"):
+        eq(nm, trk.stage_view("mrg_" + nm), o.get("mrg_" + nm))
+    # 3.9.6 chains
+    eq("n_merged", m["n_merged"], o.get("mrg_seg_start").size - 1)
+    eq("merged_of_track", m["merged_of_track"], o.get("mrg_of_track"))
+    eq("seg_start", m["seg_start"], o.get("mrg_seg_start"))
+    eq("seg_idx", m["seg_idx"], o.get("mrg_seg_idx"))
+    # 3.9.7 merged refit
+    eq("par", m["par"], o.get("mrg_par").astype(f32).reshape(-1, 5))
+    eq("cov", m["cov"], o.get("mrg_cov").astype(f32).reshape(-1, 15))
+    for nm in ("x_ref", "z_ref", "chi2"):
+        eq(nm, m[nm], o.get("mrg_" + nm).astype(f32))
+    for nm in ("ndf", "n_fit", "sector", "n_clusters"):
+        eq(nm, m[nm], o.get("mrg_" + nm))
+    if bad:
+        for nm in ("best_b", "best_a"):
+            gk = trk.stage_view("mrg_" + nm)
+            gk = np.where(gk == np.uint64(0xFFFFFFFFFFFFFFFF), -1, (gk & np.uint64(0xFFFFFFFF)).astype(np.int64)) if nm == "best_a" else gk
+            w = np.nonzero(gk != o.get("mrg_" + nm))[0][:5]
+            bad.append((nm, w.tolist(), gk[w].tolist(), o.get("mrg_" + nm)[w].tolist(), trk.stage_view("mrg_chi_b")[w].tolist(), o.get("mrg_chi2_b")[w].tolist()))
+    assert not bad, bad
+    links = int((o.get("mrg_next") >= 0).sum())
+    assert links >= min_links, links
+    return m, o, links
+
+
+def test_merge_central_event(mini_event):
+    m, o, links = _merge_parity(mini_event, min_links=300)
+    assert (o.get("mrg_dir") != 0).sum() > 300
+
+
+def test_merge_piled_up_slice_and_repeat(mini_tf):
+    m, o, links = _merge_parity(mini_tf, min_links=3000)
+    # the call is repeatable on the same handle state (ids come from scans, choices from order-independent minima)
+    P, trk, out = run_gpu(mini_tf)
+    T = out.numpy()["n_tracks"]
+    a = trk.merge(T); b = trk.merge(T)
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_merge_other_cuts_and_long_holes(mini_tf):
+    """A wide row window and z window, a loose and a very tight chi2 cut, no neighbour search at all (edge = 0 keeps only
+    ends outside the sector), rows removed from the frame so that same-sector links (dir = 0) occur."""
+    import copy
+    tf = copy.copy(mini_tf)
+    keep = ~np.isin(tf.row, np.arange(70, 76))
+    for f in ("sector", "row", "x", "y", "z", "track_id"):
+        setattr(tf, f, getattr(mini_tf, f)[keep].copy())
+    m, o, links = _merge_parity(tf, cuts=dict(max_rows=40), min_links=3000)
+    assert ((o.get("mrg_next") >= 0) & (o.get("mrg_dir") == 0)).sum() > 300
+    _merge_parity(mini_tf, cuts=dict(max_rows=60, dz_win=120.0, chi2_cut=400.0), min_links=3000)
+    _merge_parity(mini_tf, cuts=dict(chi2_cut=2.0), min_links=100)
+    _merge_parity(mini_tf, cuts=dict(edge=0.0, back_rows=0), min_links=0)
+
+
+def test_merge_non_uniform_pitch():
+    from tpc_synth import FOUR_REGION_PITCH, Geometry, generate
+    from tpc_synth.generator import CONFIGS
+    rec = dict(CONFIGS["cfg2"]); rec.update(n_tracks=600, seed=31)
+    tf = generate(rec, geometry=Geometry(pitch_regions=FOUR_REGION_PITCH, x_last=85.0 + 0.75 * 62.5 + 1.0 * 34 + 1.2 * 30 + 1.5 * 25))
+    _merge_parity(tf, min_links=200)
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4"])
+def test_merge_full_size_configs(name):
+    tf = generate_config(name, device="cuda")
+    m, o, links = _merge_parity(tf, min_links=5000)
+    print(name, "tracks", o.get("trk_seed").size, "merged", m["n_merged"], "links", links)
+
+
+def test_merge_at_time_frame_density():
+    """Six whole sectors of the 50 kHz Pb-Pb time frame (cfg5: 11.4 ms of z, 5 % noise) as a frame of their own: three
+    neighbours on the A side, three on the C side, ~15 M clusters."""
+    from tpc_synth import select_sectors
+    tf = generate_config("cfg5", device="cuda")
+    sub, _ = select_sectors(tf, [0, 1, 2, 20, 21, 22])
+    del tf
+    P = default_params(sub)
+    m, o, links = _merge_parity(sub, P=P, min_links=50000)
+    print("tracks", o.get("trk_seed").size, "merged", m["n_merged"], "links", links)
+
+
+def test_merge_rejects_bad_arguments(cfg1):
+    import ctypes as C
+    import paper_2009_07515_b200 as tpc
+    P, trk, out = run_gpu(cfg1)
+    fit = trk.new_fit(); mg = trk.new_merged()
+    trk.refit_into(fit)
+    for bad in (dict(dz_win=0.0), dict(dz_win=float("inf")), dict(max_rows=-1), dict(chi2_cut=float("nan")), dict(edge=-1.0)):
+        with pytest.raises(RuntimeError):
+            trk.merge_into(fit, mg, bad)
+    trk.merge_into(fit, mg)
+    torch.cuda.synchronize()
+    assert int(mg["n_merged"].item()) >= 1
