@@ -276,6 +276,8 @@ typedef struct {
   float edge;         /* cm: a neighbour is tried only if the outer end lies within `edge` of the sector boundary (6) */
   float dz_win;       /* cm: |z_in(B) - z_out(A)| window of the candidates (50); > 0 */
   float chi2_cut;     /* candidates need chi2 <= chi2_cut over the five parameters (100) */
+  float road_z0;      /* cm: z road around the straight continuation of the outer state, |dz| <= road_z0 + road_z1 |dx| (2) */
+  float road_z1;      /* cm per cm (0.3) */
 } tpc_merge_cuts_t;
 
 /* Merged tracks (DEVICE pointers, caller-allocated for max_tracks entries each; layouts as in tpc_tracks_t).

@@ -64,7 +64,7 @@ def _load():
         lib.orc_protect.restype = None
         lib.orc_protect.argtypes = [C.c_void_p, C.c_float, C.c_float]
         lib.orc_merge.restype = None
-        lib.orc_merge.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float]
+        lib.orc_merge.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float]
         lib.orc_kf_rotate.restype = C.c_double
         lib.orc_kf_rotate.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double]
         lib.orc_search.restype = C.c_int
@@ -121,10 +121,11 @@ class Oracle:
         self._lib.orc_protect(self._h, float(road_y), float(road_z))
         return self.get("keep")
 
-    def merge(self, max_rows: int = 30, back_rows: int = 1, edge: float = 6.0, dz_win: float = 100.0,
-              chi2_cut: float = 100.0) -> "Oracle":
+    def merge(self, max_rows: int = 30, back_rows: int = 1, edge: float = 6.0, dz_win: float = 50.0,
+              chi2_cut: float = 100.0, road_z0: float = 2.0, road_z1: float = 0.3) -> "Oracle":
         """DESIGN.md section 3.9 on the tracks and the refit of the last run (last_stage = 6): results under mrg_*."""
-        self._lib.orc_merge(self._h, int(max_rows), int(back_rows), float(edge), float(dz_win), float(chi2_cut))
+        self._lib.orc_merge(self._h, int(max_rows), int(back_rows), float(edge), float(dz_win), float(chi2_cut),
+                            float(road_z0), float(road_z1))
         return self
 
     def kf_rotate(self, par, cov15, x, sa, ca, precision=64):

@@ -687,7 +687,7 @@ struct Oracle {
   // stage6 (the downward refit gives every segment's state at its INNER end).
   //   9.1 upward refit: the state at the OUTER end;  9.2-9.4 candidates and score;  9.5 mutual best;  9.6 chains;
   //   9.7 downward refit of every merged track through all its segments, turning the frame at sector changes.
-  struct MergeCuts { int32_t max_rows, back_rows; float edge, dz_win, chi2_cut; };
+  struct MergeCuts { int32_t max_rows, back_rows; float edge, dz_win, chi2_cut, road_z0, road_z1; };
 
   template <class T>
   void stage9(const MergeCuts& mc) {
@@ -756,6 +756,12 @@ struct Oracle {
           sb = (sa_ / n_az) * n_az + ((sa_ % n_az) + dir + n_az) % n_az;
           if (sb == sa_) continue;                        // a one-sector geometry has no neighbour
         }
+        // 9.4 (first half) the outer state of a, turned into the neighbour's frame if that is where this pass looks
+        KF<T> k0; load_kf(k0, &up_par[(size_t)a * 5], &up_cov[(size_t)a * 15], 0.0);
+        T x0 = T(up_x_ref[a]);
+        if (dir != 0 && !kf_rotate<T>(k0, kbT, x0, dir > 0 ? sin_a : T(0) - sin_a, cos_a, msp, &x0)) continue;
+        // the road: where a straight continuation of that state has its z at a given x
+        const T zslope = k0.p[3] / std::sqrt(T(1) - k0.p[2] * k0.p[2]);
         const auto& lst = by_sector[sb];
         const T zlo = z_out[a] - dzw, zhi = z_out[a] + dzw;
         auto it = std::lower_bound(lst.begin(), lst.end(), zlo, [&](int32_t b, T v) { return z_in[b] < v; });
@@ -764,11 +770,11 @@ struct Oracle {
           if (b == a || up_n[b] < 2 || fit_n[b] < 2) continue;
           const int rb = fit_row[b];
           if (dir == 0 ? (rb < ra + 1 || rb > ra + mc.max_rows) : (rb < ra - mc.back_rows || rb > ra + mc.max_rows)) continue;
-          // 9.4 the outer state of a, turned into b's frame if that is another sector, moved to b's inner plane
-          KF<T> k; load_kf(k, &up_par[(size_t)a * 5], &up_cov[(size_t)a * 15], 0.0);
-          T x = T(up_x_ref[a]);
-          if (dir != 0 && !kf_rotate<T>(k, kbT, x, dir > 0 ? sin_a : T(0) - sin_a, cos_a, msp, &x)) continue;
-          if (!kf_propagate<T>(k, kbT, T(fit_x_ref[b]) - x, msp, (T*)nullptr)) continue;
+          const T dxb = T(fit_x_ref[b]) - x0;
+          if (!(std::fabs(z_in[b] - (z_out[a] + dxb * zslope)) <= T(mc.road_z0) + T(mc.road_z1) * std::fabs(dxb))) continue;
+          // 9.4 (second half) moved to b's inner plane
+          KF<T> k = k0;
+          if (!kf_propagate<T>(k, kbT, dxb, msp, (T*)nullptr)) continue;
           const double* pb = &fit_par[(size_t)b * 5]; const double* cb = &fit_cov[(size_t)b * 15];
           T d[5];
           d[0] = T(pb[0]) - k.p[0];
@@ -1040,9 +1046,9 @@ int orc_kf_fit(const void* params, int prec, int npt, const double* x, const dou
 void orc_protect(void* h, float road_y, float road_z) { reinterpret_cast<Oracle*>(h)->stage7_protect(road_y, road_z); }
 
 // S9 on the tracks and the refit of the last orc_run (last_stage >= 6)
-void orc_merge(void* h, int max_rows, int back_rows, float edge, float dz_win, float chi2_cut) {
+void orc_merge(void* h, int max_rows, int back_rows, float edge, float dz_win, float chi2_cut, float road_z0, float road_z1) {
   Oracle* o = reinterpret_cast<Oracle*>(h);
-  const Oracle::MergeCuts mc{max_rows, back_rows, edge, dz_win, chi2_cut};
+  const Oracle::MergeCuts mc{max_rows, back_rows, edge, dz_win, chi2_cut, road_z0, road_z1};
   if (o->s4_prec == 64) o->stage9<double>(mc); else o->stage9<float>(mc);
 }
 

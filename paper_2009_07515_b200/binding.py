@@ -55,7 +55,7 @@ class tpc_fit_t(C.Structure):
 
 class tpc_merge_cuts_t(C.Structure):
     _fields_ = [("max_rows", C.c_int32), ("back_rows", C.c_int32), ("edge", C.c_float), ("dz_win", C.c_float),
-                ("chi2_cut", C.c_float)]
+                ("chi2_cut", C.c_float), ("road_z0", C.c_float), ("road_z1", C.c_float)]
 
 
 _MERGED_FIELDS = ["n_merged", "merged_of_track", "seg_start", "seg_idx", "par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit",
@@ -66,7 +66,7 @@ class tpc_merged_t(C.Structure):
     _fields_ = [("max_tracks", C.c_int64)] + [(f, C.c_void_p) for f in _MERGED_FIELDS]
 
 
-MERGE_CUTS = dict(max_rows=30, back_rows=1, edge=6.0, dz_win=50.0, chi2_cut=100.0)
+MERGE_CUTS = dict(max_rows=30, back_rows=1, edge=6.0, dz_win=50.0, chi2_cut=100.0, road_z0=2.0, road_z1=0.3)
 
 
 class tpc_counters_t(C.Structure):
@@ -367,7 +367,8 @@ class Tracker:
         for k in ("par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit"):
             setattr(f, k, fit[k].data_ptr())
         kw = dict(MERGE_CUTS); kw.update(cuts or {})
-        c = tpc_merge_cuts_t(int(kw["max_rows"]), int(kw["back_rows"]), float(kw["edge"]), float(kw["dz_win"]), float(kw["chi2_cut"]))
+        c = tpc_merge_cuts_t(int(kw["max_rows"]), int(kw["back_rows"]), float(kw["edge"]), float(kw["dz_win"]), float(kw["chi2_cut"]),
+                             float(kw["road_z0"]), float(kw["road_z1"]))
         m = tpc_merged_t()
         m.max_tracks = self.caps[3]
         for k in _MERGED_FIELDS:

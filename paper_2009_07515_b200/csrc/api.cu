@@ -442,7 +442,7 @@ int tpc_tracker_merge(tpc_tracker_t* t, const tpc_fit_t* fit, const tpc_merge_cu
       !out->z_ref || !out->chi2 || !out->ndf || !out->n_fit || !out->sector || !out->n_clusters)
     return TPC_ERR_INVALID_ARG;
   if (cuts->max_rows < 0 || cuts->back_rows < 0 || !(cuts->edge >= 0.f) || !(cuts->dz_win > 0.f) || !(cuts->dz_win < INFINITY) ||
-      !(cuts->chi2_cut >= 0.f))
+      !(cuts->chi2_cut >= 0.f) || !(cuts->road_z0 >= 0.f) || !(cuts->road_z1 >= 0.f))
     return TPC_ERR_INVALID_ARG;
   if (fit->max_tracks < 1 || fit->max_tracks > t->max_tracks || out->max_tracks < 1 || out->max_tracks > t->max_tracks)
     return TPC_ERR_CAPACITY;
@@ -451,6 +451,7 @@ int tpc_tracker_merge(tpc_tracker_t* t, const tpc_fit_t* fit, const tpc_merge_cu
   f.n_fit = fit->n_fit; f.max_tracks = (int)fit->max_tracks;
   MergePtrs o{};
   o.max_rows = cuts->max_rows; o.back_rows = cuts->back_rows; o.edge = cuts->edge; o.dz_win = cuts->dz_win; o.chi2_cut = cuts->chi2_cut;
+  o.road_z0 = cuts->road_z0; o.road_z1 = cuts->road_z1;
   // sine and cosine of the sector angle from tan_half_sector alone, fp32, one rounding per operation
   const float th = t->params.tan_half_sector;
   const float den = 1.0f + th * th;

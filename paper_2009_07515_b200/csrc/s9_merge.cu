@@ -9,8 +9,8 @@
 //                    inner end into its (sector, z) bin
 //   scan + k_merge_fill   counting sort of 16-byte inner-end records by (sector, z bin): "extensive use of sort" - here
 //                    a hand-written counting sort (no Thrust / CUB), the window of 3.9.3 is then a contiguous run of bins
-//   k_merge_match    thread per outer end: candidates of 3.9.3 from the bins around z_out, score 3.9.4 (rotation +
-//                    helix step + chi2), best partner of the outer end in registers (ties -> lowest id), best partner of
+//   k_merge_match    warp per outer end: candidates of 3.9.3 from the bins around z_out, score 3.9.4 (rotation +
+//                    helix step + chi2), best partner of the outer end by a warp reduction (ties -> lowest id), best partner of
 //                    every inner end by a 64-bit atomicMin of (chi2 bits, id) - both independent of the visiting order
 //   k_merge_link     mutual best -> links (3.9.5);  flags + scan -> merged ids (3.9.6)
 //   k_chain_len / scan / k_chain_fill   chains followed from their heads: merged_of_track, CSR merged -> segments
@@ -215,8 +215,8 @@ __global__ void __launch_bounds__(kThreads) k_refit_up(Ctx c, FitPtrs f, MergePt
     // the inner end goes into its (sector, z) bin (every track: those that take no part are skipped when read)
     const int b = merge_bin(c, sector, z_in, inv_w);
     c.m_bin_of[id] = b;
-    // the record the candidate scan reads: z_in, the row of the inner state (-1: takes no part), the id
-    c.m_rec[id] = make_float4(z_in, __int_as_float(nfit >= 2 && f.n_fit[id] >= 2 ? c.fit_row[id] : -1), __int_as_float(id), 0.0f);
+    // the record the candidate scan reads: z_in, the row of the inner state (-1: takes no part), the id, x of the inner state
+    c.m_rec[id] = make_float4(z_in, __int_as_float(nfit >= 2 && f.n_fit[id] >= 2 ? c.fit_row[id] : -1), __int_as_float(id), f.x_ref[id]);
     atomicAdd(c.m_bin_start + b + 1, 1);              // counts at b + 1: the inclusive scan leaves the CSR starts in place
   }
 }
@@ -237,6 +237,9 @@ __global__ void __launch_bounds__(kThreads) k_merge_zero_fill(Ctx c) {
 }
 
 // ---------------------------------------------------------------------------------- 3.9.3 - 3.9.5 candidates, score, choice
+// One WARP per outer end: the lanes read the window's run of 16-byte records together (coalesced; a thread per outer end
+// walked ~130 records one dependent load after the other: 35 ms on cfg5), apply the cheap cuts, and the few lanes whose
+// record survives score their pair.  Lane-local best (chi2, then id), then a warp reduction with the same order.
 __global__ void __launch_bounds__(kThreads) k_merge_match(Ctx c, FitPtrs f, MergePtrs o) {
   extern __shared__ float sm[];
   float* tymax = sm;
@@ -246,15 +249,12 @@ __global__ void __launch_bounds__(kThreads) k_merge_match(Ctx c, FitPtrs f, Merg
   const int nt = n_tracks_of(c, o), n_az = c.S >> 1;
   const size_t mt = (size_t)c.max_tracks, ft = (size_t)f.max_tracks;
   const float inv_w = c.mcnt->inv_w;
-  for (int a = blockIdx.x * blockDim.x + threadIdx.x; a < nt; a += gridDim.x * blockDim.x) {
-    if (c.up_n[a] < 2 || f.n_fit[a] < 2) continue;
+  const int lane = threadIdx.x & 31;
+  const int warps = (gridDim.x * blockDim.x) >> 5;
+  for (int a = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; a < nt; a += warps) {
+    if (c.up_n[a] < 2 || f.n_fit[a] < 2) continue;       // warp-uniform
     const int s_a = c.m_sector[a], r_a = c.up_row[a];
-    KF ka;
-#pragma unroll
-    for (int i = 0; i < 5; ++i) ka.p[i] = c.up_par[i * mt + a];
-#pragma unroll
-    for (int i = 0; i < 15; ++i) ka.c[i] = c.up_cov[i * mt + a];
-    ka.chi2 = 0.f;
+    const float y_a = c.up_par[0 * mt + a];
     const float x_a = c.up_x[a], zref_a = c.up_zref[a], z_out = c.m_zout[a];
     const float zlo = z_out - o.dz_win, zhi = z_out + o.dz_win;
     float best = 0.f;
@@ -262,25 +262,35 @@ __global__ void __launch_bounds__(kThreads) k_merge_match(Ctx c, FitPtrs f, Merg
     for (int pass = 0; pass < 2; ++pass) {
       int dir = 0, s_b = s_a;
       if (pass == 1) {
-        if (!(fabsf(ka.p[0]) >= tymax[r_a] - o.edge)) continue;
-        dir = ka.p[0] >= 0.0f ? 1 : -1;
+        if (!(fabsf(y_a) >= tymax[r_a] - o.edge)) continue;
+        dir = y_a >= 0.0f ? 1 : -1;
         s_b = (s_a / n_az) * n_az + ((s_a % n_az) + dir + n_az) % n_az;
         if (s_b == s_a) continue;
       }
       if (c.m_nzb[s_b] == 0) continue;
+      // 3.9.4, first half (once per pass, every lane the same): the outer state, turned into the neighbour's frame
+      KF k0;
+#pragma unroll
+      for (int i = 0; i < 5; ++i) k0.p[i] = c.up_par[i * mt + a];
+#pragma unroll
+      for (int i = 0; i < 15; ++i) k0.c[i] = c.up_cov[i * mt + a];
+      k0.chi2 = 0.f;
+      float x0 = x_a;
+      if (dir != 0 && !kf_rotate(k0, c.kb, x0, dir > 0 ? o.sin_a : 0.0f - o.sin_a, o.cos_a, c.max_sinphi, &x0)) continue;
+      const float zslope = k0.p[3] / sqrtf(1.0f - k0.p[2] * k0.p[2]);   // the road of 3.9.3: dz/dx of a straight continuation
       const int b0 = merge_bin(c, s_b, zlo, inv_w), b1 = merge_bin(c, s_b, zhi, inv_w);
       const int j0 = c.m_bin_start[b0], j1 = c.m_bin_start[b1 + 1];
-      for (int j = j0; j < j1; ++j) {
-        const float4 rec = __ldg(c.m_srec + j);         // contiguous run of 16-byte records: no gather before the cheap cuts
+      for (int j = j0 + lane; j < j1; j += 32) {
+        const float4 rec = __ldg(c.m_srec + j);         // (z_in, row of the inner state or -1, id, x of the inner state)
         const int b = __float_as_int(rec.z), r_b = __float_as_int(rec.y);
         const float z_b = rec.x;
         if (b == a || r_b < 0) continue;
         if (!(z_b >= zlo && z_b <= zhi)) continue;
         if (dir == 0 ? (r_b < r_a + 1 || r_b > r_a + o.max_rows) : (r_b < r_a - o.back_rows || r_b > r_a + o.max_rows)) continue;
-        KF k = ka;
-        float x = x_a;
-        if (dir != 0 && !kf_rotate(k, c.kb, x, dir > 0 ? o.sin_a : 0.0f - o.sin_a, o.cos_a, c.max_sinphi, &x)) continue;
-        if (!kf_propagate(k, c.kb, f.x_ref[b] - x, c.max_sinphi)) continue;
+        const float dxb = rec.w - x0;
+        if (!(fabsf(z_b - (z_out + dxb * zslope)) <= o.road_z0 + o.road_z1 * fabsf(dxb))) continue;
+        KF k = k0;
+        if (!kf_propagate(k, c.kb, dxb, c.max_sinphi)) continue;
         float d[5];
         d[0] = f.par[0 * ft + b] - k.p[0];
         d[1] = z_b - (zref_a + k.p[1]);
@@ -299,7 +309,14 @@ __global__ void __launch_bounds__(kThreads) k_merge_match(Ctx c, FitPtrs f, Merg
         atomicMin(c.m_best_a + b, ((unsigned long long)ck << 32) | (unsigned)a);
       }
     }
-    c.m_best_b[a] = bb; c.m_dir_b[a] = bdir; c.m_chi_b[a] = bb >= 0 ? best : -1.0f;
+    __syncwarp();
+#pragma unroll
+    for (int off = 16; off; off >>= 1) {
+      const float ochi = __shfl_xor_sync(0xffffffffu, best, off);
+      const int ob = __shfl_xor_sync(0xffffffffu, bb, off), od = __shfl_xor_sync(0xffffffffu, bdir, off);
+      if (ob >= 0 && (bb < 0 || ochi < best || (ochi == best && ob < bb))) { best = ochi; bb = ob; bdir = od; }
+    }
+    if (lane == 0) { c.m_best_b[a] = bb; c.m_dir_b[a] = bdir; c.m_chi_b[a] = bb >= 0 ? best : -1.0f; }
   }
 }
 
@@ -442,7 +459,7 @@ int launch_merge(const Ctx& c, const FitPtrs& f, const MergePtrs& o, cudaStream_
   if (launch_scan_inclusive(c.m_bin_start, &c.mcnt->n_bins, 1, (long long)c.max_merge_bins + 1, c.tile_sums, nullptr, c.n_sms, st)) return -1;
   k_merge_zero_fill<<<gb, kThreads, 0, st>>>(c);
   k_merge_fill<<<gt, kThreads, 0, st>>>(c, o);
-  k_merge_match<<<gt, kThreads, sh, st>>>(c, f, o);
+  k_merge_match<<<grid_for((long long)c.max_tracks * 32, c, 64), kThreads, sh, st>>>(c, f, o);
   k_merge_link<<<gt, kThreads, 0, st>>>(c, o);
   k_merge_heads<<<gt, kThreads, 0, st>>>(c, o);
   if (launch_scan_inclusive(c.m_head_scan, &c.mcnt->n_scan, 0, c.max_tracks, c.tile_sums, nullptr, c.n_sms, st)) return -1;

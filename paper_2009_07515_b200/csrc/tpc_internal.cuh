@@ -105,7 +105,7 @@ struct Ctx {
   int max_merge_bins;
   int* m_bin_base; int* m_nzb;        // [S+1], [S]
   int* m_bin_start; int* m_bin_fill;  // [max_merge_bins+2], [max_merge_bins]
-  int* m_bin_of; float4* m_rec; float4* m_srec;   // [max_tracks]: bin, inner-end record (z_in, row or -1, id), records sorted by bin
+  int* m_bin_of; float4* m_rec; float4* m_srec;   // [max_tracks]: bin, inner-end record (z_in, row or -1, id, x_in), records sorted by bin
   int* m_best_b; float* m_chi_b; int* m_dir_b; unsigned long long* m_best_a;
   int* m_next; int* m_prev; int* m_dir;
   int* m_head_scan; int* m_seg_scan; int* m_head_of;
@@ -135,7 +135,7 @@ struct FitPtrs {
 };
 int launch_refit(const Ctx& c, const FitPtrs& o, cudaStream_t st);   // S7, separate call
 struct MergePtrs {                    // S9: cuts + the caller's outputs
-  int max_rows, back_rows; float edge, dz_win, chi2_cut;
+  int max_rows, back_rows; float edge, dz_win, chi2_cut, road_z0, road_z1;
   float sin_a, cos_a;                 // sine / cosine of the sector angle, host-computed in fp32
   int* n_merged; int* merged_of_track; int* seg_start; int* seg_idx;
   float* par; float* cov; float* x_ref; float* z_ref; float* chi2; int* ndf; int* n_fit; int* sector; int* n_clusters;

@@ -10,7 +10,7 @@ from tpc_synth import default_params, generate_config
 
 pytestmark = pytest.mark.gpu
 
-CUTS = dict(max_rows=30, back_rows=1, edge=6.0, dz_win=50.0, chi2_cut=100.0)
+CUTS = dict(max_rows=30, back_rows=1, edge=6.0, dz_win=50.0, chi2_cut=100.0, road_z0=2.0, road_z1=0.3)
 
 
 def _merge_parity(tf, P=None, cuts=None, min_links=1):
@@ -94,7 +94,8 @@ def test_merge_other_cuts_and_long_holes(mini_tf):
         setattr(tf, f, getattr(mini_tf, f)[keep].copy())
     m, o, links = _merge_parity(tf, cuts=dict(max_rows=40), min_links=3000)
     assert ((o.get("mrg_next") >= 0) & (o.get("mrg_dir") == 0)).sum() > 300
-    _merge_parity(mini_tf, cuts=dict(max_rows=60, dz_win=120.0, chi2_cut=400.0), min_links=3000)
+    _merge_parity(mini_tf, cuts=dict(max_rows=60, dz_win=120.0, chi2_cut=400.0, road_z0=1e9), min_links=3000)
+    _merge_parity(mini_tf, cuts=dict(road_z0=0.05, road_z1=0.01), min_links=500)
     _merge_parity(mini_tf, cuts=dict(chi2_cut=2.0), min_links=100)
     _merge_parity(mini_tf, cuts=dict(edge=0.0, back_rows=0), min_links=0)
 
@@ -132,7 +133,7 @@ def test_merge_rejects_bad_arguments(cfg1):
     P, trk, out = run_gpu(cfg1)
     fit = trk.new_fit(); mg = trk.new_merged()
     trk.refit_into(fit)
-    for bad in (dict(dz_win=0.0), dict(dz_win=float("inf")), dict(max_rows=-1), dict(chi2_cut=float("nan")), dict(edge=-1.0)):
+    for bad in (dict(dz_win=0.0), dict(dz_win=float("inf")), dict(max_rows=-1), dict(chi2_cut=float("nan")), dict(edge=-1.0), dict(road_z0=-1.0)):
         with pytest.raises(RuntimeError):
             trk.merge_into(fit, mg, bad)
     trk.merge_into(fit, mg)

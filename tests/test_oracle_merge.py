@@ -21,7 +21,7 @@ import pytest
 from oracle import Oracle
 from tpc_synth import default_params, generate_config, select_sectors
 
-CUTS = dict(max_rows=30, back_rows=1, edge=6.0, dz_win=50.0, chi2_cut=100.0)
+CUTS = dict(max_rows=30, back_rows=1, edge=6.0, dz_win=50.0, chi2_cut=100.0, road_z0=2.0, road_z1=0.3)
 A20 = math.radians(20.0)
 
 
@@ -286,6 +286,13 @@ def test_candidates_score_choice_links_and_chains_against_brute_force(mini_tf):
                 ok, par, cov, x = o.kf_rotate(par, cov, x, float(sin_a) * d, float(cos_a), precision=32)
                 if not ok:
                     continue
+            # the road: a straight continuation of the (turned) outer state
+            with np.errstate(invalid="ignore"):
+                zslope = f32(f32(par[3]) / np.sqrt(f32(f32(1) - f32(f32(par[2]) * f32(par[2])))))
+            dxb = f32(f32(fx[b]) - f32(x))
+            z_lin = f32(z_out[a] + f32(dxb * zslope))
+            if not (abs(f32(z_in[b] - z_lin)) <= f32(f32(CUTS["road_z0"]) + f32(f32(CUTS["road_z1"]) * abs(dxb)))):
+                continue
             ok, par, cov, _ = o.kf_propagate(par, cov, x, fx[b], precision=32)
             if not ok:
                 continue
