@@ -25,6 +25,23 @@
 // row's bin_start entry at the linearly extrapolated position, issued one step ahead: 15.9 ms (20 more instructions
 // in a divergent region cost more than the latency they hide).
 //
+// Round 2, measured on cfg5 with ncu source-level counters (profiles/r02_s4_regions.md): the transport and the update
+// run at 29.9 and 28.4 of 32 lanes; the grid search runs at 9.4 lanes (3.6 inside its candidate loop), is 36 % of the
+// warp instructions and 55 % of the stall samples (two dependent gathers, bin_start then (y,z)).  Tried and rejected,
+// all bit-exact:
+//  * searches batched inside the warp (lanes that need a search wait until 8 .. 28 lanes do, then search together):
+//    14.1 ms at 8, 15.0 at 16, 27 at 28 lanes - searches come in runs per lane (phase B, below the head), so waiting
+//    lanes idle for many steps and the memory-level parallelism drops;
+//  * the bin_start line of the next search prefetched (prefetch.global.L1 / .L2, or a real load kept in a register)
+//    at the straight-line prediction before the transport: 13.0 - 13.4 ms against 12.9 for the same code without it;
+//    ncu: L1 hits rose by the number of prefetches, the stall at the first use of bin_start did not move - a warp waits
+//    for the slowest of its ~9 searching lanes (second bin row, rare misprediction), not for the average one;
+//  * streaming stores / loads (st.global.cs, ld.global.cs) for the hit table: 12.26 ms against 12.06;
+//  * covariance in shared memory, two buffers (live / last update, no copy), transport staged row by row: 64 registers,
+//    8 CTAs per SM, occupancy 37 -> 49 %: 11.8 ms (7 CTAs 11.7, 9 CTAs 12.8, 10 CTAs 19.8), but DRAM reads 10.5 -> 16.7 GB
+//    and L2 hit rate 53 -> 47 %: the lanes in flight (608-byte hit table each, plus the rows they walk) already exceed
+//    L2, so more warps buy latency hiding with cache misses - occupancy is not the lever, the working set is.
+//
 // Arithmetic is written operation by operation in the order of DESIGN.md section 3.4 (compiled with
 // -fmad=false; fused multiply-adds only where the text writes fma(), as __fmaf_rn): the transport J C J^T skips only
 // the terms that are structurally 0*x or 1*x.
