@@ -10,6 +10,16 @@
 // 14.1 ms; the five phases (up k=1, up k=2, down k=1, down k=2, scoring) on compacted CTA work lists with the cluster
 // state in shared memory 10.4 ms (twelve CTA barriers per tile cost more than the idle lanes they remove); the k = 2 up
 // retries (40 % of the clusters, 2 ms of the kernel) deferred to a second, compacted launch 6.5 ms.
+// Round 2 (profiles/r02_s2_regions.md: 49 % of the instructions are the rectangle query at 10 - 18 lanes, 20 % the pair
+// scoring at 9.6 lanes; DRAM traffic = 1.0 x the algorithmic bytes).  Two more designs measured and rejected on cfg5
+// (this version: 5.74 ms), both bit-exact:
+//  * the rectangle query split in two halves (bin cover + the four bin_start loads / the candidate walk) so that the
+//    loads of the up and the down query of a cluster are in flight together before either walk starts: 6.12 ms - the
+//    down query is then computed for the 15 % of the clusters whose up window turns out empty, and eight more live
+//    values per thread cost more than the overlapped latency (the kernel is issue-bound, 75 % of the slots busy);
+//  * the candidate lists keep (position, y, z) so that the scoring does not gather the candidates a second time
+//    (kCap 4 to keep 5 CTAs per SM): 7.77 ms - the second gather hits L1 anyway, while the lists' shared-memory
+//    traffic triples and windows with 5 - 8 candidates fall back to the re-walk.
 #include "tpc_internal.cuh"
 
 namespace tpc {
