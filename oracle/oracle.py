@@ -65,6 +65,8 @@ def _load():
         lib.orc_protect.argtypes = [C.c_void_p, C.c_float, C.c_float]
         lib.orc_merge.restype = None
         lib.orc_merge.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float]
+        lib.orc_apex.restype = None
+        lib.orc_apex.argtypes = [C.c_void_p, C.c_int] + [C.c_float] * 6
         lib.orc_kf_rotate.restype = C.c_double
         lib.orc_kf_rotate.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double]
         lib.orc_search.restype = C.c_int
@@ -126,6 +128,12 @@ class Oracle:
         """DESIGN.md section 3.9 on the tracks and the refit of the last run (last_stage = 6): results under mrg_*."""
         self._lib.orc_merge(self._h, int(max_rows), int(back_rows), float(edge), float(dz_win), float(chi2_cut),
                             float(road_z0), float(road_z1))
+        return self
+
+    def apex(self, max_k: int = 4, min_s: float = 0.6, dz_win: float = 150.0, tol_c: float = 0.1, tol_z: float = 4.0,
+             tol_t: float = 0.1, cut: float = 3.0) -> "Oracle":
+        """DESIGN.md section 3.9.8 on the merged tracks of the last merge(): results under apx_*."""
+        self._lib.orc_apex(self._h, int(max_k), float(min_s), float(dz_win), float(tol_c), float(tol_z), float(tol_t), float(cut))
         return self
 
     def kf_rotate(self, par, cov15, x, sa, ca, precision=64):

@@ -300,6 +300,9 @@ struct Oracle {
   std::vector<int32_t> mrg_of_track, mrg_seg_start, mrg_seg_idx;   // merged id of every track; CSR merged -> tracks, inner to outer
   std::vector<double> mrg_par, mrg_cov, mrg_x_ref, mrg_z_ref, mrg_chi2;
   std::vector<int32_t> mrg_n_fit, mrg_ndf, mrg_sector, mrg_n_clusters;
+  // S9 apex links of loopers
+  std::vector<int32_t> apx_best, apx_partner, apx_leg;             // [n_merged]
+  std::vector<double> apx_score;                                   // [n_merged] score of apx_best or -1
   int s4_prec = 32;
   std::vector<int32_t> trk_cl_start, trk_cl_idx, cluster_track;
   std::vector<double> stage_seconds;                              // [5]
@@ -863,6 +866,111 @@ struct Oracle {
     }
   }
 
+
+  // ---------------------------------------------------------------------------------------- S9, part 2
+  // Apex links: looper following ("secondary legs of looping tracks", PAPER.md:107
+  // "the following of looping tracks").  A track that curls up inside the TPC is found as two merged tracks, the outgoing
+  // leg and the returning leg (which the finder walks outwards, against the particle's motion); they are never
+  // joined by 3.9.3 because the stretch around the apex, where |sin(phi)| >= max_sinphi, cannot be parametrised in x.
+  // Both legs end steeply at the apex side and lie on ONE circle: their OUTER ends are compared through the circle
+  // centres, the z advance along the arc between the two end points and the dip angles.
+  struct ApexCuts { int32_t max_k; float min_s, dz_win, tol_c, tol_z, tol_t, cut; };
+
+  template <class T>
+  void stage10(const ApexCuts& ac) {
+    const int nm = (int)mrg_seg_start.size() - 1, n_az = P.n_sectors / 2;
+    const T kbT = T(kb);
+    const T th = T(P.tan_half_sector);
+    const T den = T(1) + th * th;
+    const T sin_a = (T(2) * th) / den, cos_a = (T(1) - th * th) / den;
+    apx_best.assign(nm, -1); apx_partner.assign(nm, -1); apx_leg.assign(nm, 0); apx_score.assign(nm, -1.0);
+    std::vector<int32_t> tail(nm);
+    std::vector<T> zo(nm);
+    for (int m = 0; m < nm; ++m) {
+      tail[m] = mrg_seg_idx[mrg_seg_start[m + 1] - 1];
+      zo[m] = T(up_z_ref[tail[m]]) + T(up_par[(size_t)tail[m] * 5 + 1]);
+    }
+    // a tail takes part iff its outer state is steep (it ends because the track curls over) and has a curvature
+    auto steep = [&](int m) {
+      const int t = tail[m];
+      const T s = T(up_par[(size_t)t * 5 + 2]);
+      return up_n[t] >= 2 && std::fabs(s) >= T(ac.min_s) && std::fabs(s) < T(1) && kbT * T(up_par[(size_t)t * 5 + 4]) != T(0);
+    };
+    // circle centre of a tail in its own sector frame: xc = x - sin(phi)/c, yc = y + cos(phi)/c
+    auto centre = [&](int t, T* xc, T* yc, T* R, T* c) {
+      const T s = T(up_par[(size_t)t * 5 + 2]);
+      *c = kbT * T(up_par[(size_t)t * 5 + 4]);
+      *xc = T(up_x_ref[t]) - s / *c;
+      *yc = T(up_par[(size_t)t * 5 + 0]) + std::sqrt(T(1) - s * s) / *c;
+      *R = T(1) / std::fabs(*c);
+    };
+    for (int A = 0; A < nm; ++A) {
+      if (!steep(A)) continue;
+      const int a = tail[A], s_a = trk_sector[a];
+      const T xA = T(up_x_ref[a]), yA = T(up_par[(size_t)a * 5 + 0]), tA = T(up_par[(size_t)a * 5 + 3]);
+      const int dirA = T(up_par[(size_t)a * 5 + 2]) >= T(0) ? 1 : -1;   // the side the track curls to
+      T xcA, ycA, RA, cA;
+      centre(a, &xcA, &ycA, &RA, &cA);
+      T best = T(0); int bb = -1;
+      T sk = T(0), ck = T(1);                               // sine and cosine of k sector angles
+      for (int k = 0; k <= ac.max_k; ++k) {
+        if (k > 0) {
+          const T s2 = sk * cos_a + ck * sin_a, c2 = ck * cos_a - sk * sin_a;
+          sk = s2; ck = c2;
+        }
+        const int s_b = (s_a / n_az) * n_az + ((((s_a % n_az) + dirA * k) % n_az) + n_az) % n_az;
+        if (k > 0 && s_b == s_a) break;                     // once round
+        const T sd = dirA > 0 ? sk : T(0) - sk;             // sector s_b is the frame of s_a turned by dirA * k sector angles
+        for (int B = 0; B < nm; ++B) {                       // plain scan; the predicates below define the set
+          if (B == A || !steep(B)) continue;
+          const int b = tail[B];
+          if (trk_sector[b] != s_b) continue;
+          if (!(std::fabs(zo[B] - zo[A]) <= T(ac.dz_win))) continue;
+          T xcB, ycB, RB, cB;
+          centre(b, &xcB, &ycB, &RB, &cB);
+          if (!(cA * cB < T(0))) continue;                  // the returning leg is walked against the motion
+          // b's centre and end point in a's frame
+          const T xcB_a = xcB * ck - ycB * sd, ycB_a = xcB * sd + ycB * ck;
+          const T xB = T(up_x_ref[b]), yB = T(up_par[(size_t)b * 5 + 0]);
+          const T xB_a = xB * ck - yB * sd, yB_a = xB * sd + yB * ck;
+          const T Rm = T(0.5) * (RA + RB);
+          const T dcx = xcA - xcB_a, dcy = ycA - ycB_a;
+          const T dc2 = dcx * dcx + dcy * dcy;
+          const T ex = xB_a - xA, ey = yB_a - yA;
+          const T d = std::sqrt(ex * ex + ey * ey);
+          const T h = (T(0.5) * d) / Rm;                    // sine of half the turning angle between the two end points
+          if (!(h < T(0.98))) continue;
+          // arc = 2 Rm asin(h) = 4 Rm asin(h1), h1 = sine of a quarter of the turning angle; 5-term series of section 3.4.1
+          const T h1 = h / std::sqrt(T(2) * (T(1) + std::sqrt(T(1) - h * h)));
+          const T w = h1 * h1;
+          const T ser = T(1) + w * (T(1.0 / 6.0) + w * (T(3.0 / 40.0) + w * (T(5.0 / 112.0) + w * T(35.0 / 1152.0))));
+          const T arc = (T(4) * Rm) * (h1 * ser);
+          const T dz = zo[B] - (zo[A] + tA * arc);
+          const T dt = tA + T(up_par[(size_t)b * 5 + 3]);
+          const T tc = T(ac.tol_c) * Rm;
+          const T score = dc2 / (tc * tc) + (dz * dz) / (T(ac.tol_z) * T(ac.tol_z)) + (dt * dt) / (T(ac.tol_t) * T(ac.tol_t));
+          if (!(score <= T(ac.cut))) continue;
+          if (bb < 0 || score < best || (score == best && B < bb)) { best = score; bb = B; }
+        }
+      }
+      apx_best[A] = bb; apx_score[A] = bb >= 0 ? (double)best : -1.0;
+    }
+    for (int A = 0; A < nm; ++A) {
+      const int B = apx_best[A];
+      if (B >= 0 && apx_best[B] == A) apx_partner[A] = B;
+    }
+    // Which leg is the returning ("secondary") one: a primary moves away from the central electrode, so |z| grows along
+    // its motion - on the A side the leg whose apex-side end has the larger z comes later, on the C side the one with the
+    // smaller z (the time shift of continuous readout moves both ends alike).  Ties -> the higher id.
+    for (int A = 0; A < nm; ++A) {
+      const int B = apx_partner[A];
+      if (B < 0) continue;
+      const bool a_side = trk_sector[tail[A]] < n_az;
+      const bool later = a_side ? zo[A] > zo[B] : zo[A] < zo[B];
+      apx_leg[A] = (later || (zo[A] == zo[B] && A > B)) ? 1 : 0;
+    }
+  }
+
   // ---------------------------------------------------------------------------------------- S8
   // Cluster protection for hit removal, "strategy B": "runs only the online tracking and removes all hits not in the
   // vicinity of good tracks".  A cluster is protected iff it is attached to a track or
@@ -1006,6 +1114,7 @@ int orc_get(void* h, const char* name, const void** ptr, int64_t* n, int* kind) 
   I32(fit_row); F64(up_par); F64(up_cov); F64(up_x_ref); F64(up_z_ref); F64(up_chi2); I32(up_row); I32(up_n);
   I32(mrg_best_b); I32(mrg_best_a); I32(mrg_next); I32(mrg_prev); I32(mrg_dir); F64(mrg_chi2_b);
   I32(mrg_of_track); I32(mrg_seg_start); I32(mrg_seg_idx);
+  I32(apx_best); I32(apx_partner); I32(apx_leg); F64(apx_score);
   F64(mrg_par); F64(mrg_cov); F64(mrg_x_ref); F64(mrg_z_ref); F64(mrg_chi2); I32(mrg_n_fit); I32(mrg_ndf); I32(mrg_sector); I32(mrg_n_clusters);
   F32(up_dx); F32(up_ratio); F32(up_wy); F32(up_wz); F32(dn_dx); F32(dn_ratio); F32(dn_wy); F32(dn_wz);
 #undef I32
@@ -1050,6 +1159,13 @@ void orc_merge(void* h, int max_rows, int back_rows, float edge, float dz_win, f
   Oracle* o = reinterpret_cast<Oracle*>(h);
   const Oracle::MergeCuts mc{max_rows, back_rows, edge, dz_win, chi2_cut, road_z0, road_z1};
   if (o->s4_prec == 64) o->stage9<double>(mc); else o->stage9<float>(mc);
+}
+
+// apex links on the merged tracks of the last orc_merge
+void orc_apex(void* h, int max_k, float min_s, float dz_win, float tol_c, float tol_z, float tol_t, float cut) {
+  Oracle* o = reinterpret_cast<Oracle*>(h);
+  const Oracle::ApexCuts ac{max_k, min_s, dz_win, tol_c, tol_z, tol_t, cut};
+  if (o->s4_prec == 64) o->stage10<double>(ac); else o->stage10<float>(ac);
 }
 
 // one rotation of DESIGN.md section 3.9.2 (for the pins): par / cov15 in place, returns the new x or NaN on failure

@@ -8,7 +8,10 @@ the same shape.  This module produces them:
   x = 85 .. 245 cm (uniform pitch), Bz = 0.5 T, drift velocity 2.5 cm/us over
   250 cm (100 us drift window; BASELINE.json configs[2]; PAPER.md:29 says 90 us);
 * primary helices from (0, 0, z_v): phi0 ~ U[0, 2pi), charge +-1, tan(lambda)
-  ~ U[-0.9, 0.9], pT per config; first outgoing branch only (no loopers);
+  ~ U[-0.9, 0.9], pT per config; first outgoing branch only - with the recipe key
+  ``loopers=True`` also the RETURNING branch of tracks that curl up inside the TPC
+  (second intersection of the circle with every pad-row line, truth-labelled in
+  ``TimeFrame.leg``; PAPER.md:57, 107: "secondary legs of looping tracks");
 * one cluster per crossed (sector, row): exact circle / row-line intersection
   in double precision in the sector-local frame, Gaussian smearing in y and z;
 * continuous readout: the cluster z handed to the tracker is
@@ -79,6 +82,7 @@ class TimeFrame:
     tf_length_us: float = 0.0
     sigma: float = 0.1
     name: str = ""
+    leg: np.ndarray | None = None   # int8 [N]: 0 outgoing branch, 1 returning branch of a looper (recipe key `loopers`); truth
 
     @property
     def n(self) -> int:
@@ -94,6 +98,7 @@ _STREAM_COLLISIONS = 0
 _STREAM_NOISE = 1
 _STREAM_TRACKS = 2
 _STREAM_SMEAR0 = 1000
+_STREAM_SMEAR_RET0 = 2_000_000   # smear normals of the returning branches (recipe key `loopers`)
 _SMEAR_CHUNK = 8192  # tracks per smear stream; fixed, part of the recipe
 
 
@@ -187,7 +192,7 @@ def generate(rec: dict, geometry: Geometry | None = None, device: str = "cpu") -
     # big chunks on a GPU, cache-sized on the host; always a multiple of the smear-stream size
     chunk = _SMEAR_CHUNK * (16 if dev.type == "cuda" else 1)
 
-    out_sector, out_row, out_y, out_z, out_tid = [], [], [], [], []
+    out_sector, out_row, out_y, out_z, out_tid, out_leg = [], [], [], [], [], []
     for c0 in range(0, n_tot, chunk):
         c1 = min(n_tot, c0 + chunk)
         m = c1 - c0
@@ -237,10 +242,49 @@ def generate(rec: dict, geometry: Geometry | None = None, device: str = "cpu") -
         out_y.append(ysm[ok].to(torch.float32).cpu())
         out_z.append(zps[ok].to(torch.float32).cpu())
         out_tid.append(tids[ok].to(torch.int32).cpu())
+        out_leg.append(torch.zeros(int(ok.sum()), dtype=torch.int8))
+        if rec.get("loopers", False):
+            # the returning branch: the circle through the origin meets the row line x = X of a sector frame a second
+            # time, with cos(phi) < 0 (the particle comes back inwards), at y = (c_0 + c_1) / c, after the turning angle
+            # 2 (pi - asin|u|) for the chord u = c chord / 2.  Its azimuth at radius rho is phi0 + sgn(c) pi - asin(u).
+            sgn = torch.sign(cv)
+            az_r = p0 + sgn * math.pi - torch.asin(u_probe.clamp(-1.0, 1.0))
+            a_r = torch.remainder(torch.floor(az_r / sect_w).to(torch.int64) + cand_off[None, None, :], n_az)
+            alpha_r = (a_r.to(f64) + 0.5) * sect_w
+            ploc_r = torch.remainder(p0 - alpha_r + math.pi, 2.0 * math.pi) - math.pi
+            s_0r = torch.sin(ploc_r); c_0r = torch.cos(ploc_r)
+            s_1r = s_0r + cv * X
+            ok_r = reach & (cv != 0) & (s_1r.abs() < 0.95)
+            c_1r = torch.sqrt((1.0 - s_1r * s_1r).clamp_min(0.0))
+            cvs = torch.where(cv == 0, torch.ones_like(cv), cv)
+            y_r = (c_0r + c_1r) / cvs
+            chord_r = torch.sqrt(X * X + y_r * y_r)
+            u_r = (0.5 * cvs.abs() * chord_r).clamp(0.0, 1.0)
+            arc_r = 2.0 * (math.pi - torch.asin(u_r)) / cvs.abs()
+            z_r = zv + tl * arc_r
+            ok_r &= (y_r.abs() <= ymax[None, :, None]) & (z_r.abs() < g.drift_length)
+            c_side_r = z_r < 0
+            sec_r = a_r + c_side_r.to(torch.int64) * n_az
+            n1r = np.empty((m, g.n_rows)); n2r = np.empty((m, g.n_rows))
+            for s0 in range(c0, c1, _SMEAR_CHUNK):
+                s1 = min(c1, s0 + _SMEAR_CHUNK)
+                nn = _rng(seed, _STREAM_SMEAR_RET0 + s0 // _SMEAR_CHUNK).standard_normal((s1 - s0, g.n_rows, 2))
+                n1r[s0 - c0:s1 - c0] = nn[..., 0]
+                n2r[s0 - c0:s1 - c0] = nn[..., 1]
+            ysm_r = y_r + sigma * T(n1r)[:, :, None]
+            zsm_r = z_r + sigma * T(n2r)[:, :, None]
+            zps_r = torch.where(c_side_r, zsm_r + g.v_drift * tc, zsm_r - g.v_drift * tc)
+            out_sector.append(sec_r[ok_r].to(torch.uint8).cpu())
+            out_row.append(rows[ok_r].to(torch.uint8).cpu())
+            out_y.append(ysm_r[ok_r].to(torch.float32).cpu())
+            out_z.append(zps_r[ok_r].to(torch.float32).cpu())
+            out_tid.append(tids[ok_r].to(torch.int32).cpu())
+            out_leg.append(torch.ones(int(ok_r.sum()), dtype=torch.int8))
 
     cat = lambda lst, dt: (torch.cat(lst).numpy() if lst else np.empty(0, dt))  # noqa: E731
     sector = cat(out_sector, np.uint8); row = cat(out_row, np.uint8)
     yy = cat(out_y, np.float32); zz = cat(out_z, np.float32); tid = cat(out_tid, np.int32)
+    leg = cat(out_leg, np.int8)
 
     # ---- noise clusters
     n_sig = sector.shape[0]
@@ -264,11 +308,12 @@ def generate(rec: dict, geometry: Geometry | None = None, device: str = "cpu") -
         yy = np.concatenate([yy, ny.astype(np.float32)])
         zz = np.concatenate([zz, nz.astype(np.float32)])
         tid = np.concatenate([tid, np.full(n_noise, -1, np.int32)])
+        leg = np.concatenate([leg, np.zeros(n_noise, np.int8)])
 
     x = g.row_x().astype(np.float32)[row]
     truth = dict(q_over_pt=qpt, tanl=tanl, phi0=phi0, z_v=trk_zv, t_coll=trk_t, collision=coll_of)
     return TimeFrame(sector=sector, row=row, x=x, y=yy, z=zz, track_id=tid, truth=truth, geometry=g,
-                     tf_length_us=float(rec["tf_us"]), sigma=sigma)
+                     tf_length_us=float(rec["tf_us"]), sigma=sigma, leg=leg)
 
 
 # --------------------------------------------------------------- harness rules
@@ -319,7 +364,7 @@ def to_native_time(tf: TimeFrame, time_unit_us: float = 0.2) -> tuple[TimeFrame,
     side = np.where(tf.sector < g.n_azimuthal, 1.0, -1.0)
     t = (g.drift_length - side * tf.z.astype(np.float64)) / (g.v_drift * float(time_unit_us))
     out = TimeFrame(sector=tf.sector, row=tf.row, x=tf.x, y=tf.y, z=t.astype(np.float32), track_id=tf.track_id,
-                    truth=tf.truth, geometry=g, tf_length_us=tf.tf_length_us, sigma=tf.sigma, name=tf.name + "+time")
+                    truth=tf.truth, geometry=g, tf_length_us=tf.tf_length_us, sigma=tf.sigma, name=tf.name + "+time", leg=tf.leg)
     return out, dict(z_is_time=1, cm_per_time_unit=np.float32(g.v_drift * float(time_unit_us)),
                      drift_length=np.float32(g.drift_length))
 
@@ -330,5 +375,6 @@ def select_sectors(tf: TimeFrame, sectors) -> tuple[TimeFrame, np.ndarray]:
     idx = np.nonzero(keep)[0]
     sub = TimeFrame(sector=tf.sector[idx], row=tf.row[idx], x=tf.x[idx], y=tf.y[idx], z=tf.z[idx],
                     track_id=tf.track_id[idx], truth=tf.truth, geometry=tf.geometry,
-                    tf_length_us=tf.tf_length_us, sigma=tf.sigma, name=tf.name + f"[sectors {list(sectors)}]")
+                    tf_length_us=tf.tf_length_us, sigma=tf.sigma, name=tf.name + f"[sectors {list(sectors)}]",
+                    leg=None if tf.leg is None else tf.leg[idx])
     return sub, idx
