@@ -476,7 +476,16 @@ def run_ours(args):
     torch.cuda.synchronize(dev)
     merge_ms = ev0.elapsed_time(ev1)
     n_merged = int(mg_buf["n_merged"].item())
-    del mg_buf
+    # ---- looper following (separate call after the merge)
+    ax_buf = trk.new_apex()
+    trk.apex_into(mg_buf, ax_buf)
+    ev0.record(stream)
+    trk.apex_into(mg_buf, ax_buf)
+    ev1.record(stream)
+    torch.cuda.synchronize(dev)
+    apex_ms = ev0.elapsed_time(ev1)
+    n_apex = int((ax_buf["apex_partner"][:n_merged] >= 0).sum().item()) // 2
+    del mg_buf, ax_buf
     # ---- cluster protection for hit removal, strategy B (separate call), 1 cm road
     keep = trk.protect(out, 1.0, 1.0)
     ev0.record(stream)
@@ -564,6 +573,8 @@ def run_ours(args):
                   "ms": refit_ms},
         "merge": {"what": "tpc_tracker_merge (separate call after the refit, not in the step): segments joined across sector "
                           "borders and long holes, upward + merged downward refit", "ms": merge_ms, "n_merged": n_merged},
+        "apex": {"what": "tpc_tracker_apex (separate call after the merge, not in the step): looper legs paired through their "
+                         "circles, returning leg labelled", "ms": apex_ms, "pairs": n_apex},
         "protect": {"what": "tpc_tracker_protect (separate call, not in the step): strategy-B keep flag per cluster, 1 cm road",
                     "ms": protect_ms, "kept_fraction": kept_frac},
         "roofline": roofline,

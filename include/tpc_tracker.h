@@ -200,7 +200,9 @@ enum tpc_stage_array {
   TPC_VIEW_MRG_NEXT = 35,   /* int32 [n_tracks] link to the next segment outwards or -1 (3.9.6) */
   TPC_VIEW_MRG_PREV = 36,   /* int32 [n_tracks] */
   TPC_VIEW_MRG_DIR = 37,    /* int32 [n_tracks] 0 same sector, +-1 the neighbour the link goes to */
-  TPC_VIEW_COUNT_ = 38
+  TPC_VIEW_APEX_BEST = 38,  /* int32 [max_tracks] best apex partner of every merged track or -1 (3.9.8); first n_merged valid */
+  TPC_VIEW_APEX_SCORE = 39, /* float [max_tracks] its score or -1 */
+  TPC_VIEW_COUNT_ = 40
 };
 
 typedef struct {
@@ -308,6 +310,31 @@ typedef struct {
  * INVALID_ARG for null pointers or cuts out of range, CAPACITY if a max_tracks exceeds the tracker's. */
 TPC_API int tpc_tracker_merge(tpc_tracker_t* t, const tpc_fit_t* fit, const tpc_merge_cuts_t* cuts, const tpc_merged_t* out,
                               void* cuda_stream);
+
+/* Cuts of the apex links. */
+typedef struct {
+  int32_t max_k;   /* sectors the unseen arc around the apex may span (4) */
+  float min_s;     /* a tail takes part iff |sin(phi)| of its outer state >= min_s (0.6) */
+  float dz_win;    /* cm: |z_out(B) - z_out(A)| window (150); > 0 */
+  float tol_c;     /* tolerance of the circle centres, as a fraction of the radius (0.1); > 0 */
+  float tol_z;     /* cm: tolerance of the z advance along the arc between the two ends (4); > 0 */
+  float tol_t;     /* tolerance of tan(lambda)_A + tan(lambda)_B (0.1); > 0 */
+  float cut;       /* partners need score <= cut (3) */
+} tpc_apex_cuts_t;
+
+typedef struct {
+  int64_t max_tracks;
+  int32_t* apex_partner;  /* [max_tracks] per merged track: the merged track that is the other leg of the same looper, or -1 */
+  int32_t* apex_leg;      /* [max_tracks] 1 = the returning ("secondary") leg of its pair, else 0 */
+} tpc_apex_t;
+
+/* Looper following ("secondary legs of looping tracks", "the following
+ * of looping tracks"): pairs the merged tracks of the LAST tpc_tracker_merge call on this handle that are the outgoing
+ * and the returning leg of one track curling up inside the TPC, by comparing the circles of their outermost states, and
+ * labels the returning leg.  `merged` is that call's output (DEVICE; seg_start / seg_idx are read).  Enqueued on
+ * `cuda_stream`, ordered after the merge; does not synchronise; entries [0, n_merged) are written. */
+TPC_API int tpc_tracker_apex(tpc_tracker_t* t, const tpc_merged_t* merged, const tpc_apex_cuts_t* cuts, const tpc_apex_t* out,
+                             void* cuda_stream);
 
 /* Cluster protection for hit removal, "strategy B", for the LAST
  * tpc_track_timeframe call on this handle: keep[i] = 1 iff input cluster i is attached to a track or lies, in its own

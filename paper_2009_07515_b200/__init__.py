@@ -5,6 +5,7 @@ marshals arguments.  Nothing here imports ``oracle/``.
 """
 from .binding import (  # noqa: F401
     EXPORTS,
+    APEX_CUTS,
     MERGE_CUTS,
     STATUS_BITS,
     Tracker,

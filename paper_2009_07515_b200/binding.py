@@ -66,6 +66,16 @@ class tpc_merged_t(C.Structure):
     _fields_ = [("max_tracks", C.c_int64)] + [(f, C.c_void_p) for f in _MERGED_FIELDS]
 
 
+class tpc_apex_cuts_t(C.Structure):
+    _fields_ = [("max_k", C.c_int32), ("min_s", C.c_float), ("dz_win", C.c_float), ("tol_c", C.c_float), ("tol_z", C.c_float),
+                ("tol_t", C.c_float), ("cut", C.c_float)]
+
+
+class tpc_apex_t(C.Structure):
+    _fields_ = [("max_tracks", C.c_int64), ("apex_partner", C.c_void_p), ("apex_leg", C.c_void_p)]
+
+
+APEX_CUTS = dict(max_k=4, min_s=0.6, dz_win=150.0, tol_c=0.1, tol_z=4.0, tol_t=0.1, cut=3.0)
 MERGE_CUTS = dict(max_rows=30, back_rows=1, edge=6.0, dz_win=50.0, chi2_cut=100.0, road_z0=2.0, road_z1=0.3)
 
 
@@ -85,13 +95,13 @@ VIEWS = {name: i for i, name in enumerate([
     "t_hit", "t_first_row", "t_last_row", "t_n_hits", "t_par", "t_cov", "t_chi2", "t_zref",
     "tracklet_of_seed", "k_owned",
     "fit_row", "up_par", "up_cov", "up_x", "up_zref", "up_row", "up_n",
-    "mrg_best_b", "mrg_best_a", "mrg_chi_b", "mrg_next", "mrg_prev", "mrg_dir"])}
+    "mrg_best_b", "mrg_best_a", "mrg_chi_b", "mrg_next", "mrg_prev", "mrg_dir", "apex_best", "apex_score"])}
 
 STATUS_BITS = {1: "BAD_CLUSTER", 2: "BINS_OVERFLOW", 4: "SEEDS_OVERFLOW", 8: "TRACKS_OVERFLOW", 16: "CHAIN_CYCLE"}
 
 EXPORTS = [
     "tpc_tracker_workspace_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
-    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit", "tpc_tracker_merge", "tpc_tracker_protect",
+    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit", "tpc_tracker_merge", "tpc_tracker_apex", "tpc_tracker_protect",
     "tpc_tracker_counters", "tpc_tracker_enable_stage_timing", "tpc_tracker_stage_ms", "tpc_tracker_stage_view",
     "tpc_tracker_launches_per_call", "tpc_tracker_destroy", "tpc_error_string",
 ]
@@ -136,6 +146,8 @@ def load_library(build: bool = True) -> C.CDLL:
     lib.tpc_tracker_refit.argtypes = [C.c_void_p, P(tpc_fit_t), C.c_void_p]
     lib.tpc_tracker_merge.restype = C.c_int
     lib.tpc_tracker_merge.argtypes = [C.c_void_p, P(tpc_fit_t), P(tpc_merge_cuts_t), P(tpc_merged_t), C.c_void_p]
+    lib.tpc_tracker_apex.restype = C.c_int
+    lib.tpc_tracker_apex.argtypes = [C.c_void_p, P(tpc_merged_t), P(tpc_apex_cuts_t), P(tpc_apex_t), C.c_void_p]
     lib.tpc_tracker_protect.restype = C.c_int
     lib.tpc_tracker_protect.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
     lib.tpc_tracker_counters.restype = C.c_int
@@ -376,15 +388,43 @@ class Tracker:
         _check(self.lib, self.lib.tpc_tracker_merge(self._h, C.byref(f), C.byref(c), C.byref(m), C.c_void_p(st.cuda_stream)),
                "tpc_tracker_merge")
 
-    def merge(self, n_tracks: int, cuts: dict | None = None) -> dict:
-        """Convenience: refit + merge + host copies trimmed to the tracks / merged tracks found."""
+    def apex_into(self, merged: dict, out: dict, cuts: dict | None = None, stream=None):
+        """Enqueues tpc_tracker_apex for the merged tracks of the last merge_into call (does not synchronise);
+        `out` = dict(apex_partner=int32[max_tracks], apex_leg=int32[max_tracks]) on the device."""
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        m = tpc_merged_t()
+        m.max_tracks = self.caps[3]
+        for k in _MERGED_FIELDS:
+            setattr(m, k, merged[k].data_ptr())
+        kw = dict(APEX_CUTS); kw.update(cuts or {})
+        c = tpc_apex_cuts_t(int(kw["max_k"]), float(kw["min_s"]), float(kw["dz_win"]), float(kw["tol_c"]), float(kw["tol_z"]),
+                            float(kw["tol_t"]), float(kw["cut"]))
+        o = tpc_apex_t()
+        o.max_tracks = self.caps[3]
+        o.apex_partner = out["apex_partner"].data_ptr(); o.apex_leg = out["apex_leg"].data_ptr()
+        _check(self.lib, self.lib.tpc_tracker_apex(self._h, C.byref(m), C.byref(c), C.byref(o), C.c_void_p(st.cuda_stream)),
+               "tpc_tracker_apex")
+
+    def new_apex(self) -> dict:
+        mt, dev = self.caps[3], self.device
+        return dict(apex_partner=torch.zeros(mt, dtype=torch.int32, device=dev), apex_leg=torch.zeros(mt, dtype=torch.int32, device=dev))
+
+    def merge(self, n_tracks: int, cuts: dict | None = None, apex: dict | bool | None = None) -> dict:
+        """Convenience: refit + merge (+ apex links when `apex` is True or a dict of cuts) + host copies trimmed to the
+        tracks / merged tracks found."""
         fit = self.new_fit(); mg = self.new_merged()
         self.refit_into(fit)
         self.merge_into(fit, mg, cuts)
+        extra = {}
+        if apex:
+            ax = self.new_apex()
+            self.apex_into(mg, ax, apex if isinstance(apex, dict) else None)
         torch.cuda.synchronize(self.device)
         T = int(n_tracks); M = int(mg["n_merged"].item())
+        if apex:
+            extra = dict(apex_partner=ax["apex_partner"].cpu().numpy()[:M].copy(), apex_leg=ax["apex_leg"].cpu().numpy()[:M].copy())
         h = {k: v.cpu().numpy() for k, v in mg.items()}
-        return dict(n_merged=M, merged_of_track=h["merged_of_track"][:T].copy(), seg_start=h["seg_start"][:M + 1].copy(),
+        return dict(**extra, n_merged=M, merged_of_track=h["merged_of_track"][:T].copy(), seg_start=h["seg_start"][:M + 1].copy(),
                     seg_idx=h["seg_idx"][:T].copy(), par=h["par"][:, :M].T.copy(), cov=h["cov"][:, :M].T.copy(),
                     **{k: h[k][:M].copy() for k in ("x_ref", "z_ref", "chi2", "ndf", "n_fit", "sector", "n_clusters")})
 

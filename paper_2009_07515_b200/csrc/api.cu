@@ -117,6 +117,8 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   c.m_best_a = cv.take<unsigned long long>(T);
   c.m_next = cv.take<int>(T); c.m_prev = cv.take<int>(T); c.m_dir = cv.take<int>(T);
   c.m_head_scan = cv.take<int>(T); c.m_seg_scan = cv.take<int>(T); c.m_head_of = cv.take<int>(T);
+  c.a_c4 = cv.take<float4>(T); c.a_p4 = cv.take<float4>(T); c.a_sector = cv.take<int>(T); c.a_best = cv.take<int>(T);
+  c.a_score = cv.take<float>(T);
   c.mcnt = cv.take<MergeCounters>(1);
   for (int k = 0; k < t->host_io; ++k) {
     const size_t TC = (size_t)t->max_track_clusters;
@@ -464,6 +466,28 @@ int tpc_tracker_merge(tpc_tracker_t* t, const tpc_fit_t* fit, const tpc_merge_cu
   return launch_merge(t->ctx, f, o, st) ? TPC_ERR_CUDA : TPC_OK;
 }
 
+int tpc_tracker_apex(tpc_tracker_t* t, const tpc_merged_t* merged, const tpc_apex_cuts_t* cuts, const tpc_apex_t* out,
+                     void* cuda_stream) {
+  if (!t || !merged || !cuts || !out || !merged->seg_start || !merged->seg_idx || !out->apex_partner || !out->apex_leg)
+    return TPC_ERR_INVALID_ARG;
+  if (cuts->max_k < 0 || !(cuts->min_s >= 0.f) || !(cuts->dz_win > 0.f) || !(cuts->dz_win < INFINITY) || !(cuts->tol_c > 0.f) ||
+      !(cuts->tol_z > 0.f) || !(cuts->tol_t > 0.f) || !(cuts->cut >= 0.f))
+    return TPC_ERR_INVALID_ARG;
+  if (out->max_tracks < 1 || out->max_tracks > t->max_tracks || merged->max_tracks > t->max_tracks) return TPC_ERR_CAPACITY;
+  MergePtrs m{};
+  const float th = t->params.tan_half_sector;
+  const float den = 1.0f + th * th;
+  m.sin_a = (2.0f * th) / den; m.cos_a = (1.0f - th * th) / den;
+  m.seg_start = merged->seg_start; m.seg_idx = merged->seg_idx; m.max_tracks = (int)merged->max_tracks;
+  ApexPtrs o{};
+  o.max_k = cuts->max_k; o.min_s = cuts->min_s; o.dz_win = cuts->dz_win; o.tol_c = cuts->tol_c; o.tol_z = cuts->tol_z;
+  o.tol_t = cuts->tol_t; o.cut = cuts->cut;
+  o.apex_partner = out->apex_partner; o.apex_leg = out->apex_leg; o.max_tracks = (int)out->max_tracks;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  t->last_stream = st;
+  return launch_apex(t->ctx, m, o, st) ? TPC_ERR_CUDA : TPC_OK;
+}
+
 int tpc_tracker_protect(tpc_tracker_t* t, const int32_t* cluster_track, float road_y, float road_z, uint8_t* keep,
                         void* cuda_stream) {
   if (!t || !keep || !cluster_track || !(road_y >= 0.f) || !(road_z >= 0.f)) return TPC_ERR_INVALID_ARG;
@@ -546,6 +570,8 @@ int tpc_tracker_stage_view(tpc_tracker_t* t, int32_t which, tpc_stage_view_t* ou
     case TPC_VIEW_MRG_NEXT: set(c.m_next, k.n_tracks, 4, 0); break;
     case TPC_VIEW_MRG_PREV: set(c.m_prev, k.n_tracks, 4, 0); break;
     case TPC_VIEW_MRG_DIR: set(c.m_dir, k.n_tracks, 4, 0); break;
+    case TPC_VIEW_APEX_BEST: set(c.a_best, c.max_tracks, 4, 0); break;
+    case TPC_VIEW_APEX_SCORE: set(c.a_score, c.max_tracks, 4, 1); break;
     default: return TPC_ERR_INVALID_ARG;
   }
   return TPC_OK;

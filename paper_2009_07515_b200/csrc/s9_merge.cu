@@ -112,12 +112,13 @@ struct OwnedRowsDown {
 __device__ __forceinline__ int n_tracks_of(const Ctx& c, const MergePtrs& o) { return min(c.cnt->n_tracks, o.max_tracks); }
 
 // ---------------------------------------------------------------------------------- z grid of the inner ends
-__global__ void k_merge_tables(Ctx c, MergePtrs o) {
+__global__ void k_merge_tables(Ctx c, float w0, int new_merge) {
   if (threadIdx.x || blockIdx.x) return;
   MergeCounters& mc = *c.mcnt;
-  mc.n_merged = 0; mc.status = 0;
+  if (new_merge) mc.n_merged = 0;
+  mc.status = 0;
   // bins a quarter of the window wide: a query reads 9-10 bins, 1.25 x the window instead of 3 x with bins of dz_win
-  float w = o.dz_win * 0.25f;
+  float w = w0;
   for (int it = 0; it < 64; ++it, w = w * 2.0f) {
     const float inv_w = 1.0f / w;
     long long acc = 0;
@@ -438,6 +439,148 @@ __global__ void __launch_bounds__(kThreads) k_refit_merged(Ctx c, MergePtrs o) {
   }
 }
 
+
+// ---------------------------------------------------------------------------------- 3.9.8 apex links (looper following)
+// k_apex_prep   thread per merged track: its tail's circle (centre, radius, curvature), end point, dip, z_out; the steep
+//               ones are counted into (sector, z_out) bins
+// k_apex_fill   counting sort of 16-byte records (z_out, id, tan(lambda), curvature): what the cheap cuts need
+// k_apex_match  warp per tail: the sectors the track curls through, the window's run of records read together, exact
+//               pre-cuts (z window, curvature signs, the dip term alone above the cut), score, lane-local best, warp reduction
+// k_apex_link   mutual best -> partners; secondary-leg label
+__global__ void __launch_bounds__(kThreads) k_apex_prep(Ctx c, MergePtrs m, ApexPtrs o) {
+  const int nm = c.mcnt->n_merged;
+  const float inv_w = c.mcnt->inv_w;
+  const size_t mt = (size_t)c.max_tracks;
+  for (int A = blockIdx.x * blockDim.x + threadIdx.x; A < nm; A += gridDim.x * blockDim.x) {
+    const int t = m.seg_idx[m.seg_start[A + 1] - 1];
+    const float x = c.up_x[t], y = c.up_par[0 * mt + t], s = c.up_par[2 * mt + t], tl = c.up_par[3 * mt + t];
+    const float cv = c.kb * c.up_par[4 * mt + t];
+    const float zo = c.up_zref[t] + c.up_par[1 * mt + t];
+    const int sector = c.m_sector[t];
+    const bool steep = c.up_n[t] >= 2 && fabsf(s) >= o.min_s && fabsf(s) < 1.0f && cv != 0.0f;
+    float xc = 0.f, yc = 0.f, R = 0.f;
+    if (steep) {
+      xc = x - s / cv;
+      yc = y + sqrtf(1.0f - s * s) / cv;
+      R = 1.0f / fabsf(cv);
+    }
+    c.a_c4[A] = make_float4(xc, yc, R, cv);
+    c.a_p4[A] = make_float4(x, y, tl, zo);
+    c.a_sector[A] = steep ? (sector | (s >= 0.0f ? 0x100 : 0)) : -1;     // bit 8: curls to +y
+    c.a_best[A] = -1; c.a_score[A] = -1.0f;
+    o.apex_partner[A] = -1; o.apex_leg[A] = 0;
+    int b = -1;
+    if (steep && c.m_nzb[sector] > 0) {
+      b = merge_bin(c, sector, zo, inv_w);
+      atomicAdd(c.m_bin_start + b + 1, 1);
+    }
+    c.m_bin_of[A] = b;
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_apex_clear(Ctx c) {
+  const int nb = c.mcnt->n_bins;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i <= nb; i += gridDim.x * blockDim.x) {
+    c.m_bin_start[i] = 0;
+    if (i < nb) c.m_bin_fill[i] = 0;
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_apex_fill(Ctx c) {
+  const int nm = c.mcnt->n_merged;
+  for (int A = blockIdx.x * blockDim.x + threadIdx.x; A < nm; A += gridDim.x * blockDim.x) {
+    const int b = c.m_bin_of[A];
+    if (b < 0) continue;
+    const int pos = c.m_bin_start[b] + atomicAdd(c.m_bin_fill + b, 1);
+    const float4 p = c.a_p4[A];
+    c.m_srec[pos] = make_float4(p.w, __int_as_float(A), p.z, c.a_c4[A].w);
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_apex_match(Ctx c, MergePtrs m, ApexPtrs o) {
+  const int nm = c.mcnt->n_merged, n_az = c.S >> 1;
+  const float inv_w = c.mcnt->inv_w;
+  const int lane = threadIdx.x & 31;
+  const int warps = (gridDim.x * blockDim.x) >> 5;
+  const float tz2 = o.tol_z * o.tol_z, tt2 = o.tol_t * o.tol_t;
+  for (int A = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; A < nm; A += warps) {
+    const int sa = c.a_sector[A];
+    if (sa < 0) continue;                                 // warp-uniform
+    const int s_a = sa & 0xFF, dirA = (sa & 0x100) ? 1 : -1;
+    const float4 cA = c.a_c4[A], pA = c.a_p4[A];          // (xc, yc, R, c), (x, y, t, z_out)
+    const float zlo = pA.w - o.dz_win, zhi = pA.w + o.dz_win;
+    float best = 0.f;
+    int bb = -1;
+    float sk = 0.0f, ck = 1.0f;
+    for (int k = 0; k <= o.max_k; ++k) {
+      if (k > 0) {
+        const float s2 = sk * m.cos_a + ck * m.sin_a, c2 = ck * m.cos_a - sk * m.sin_a;
+        sk = s2; ck = c2;
+      }
+      const int s_b = (s_a / n_az) * n_az + ((((s_a % n_az) + dirA * k) % n_az) + n_az) % n_az;
+      if (k > 0 && s_b == s_a) break;
+      if (c.m_nzb[s_b] == 0) continue;
+      const float sd = dirA > 0 ? sk : 0.0f - sk;
+      // |z_out(B) - z_out(A)| <= dz_win: the bins of [zlo, zhi] hold every such B (monotone clamped floor); the
+      // predicate itself is applied below with the written expression
+      // (one more bin on either side: zlo / zhi are rounded sums, the predicate below is a rounded difference)
+      const int base = c.m_bin_base[s_b];
+      const int b0 = max(base, merge_bin(c, s_b, zlo, inv_w) - 1), b1 = min(base + c.m_nzb[s_b] - 1, merge_bin(c, s_b, zhi, inv_w) + 1);
+      const int j0 = c.m_bin_start[b0], j1 = c.m_bin_start[b1 + 1];
+      for (int j = j0 + lane; j < j1; j += 32) {
+        const float4 rec = __ldg(c.m_srec + j);           // (z_out, id, tan(lambda), curvature)
+        const int B = __float_as_int(rec.y);
+        if (B == A) continue;
+        if (!(fabsf(rec.x - pA.w) <= o.dz_win)) continue;
+        if (!(cA.w * rec.w < 0.0f)) continue;
+        const float dt = pA.z + rec.z;
+        const float term_t = (dt * dt) / tt2;
+        if (!(term_t <= o.cut)) continue;                 // exact pre-cut: the other two terms are >= 0 and rounding is monotone
+        const float4 cB = c.a_c4[B], pB = c.a_p4[B];
+        const float xcB = cB.x * ck - cB.y * sd, ycB = cB.x * sd + cB.y * ck;
+        const float xB = pB.x * ck - pB.y * sd, yB = pB.x * sd + pB.y * ck;
+        const float Rm = 0.5f * (cA.z + cB.z);
+        const float dcx = cA.x - xcB, dcy = cA.y - ycB;
+        const float dc2 = dcx * dcx + dcy * dcy;
+        const float ex = xB - pA.x, ey = yB - pA.y;
+        const float d = sqrtf(ex * ex + ey * ey);
+        const float h = (0.5f * d) / Rm;
+        if (!(h < 0.98f)) continue;
+        const float h1 = h / sqrtf(2.0f * (1.0f + sqrtf(1.0f - h * h)));
+        const float w = h1 * h1;
+        const float ser = 1.0f + w * ((float)(1.0 / 6.0) + w * ((float)(3.0 / 40.0) + w * ((float)(5.0 / 112.0) + w * (float)(35.0 / 1152.0))));
+        const float arc = (4.0f * Rm) * (h1 * ser);
+        const float dz = rec.x - (pA.w + pA.z * arc);
+        const float tc = o.tol_c * Rm;
+        const float score = dc2 / (tc * tc) + (dz * dz) / tz2 + term_t;
+        if (!(score <= o.cut)) continue;
+        if (bb < 0 || score < best || (score == best && B < bb)) { best = score; bb = B; }
+      }
+    }
+    __syncwarp();
+#pragma unroll
+    for (int off = 16; off; off >>= 1) {
+      const float os = __shfl_xor_sync(0xffffffffu, best, off);
+      const int ob = __shfl_xor_sync(0xffffffffu, bb, off);
+      if (ob >= 0 && (bb < 0 || os < best || (os == best && ob < bb))) { best = os; bb = ob; }
+    }
+    if (lane == 0) { c.a_best[A] = bb; c.a_score[A] = bb >= 0 ? best : -1.0f; }
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_apex_link(Ctx c, ApexPtrs o) {
+  const int nm = c.mcnt->n_merged, n_az = c.S >> 1;
+  for (int A = blockIdx.x * blockDim.x + threadIdx.x; A < nm; A += gridDim.x * blockDim.x) {
+    const int B = c.a_best[A];
+    if (B < 0 || c.a_best[B] != A) continue;
+    o.apex_partner[A] = B;
+    const float zA = c.a_p4[A].w, zB = c.a_p4[B].w;
+    const bool a_side = (c.a_sector[A] & 0xFF) < n_az;
+    const bool later = a_side ? zA > zB : zA < zB;
+    o.apex_leg[A] = (later || (zA == zB && A > B)) ? 1 : 0;
+  }
+}
+
 unsigned grid_for(long long n, const Ctx& c, int per_sm) {
   long long g = (n + kThreads - 1) / kThreads;
   const long long cap = (long long)c.n_sms * per_sm;
@@ -452,7 +595,7 @@ int launches_merge() { return 12 + 6; }
 int launch_merge(const Ctx& c, const FitPtrs& f, const MergePtrs& o, cudaStream_t st) {
   const unsigned gt = grid_for(c.max_tracks, c, 64), gb = grid_for(c.max_merge_bins, c, 16);
   const size_t sh = c.R * sizeof(float);
-  k_merge_tables<<<1, 32, 0, st>>>(c, o);
+  k_merge_tables<<<1, 32, 0, st>>>(c, o.dz_win * 0.25f, 1);
   k_merge_clear<<<gt > gb ? gt : gb, kThreads, 0, st>>>(c, o);
   k_refit_up<<<gt, kThreads, sh, st>>>(c, f, o);
   // CSR starts of the (sector, z) bins: inclusive scan of the counts written at b + 1 (entry 0 stays 0)
@@ -467,6 +610,19 @@ int launch_merge(const Ctx& c, const FitPtrs& f, const MergePtrs& o, cudaStream_
   if (launch_scan_inclusive(c.m_seg_scan, &c.mcnt->n_merged, 0, c.max_tracks, c.tile_sums, nullptr, c.n_sms, st)) return -1;
   k_chain_fill<<<gt, kThreads, 0, st>>>(c, o);
   k_refit_merged<<<gt, kThreads, sh, st>>>(c, o);
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+int launches_apex() { return 6 + 3; }
+int launch_apex(const Ctx& c, const MergePtrs& m, const ApexPtrs& o, cudaStream_t st) {
+  const unsigned gt = grid_for(c.max_tracks, c, 64), gb = grid_for(c.max_merge_bins, c, 16);
+  k_merge_tables<<<1, 32, 0, st>>>(c, o.dz_win * 0.25f, 0);   // n_merged of the merge call stays
+  k_apex_clear<<<gb, kThreads, 0, st>>>(c);
+  k_apex_prep<<<gt, kThreads, 0, st>>>(c, m, o);
+  if (launch_scan_inclusive(c.m_bin_start, &c.mcnt->n_bins, 1, (long long)c.max_merge_bins + 1, c.tile_sums, nullptr, c.n_sms, st)) return -1;
+  k_apex_fill<<<gt, kThreads, 0, st>>>(c);
+  k_apex_match<<<grid_for((long long)c.max_tracks * 32, c, 64), kThreads, 0, st>>>(c, m, o);
+  k_apex_link<<<gt, kThreads, 0, st>>>(c, o);
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 

@@ -109,6 +109,7 @@ struct Ctx {
   int* m_best_b; float* m_chi_b; int* m_dir_b; unsigned long long* m_best_a;
   int* m_next; int* m_prev; int* m_dir;
   int* m_head_scan; int* m_seg_scan; int* m_head_of;
+  float4* a_c4; float4* a_p4; int* a_sector; int* a_best; float* a_score;   // apex links (3.9.8), per merged track
   MergeCounters* mcnt;
   Counters* cnt;
   int n_sms;
@@ -143,6 +144,13 @@ struct MergePtrs {                    // S9: cuts + the caller's outputs
 };
 int launch_merge(const Ctx& c, const FitPtrs& f, const MergePtrs& o, cudaStream_t st);   // S9, separate call
 int launches_merge();
+struct ApexPtrs {                     // apex links: cuts + the caller's outputs
+  int max_k; float min_s, dz_win, tol_c, tol_z, tol_t, cut;
+  int* apex_partner; int* apex_leg;
+  int max_tracks;
+};
+int launch_apex(const Ctx& c, const MergePtrs& m, const ApexPtrs& o, cudaStream_t st);
+int launches_apex();
 int launch_protect(const Ctx& c, const int* cluster_track, float road_y, float road_z, unsigned char* keep, cudaStream_t st);   // S8
 
 // In-place inclusive scan of data[0 .. *n_ptr + n_add) (int32), length known only on the device.

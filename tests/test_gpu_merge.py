@@ -139,3 +139,44 @@ def test_merge_rejects_bad_arguments(cfg1):
     trk.merge_into(fit, mg)
     torch.cuda.synchronize()
     assert int(mg["n_merged"].item()) >= 1
+
+
+# ------------------------------------------------------------------------------------------------ apex links (3.9.8)
+APEX = dict(max_k=4, min_s=0.6, dz_win=150.0, tol_c=0.1, tol_z=4.0, tol_t=0.1, cut=3.0)
+
+
+def _apex_parity(tf, cuts=None, min_pairs=1):
+    kw = dict(APEX); kw.update(cuts or {})
+    P, trk, out = run_gpu(tf)
+    T = out.numpy()["n_tracks"]
+    m = trk.merge(T, apex=kw)
+    o = run_oracle(tf, P, last_stage=6).merge(**CUTS).apex(**kw)
+    M = m["n_merged"]
+    assert M == o.get("mrg_seg_start").size - 1 and np.array_equal(m["seg_idx"], o.get("mrg_seg_idx"))
+    assert np.array_equal(trk.stage_view("apex_best")[:M], o.get("apx_best"))
+    assert np.array_equal(trk.stage_view("apex_score")[:M], o.get("apx_score").astype(np.float32))
+    assert np.array_equal(m["apex_partner"], o.get("apx_partner")) and np.array_equal(m["apex_leg"], o.get("apx_leg"))
+    pairs = int((o.get("apx_partner") >= 0).sum()) // 2
+    assert pairs >= min_pairs, pairs
+    return m, o, pairs
+
+
+def test_apex_links_bit_exact_on_looper_frames():
+    tf = generate_config("cfg3", n_collisions=3, loopers=True)
+    m, o, pairs = _apex_parity(tf, min_pairs=2000)
+    # the pairs are what the generator says: the two legs of one truth track
+    _apex_parity(generate_config("cfg2", n_tracks=1500, seed=8, loopers=True), min_pairs=500)
+    _apex_parity(tf, cuts=dict(max_k=2, min_s=0.8, dz_win=40.0, tol_c=0.03, tol_z=1.0, tol_t=0.03, cut=1.0), min_pairs=20)
+    _apex_parity(tf, cuts=dict(max_k=17, min_s=0.0, dz_win=400.0, tol_c=0.5, tol_z=20.0, tol_t=0.5, cut=10.0), min_pairs=2000)
+
+
+def test_apex_links_without_loopers_and_bad_arguments(mini_event):
+    m, o, pairs = _apex_parity(mini_event, min_pairs=0)
+    P, trk, out = run_gpu(mini_event)
+    fit = trk.new_fit(); mg = trk.new_merged(); ax = trk.new_apex()
+    trk.refit_into(fit); trk.merge_into(fit, mg)
+    for bad in (dict(dz_win=0.0), dict(tol_c=0.0), dict(tol_z=-1.0), dict(max_k=-1), dict(cut=float("nan"))):
+        with pytest.raises(RuntimeError):
+            trk.apex_into(mg, ax, bad)
+    trk.apex_into(mg, ax)
+    torch.cuda.synchronize()
