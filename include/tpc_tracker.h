@@ -243,7 +243,9 @@ TPC_API int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, cons
 
 /* Same from/to HOST buffers (tracker created with host_io != 0): copies the SoA input to the device,
  * runs S1..S5, copies n_tracks, status, the track list, the CSR and cluster_track back, all on
- * `cuda_stream`, then synchronises that stream.  Copy sizes of the outputs are bounded by the
+ * `cuda_stream`, then synchronises that stream.  On the host paths (this call and the begin / end pair)
+ * out->cluster_track may be NULL: the per-cluster assignment is then not copied back (4 bytes per input cluster,
+ * 39 % of the download on a Pb-Pb time frame; the CSR trk_cl_start / trk_cl_idx carries the same information).  Copy sizes of the outputs are bounded by the
  * capacities; the per-track arrays are copied for the n_tracks tracks found. */
 TPC_API int tpc_track_timeframe_host(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tracks_t* out, void* cuda_stream);
 

@@ -189,8 +189,10 @@ def pack_params(params: dict):
 class Tracks:
     """Output buffers (torch tensors on `device`, or pinned host tensors) laid out as tpc_tracks_t wants."""
 
-    def __init__(self, n_clusters: int, max_tracks: int, max_track_clusters: int, device):
+    def __init__(self, n_clusters: int, max_tracks: int, max_track_clusters: int, device, with_cluster_track: bool = True):
         host = torch.device(device).type == "cpu"
+        assert host or with_cluster_track, "the device path always writes cluster_track"
+        self.with_cluster_track = bool(with_cluster_track)
         kw = dict(device=device, pin_memory=True) if host else dict(device=device)
         i32 = lambda *s: torch.empty(*s, dtype=torch.int32, **kw)   # noqa: E731
         f32 = lambda *s: torch.empty(*s, dtype=torch.float32, **kw)  # noqa: E731
@@ -210,13 +212,15 @@ class Tracks:
         s.max_tracks = self.max_tracks; s.max_track_clusters = self.max_track_clusters
         for f in _TRACK_FIELDS:
             setattr(s, f, getattr(self, f).data_ptr())
+        if not self.with_cluster_track:
+            s.cluster_track = None              # host paths: do not copy the per-cluster assignment back
         return s
 
     def bytes_out(self) -> int:
         """Bytes a host run copies back for the tracks found (d2h_bytes_per_step)."""
         T = int(self.n_tracks.item())
         ntc = int(self.trk_cl_start[T].item()) if T else 0
-        return 8 + T * 4 * (9 + 5 + 15) + (T + 1) * 4 + ntc * 4 + self.n_in * 4
+        return 8 + T * 4 * (9 + 5 + 15) + (T + 1) * 4 + ntc * 4 + (self.n_in * 4 if self.with_cluster_track else 0)
 
     def numpy(self) -> dict:
         """Host copies trimmed to the tracks found."""
@@ -289,8 +293,8 @@ class Tracker:
         c.sector = sector.data_ptr(); c.row = row.data_ptr(); c.x = None; c.y = y.data_ptr(); c.z = z.data_ptr()
         return c
 
-    def new_tracks(self, n_clusters: int, host: bool = False) -> Tracks:
-        return Tracks(n_clusters, self.caps[3], self.caps[4], "cpu" if host else self.device)
+    def new_tracks(self, n_clusters: int, host: bool = False, with_cluster_track: bool = True) -> Tracks:
+        return Tracks(n_clusters, self.caps[3], self.caps[4], "cpu" if host else self.device, with_cluster_track)
 
     def track_timeframe(self, sector, row, y, z, out: Tracks, stream=None):
         """Device tensors in, device tensors out; enqueues on `stream` (default: torch's current stream)."""

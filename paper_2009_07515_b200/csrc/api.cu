@@ -212,9 +212,10 @@ int run_device(tpc_tracker* t, const tpc_clusters_t* in, const OutPtrs& o, cudaS
   return cudaGetLastError() == cudaSuccess ? TPC_OK : TPC_ERR_CUDA;
 }
 
-bool out_ok(const tpc_tracks_t* o) {
+// host outputs may leave cluster_track NULL: it is then not copied back (it is recomputable from the CSR)
+bool out_ok(const tpc_tracks_t* o, bool host = false) {
   return o && o->n_tracks && o->status && o->sector && o->first_row && o->last_row && o->n_clusters && o->par && o->cov &&
-         o->x_ref && o->z_ref && o->chi2 && o->ndf && o->trk_cl_start && o->trk_cl_idx && o->cluster_track && o->z_beam &&
+         o->x_ref && o->z_ref && o->chi2 && o->ndf && o->trk_cl_start && o->trk_cl_idx && (host || o->cluster_track) && o->z_beam &&
          o->max_tracks >= 1 && o->max_track_clusters >= 1;
 }
 
@@ -247,7 +248,7 @@ bool copy_tracks_d2h(const OutPtrs& o, const tpc_tracks_t* out, size_t n, size_t
   } else {
     out->trk_cl_start[0] = 0;
   }
-  return ok && d2h(out->cluster_track, o.cluster_track, n * 4);
+  return ok && (!out->cluster_track || d2h(out->cluster_track, o.cluster_track, n * 4));
 }
 
 }  // namespace
@@ -326,7 +327,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tr
 }
 
 int tpc_track_timeframe_host(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tracks_t* out, void* cuda_stream) {
-  if (!t || !in || !out_ok(out) || !t->host_io) return TPC_ERR_INVALID_ARG;
+  if (!t || !in || !out_ok(out, true) || !t->host_io) return TPC_ERR_INVALID_ARG;
   if (in->n < 0 || (in->n > 0 && (!in->sector || !in->row || !in->y || !in->z))) return TPC_ERR_INVALID_ARG;
   if (in->n > t->max_clusters || out->max_tracks > t->max_tracks || out->max_track_clusters > t->max_track_clusters)
     return TPC_ERR_CAPACITY;
@@ -407,7 +408,7 @@ int tpc_track_timeframe_host_begin(tpc_tracker_t* t, const tpc_clusters_t* in, i
 }
 
 int tpc_track_timeframe_host_end(tpc_tracker_t* t, const tpc_tracks_t* out, int32_t slot) {
-  if (!t || !out_ok(out) || t->host_io < 2 || slot < 0 || slot >= t->host_io) return TPC_ERR_INVALID_ARG;
+  if (!t || !out_ok(out, true) || t->host_io < 2 || slot < 0 || slot >= t->host_io) return TPC_ERR_INVALID_ARG;
   tpc_tracker::Slot& sl = t->slot[slot];
   if (!sl.busy) return TPC_ERR_INVALID_ARG;
   if (out->max_tracks != t->max_tracks || out->max_track_clusters != t->max_track_clusters) return TPC_ERR_INVALID_ARG;

@@ -136,6 +136,28 @@ def test_host_path_equals_device_path(mini_event):
             assert np.array_equal(a[k], b[k]), k
 
 
+def test_host_paths_without_cluster_track(mini_event):
+    """cluster_track = NULL on the host paths: nothing is copied there, everything else is unchanged."""
+    tf = mini_event
+    P, trk, out = run_gpu(tf, host=3)
+    ref = out.numpy()
+    ins = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (tf.sector, tf.row, tf.y, tf.z)]
+    o2 = trk.new_tracks(tf.n, host=True, with_cluster_track=False)
+    o2.cluster_track.fill_(-7)
+    trk.track_timeframe_host(*ins, o2)
+    a = o2.numpy()
+    assert np.all(a["cluster_track"] == -7) and o2.bytes_out() == out.bytes_out() - 4 * tf.n
+    for k in ref:
+        if k != "cluster_track" and isinstance(ref[k], np.ndarray):
+            assert np.array_equal(ref[k], a[k]), k
+    o3 = trk.new_tracks(tf.n, host=True, with_cluster_track=False)
+    o3.cluster_track.fill_(-7)
+    trk.track_timeframe_host_begin(*ins, 1)
+    trk.track_timeframe_host_end(o3, 1)
+    b = o3.numpy()
+    assert np.all(b["cluster_track"] == -7) and np.array_equal(b["trk_cl_idx"], ref["trk_cl_idx"]) and b["n_tracks"] == ref["n_tracks"]
+
+
 def test_repeatable_and_reusable(mini_event):
     """Two calls on one handle give identical results (ids come from scans, not from atomics)."""
     import paper_2009_07515_b200 as tpc
