@@ -28,7 +28,10 @@
 // the field constant vs the textbook radius of curvature (tests/golden/helix_radius.txt); the two CHOICES among
 // several candidates - the S4 search (gate, strict minimum, tie -> lowest position, window, weights) and the S2 pair
 // choice and link cut - on hand-built dyadic constructions whose answers are known by hand, plus a whole-row scan
-// (tests/test_oracle_choice_pins.py; each case lists the mutations it kills).  Nothing is left "parity unpinned".
+// (tests/test_oracle_choice_pins.py; each case lists the mutations it kills); the native time input, the track merger
+// (rotation, upward and merged refit, candidates / score / mutual choice / chains) and the apex links of loopers in
+// tests/test_oracle_time_input.py, test_oracle_merge.py, test_oracle_apex.py (DESIGN.md section 9 lists the pins and the
+// twenty mutations they kill).  Nothing is left "parity unpinned".
 // =============================================================================================
 #include <algorithm>
 #include <chrono>

@@ -193,7 +193,7 @@ def test_the_two_tracks_around_a_long_hole_become_one(singles):
         assert abs(o.get("mrg_par")[4] - q_true) < 1e-4 * abs(q_true)
         assert o.get("mrg_x_ref")[0] == np.float32(P["row_x"][holed.row.min()])
         # too long a hole for the row window: left alone
-        o2 = _run_merge(_subset(tf, ~np.isin(tf.row, np.arange(r0, r0 + 12))), P, max_rows=11)
+        o2 = _run_merge(_subset(tf, ~np.isin(tf.row, np.arange(r0, r0 + 12))), P, max_rows=12)   # fit_row_B = r_A + 13
         assert o2.get("trk_seed").size == 2 and o2.get("mrg_seg_start").size == 3
         o3 = _run_merge(_subset(tf, ~np.isin(tf.row, np.arange(r0, r0 + 12))), P, max_rows=13)
         assert o3.get("mrg_seg_start").size == 2
@@ -233,6 +233,52 @@ def test_foreign_segments_are_not_taken_and_the_right_continuation_is_chosen(sin
         assert o.get("mrg_next")[L] == U and o.get("mrg_prev")[U] == L and o.get("mrg_prev")[U2] < 0
         assert o.get("mrg_best_a")[U2] == L                    # U2 did want L: only the mutual test keeps it out
         assert o.get("mrg_of_track")[L] == o.get("mrg_of_track")[U] != o.get("mrg_of_track")[U2]
+
+
+def test_choice_is_the_best_not_the_first_and_links_are_mutual(singles):
+    """(i) the foreign continuation comes FIRST in z order (shift -0.25 cm as well as +0.25): the best is still taken;
+    (ii) two lower parts (L and a copy shifted by 0.25 cm) want the same upper part U: only the better one gets it, the
+    other stays alone (without the mutual test U's back link is overwritten by the last taker);
+    (iii) a continuation that starts on the very next row (a 1.5 cm kink the finder does not follow) is a candidate:
+    the row window starts at r_A + 1.  Kills: first-candidate, no-mutual-test, row window off by one."""
+    tf = _long_ones(singles, 1)[0]
+    P = default_params(tf, cell=4.0)
+    r0 = int(tf.row.min()) + 50
+    lower, upper = tf.row < r0, tf.row >= r0 + 6
+
+    def build(parts):
+        out = _subset(tf, np.zeros(tf.n, bool))
+        for f in ("sector", "row", "x", "y", "z", "track_id"):
+            setattr(out, f, np.concatenate([getattr(p_, f) for p_ in parts]))
+        return out
+
+    def shifted(mask, dz):
+        q = _subset(tf, mask); q.z = (q.z + np.float32(dz)).astype(np.float32)
+        return q
+    for dz in (0.25, -0.25):                                  # (i)
+        o = _run_merge(build([_subset(tf, lower), _subset(tf, upper), shifted(upper, dz)]), P)
+        assert o.get("trk_seed").size == 3
+        first = o.get("trk_first_row"); L = int(np.argmin(first))
+        ztop = lambda k: o.get("zs")[o.get("trk_cl_pos")[o.get("trk_cl_start")[k + 1] - 1]]   # noqa: E731
+        zref = float(tf.z[np.argmax(tf.row)])
+        U = min((k for k in range(3) if k != L), key=lambda k: abs(ztop(k) - zref))
+        assert o.get("mrg_next")[L] == U, dz
+    o = _run_merge(build([_subset(tf, lower), shifted(lower, 0.25), _subset(tf, upper)]), P)   # (ii)
+    assert o.get("trk_seed").size == 3
+    first = o.get("trk_first_row"); U = int(np.argmax(first))
+    lows = [k for k in range(3) if k != U]
+    assert all(o.get("mrg_best_b")[k] == U for k in lows)                      # both want U
+    taker = int(o.get("mrg_best_a")[U])
+    other = [k for k in lows if k != taker][0]
+    assert o.get("mrg_chi2_b")[taker] < o.get("mrg_chi2_b")[other]
+    assert o.get("mrg_next")[taker] == U and o.get("mrg_prev")[U] == taker and o.get("mrg_next")[other] < 0
+    assert o.get("mrg_seg_start").size == 3 and o.get("mrg_of_track")[other] != o.get("mrg_of_track")[U]
+    kink = build([_subset(tf, tf.row < r0), shifted(tf.row >= r0, 1.5)])        # (iii)
+    o = _run_merge(kink, P, chi2_cut=1e6)
+    assert o.get("trk_seed").size == 2
+    lo, hi = int(np.argmin(o.get("trk_first_row"))), int(np.argmax(o.get("trk_first_row")))
+    assert o.get("fit_row")[hi] == o.get("up_row")[lo] + 1 == r0 and o.get("mrg_next")[lo] == hi
+    assert _run_merge(kink, P).get("mrg_next")[lo] < 0                         # at the default cut the kink is no continuation
 
 
 # ------------------------------------------------------------------------------------------------ definitions
