@@ -40,7 +40,11 @@
 //  * covariance in shared memory, two buffers (live / last update, no copy), transport staged row by row: 64 registers,
 //    8 CTAs per SM, occupancy 37 -> 49 %: 11.8 ms (7 CTAs 11.7, 9 CTAs 12.8, 10 CTAs 19.8), but DRAM reads 10.5 -> 16.7 GB
 //    and L2 hit rate 53 -> 47 %: the lanes in flight (608-byte hit table each, plus the rows they walk) already exceed
-//    L2, so more warps buy latency hiding with cache misses - occupancy is not the lever, the working set is.
+//    L2, so more warps buy latency hiding with cache misses - occupancy is not the lever, the working set is;
+//  * L2 warm-up: every refill asks (prefetch.global.L2::evict_last) for its slice of bin_start, (y,z) and link_up 0.5 - 4
+//    sectors ahead of the ticket: 13.2 ms, DRAM reads 10.5 -> 15.8 GB, L2 hit rate 53 -> 45 % - the kernel refills all of
+//    L2 every 0.14 ms (875 GB/s of misses into 126 MB) while a tracklet lives 0.4 ms, so nothing asked for ahead of time
+//    survives until it is used.
 //
 // Arithmetic is written operation by operation in the order of DESIGN.md section 3.4 (compiled with
 // -fmad=false; fused multiply-adds only where the text writes fma(), as __fmaf_rn): the transport J C J^T skips only
