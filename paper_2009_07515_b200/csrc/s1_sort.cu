@@ -14,6 +14,10 @@
 // The result equals std::stable_sort by (sector,row,bin) whatever order the atomics resolved in.
 // (Round 1a-c used one device-wide counting sort over the ~N global bins: every one of its ~8 accesses
 // per cluster was a random 32-byte DRAM sector; 15.1 ms on cfg5, see profiles/.)
+// Round 2, measured and rejected: the partition without global atomics (per-chunk (sector,row) histograms from the count
+// pass, offsets by a scan over the chunks, shared-memory cursors per CTA): S1 4.45 -> 6.98 ms.  Each of the 1184 CTAs then
+// owns its own 5472 write positions, ~14 records = 224 bytes per run: 6.5 M open write streams instead of 5472, and L2 no
+// longer merges the 16-byte stores into full lines.  The shared global cursors are what keeps the writes dense.
 #include "tpc_internal.cuh"
 #include "../../include/tpc_tracker.h"
 
