@@ -180,3 +180,25 @@ def test_apex_links_without_loopers_and_bad_arguments(mini_event):
             trk.apex_into(mg, ax, bad)
     trk.apex_into(mg, ax)
     torch.cuda.synchronize()
+
+
+def test_merge_and_apex_on_an_empty_frame_and_after_a_status_bit(cfg1):
+    """No tracks: n_merged = 0 and nothing is written; a frame that ended with a status bit (capacity overflow) merges
+    to nothing as well."""
+    import copy
+    import paper_2009_07515_b200 as tpc
+    empty = copy.copy(cfg1)
+    for f in ("sector", "row", "x", "y", "z", "track_id"):
+        setattr(empty, f, getattr(cfg1, f)[:0].copy())
+    P = default_params(cfg1)
+    trk = tpc.Tracker(P, 1024, 4096, 64, 64, 1024)
+    ins = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (empty.sector, empty.row, empty.y, empty.z)]
+    out = trk.new_tracks(0)
+    trk.track_timeframe(*ins, out)
+    m = trk.merge(0, apex=True)
+    assert out.numpy()["n_tracks"] == 0 and m["n_merged"] == 0 and m["seg_start"].tolist() == [0] and m["apex_partner"].size == 0
+    # seeds overflow -> status bit -> zero tracks -> zero merged tracks
+    _, trk2, out2 = run_gpu(cfg1, caps=dict(max_seeds=4))
+    assert out2.numpy()["status"] & 4 and out2.numpy()["n_tracks"] == 0
+    m2 = trk2.merge(0, apex=True)
+    assert m2["n_merged"] == 0
