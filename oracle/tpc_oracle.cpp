@@ -757,6 +757,7 @@ struct Oracle {
         int dir = 0, sb = sa_;
         if (pass == 1) {
           // the neighbour the outer end is heading for: only if that end lies within `edge` of the sector boundary
+          if (n_az < 1) continue;                         // a one-sector geometry has no neighbour
           if (!(std::fabs(ya) >= T(ymax[ra]) - T(mc.edge))) continue;
           dir = ya >= T(0) ? 1 : -1;
           sb = (sa_ / n_az) * n_az + ((sa_ % n_az) + dir + n_az) % n_az;
@@ -921,7 +922,8 @@ struct Oracle {
           const T s2 = sk * cos_a + ck * sin_a, c2 = ck * cos_a - sk * sin_a;
           sk = s2; ck = c2;
         }
-        const int s_b = (s_a / n_az) * n_az + ((((s_a % n_az) + dirA * k) % n_az) + n_az) % n_az;
+        if (k > 0 && n_az < 1) break;                       // a one-sector geometry: the tail's own sector only
+        const int s_b = n_az < 1 ? s_a : (s_a / n_az) * n_az + ((((s_a % n_az) + dirA * k) % n_az) + n_az) % n_az;
         if (k > 0 && s_b == s_a) break;                     // once round
         const T sd = dirA > 0 ? sk : T(0) - sk;             // sector s_b is the frame of s_a turned by dirA * k sector angles
         for (int B = 0; B < nm; ++B) {                       // plain scan; the predicates below define the set

@@ -263,6 +263,7 @@ __global__ void __launch_bounds__(kThreads) k_merge_match(Ctx c, FitPtrs f, Merg
     for (int pass = 0; pass < 2; ++pass) {
       int dir = 0, s_b = s_a;
       if (pass == 1) {
+        if (n_az < 1) continue;                           // a one-sector geometry has no neighbour
         if (!(fabsf(y_a) >= tymax[r_a] - o.edge)) continue;
         dir = y_a >= 0.0f ? 1 : -1;
         s_b = (s_a / n_az) * n_az + ((s_a % n_az) + dir + n_az) % n_az;
@@ -517,7 +518,8 @@ __global__ void __launch_bounds__(kThreads) k_apex_match(Ctx c, MergePtrs m, Ape
         const float s2 = sk * m.cos_a + ck * m.sin_a, c2 = ck * m.cos_a - sk * m.sin_a;
         sk = s2; ck = c2;
       }
-      const int s_b = (s_a / n_az) * n_az + ((((s_a % n_az) + dirA * k) % n_az) + n_az) % n_az;
+      if (k > 0 && n_az < 1) break;
+      const int s_b = n_az < 1 ? s_a : (s_a / n_az) * n_az + ((((s_a % n_az) + dirA * k) % n_az) + n_az) % n_az;
       if (k > 0 && s_b == s_a) break;
       if (c.m_nzb[s_b] == 0) continue;
       const float sd = dirA > 0 ? sk : 0.0f - sk;

@@ -202,3 +202,21 @@ def test_merge_and_apex_on_an_empty_frame_and_after_a_status_bit(cfg1):
     assert out2.numpy()["status"] & 4 and out2.numpy()["n_tracks"] == 0
     m2 = trk2.merge(0, apex=True)
     assert m2["n_merged"] == 0
+
+
+@pytest.mark.parametrize("S", [1, 2, 5])
+def test_merge_in_odd_geometries(S, cfg1):
+    """One sector (no neighbour), two sectors, an odd count: same results as the oracle, no neighbour arithmetic blows up."""
+    import copy
+    tf = copy.copy(cfg1)
+    keep = (cfg1.sector == np.bincount(cfg1.sector).argmax()) & ~np.isin(cfg1.row, np.arange(60, 66))
+    for f in ("sector", "row", "x", "y", "z", "track_id"):
+        setattr(tf, f, getattr(cfg1, f)[keep].copy())
+    tf.sector = np.zeros_like(tf.sector)
+    P = default_params(cfg1); P["n_sectors"] = S
+    m, o, links = _merge_parity(tf, P=P, min_links=10)
+    kw = dict(APEX)
+    Pg, trk, out = run_gpu(tf, params=P)
+    mm = trk.merge(out.numpy()["n_tracks"], apex=kw)
+    oo = run_oracle(tf, P, last_stage=6).merge(**CUTS).apex(**kw)
+    assert np.array_equal(mm["apex_partner"], oo.get("apx_partner"))

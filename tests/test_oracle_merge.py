@@ -481,3 +481,17 @@ def test_merging_against_generator_truth(mini_tf):
         em.append((mq[m] - q) / abs(q)); es.append((fq[segs[0]] - q) / abs(q))
     em, es = np.array(em), np.array(es)
     assert em.size > 1000 and np.median(np.abs(em)) < 0.7 * np.median(np.abs(es)), (np.median(np.abs(em)), np.median(np.abs(es)))
+
+
+def test_odd_geometries_do_not_break_the_neighbour_arithmetic(singles):
+    """One sector (no neighbour at all), two sectors (each side has a single sector: its neighbour is itself, skipped),
+    an odd sector count: the merger and the apex search run and only join what lies in one sector."""
+    tf = _long_ones(singles, 1)[0]
+    r0 = int(tf.row.min()) + 45
+    holed = _subset(tf, ~np.isin(tf.row, np.arange(r0, r0 + 5)))
+    for S in (1, 2, 5):
+        P = default_params(tf, cell=4.0); P["n_sectors"] = S
+        holed.sector = np.zeros_like(holed.sector)
+        o = Oracle(P).run(holed.sector, holed.row, holed.y, holed.z, last_stage=6).merge(**CUTS).apex()
+        assert o.get("trk_seed").size == 2 and np.array_equal(o.get("mrg_seg_idx"), [0, 1]) and o.get("mrg_dir")[0] == 0, S
+        assert np.all(o.get("apx_partner") < 0)
