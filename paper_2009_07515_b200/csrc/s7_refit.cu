@@ -4,6 +4,9 @@
 // track) and writes one fitted state per track.
 // One thread per track.  The owned clusters are walked from the top row down through the ownership bit mask; the seed
 // direction comes from the top two, q/pT from the track, then propagate + update (no gate) cluster by cluster.
+// Round 2, measured and rejected: the S4 pattern (persistent kernel, every lane pulls its next track from a ticket, one
+// propagate + update step per loop iteration) - 10 -> ~25 of 32 lanes active, but 2.79 ms against 2.83: the kernel waits for
+// the random 32-byte sectors of (y,z) behind the hit table (2.6 GB for 82 M clusters), not for idle lanes.
 #include "kf.cuh"
 #include "tpc_internal.cuh"
 
