@@ -11,15 +11,20 @@
 // state in shared memory 10.4 ms (twelve CTA barriers per tile cost more than the idle lanes they remove); the k = 2 up
 // retries (40 % of the clusters, 2 ms of the kernel) deferred to a second, compacted launch 6.5 ms.
 // Round 2 (profiles/r02_s2_regions.md: 49 % of the instructions are the rectangle query at 10 - 18 lanes, 20 % the pair
-// scoring at 9.6 lanes; DRAM traffic = 1.0 x the algorithmic bytes).  Two more designs measured and rejected on cfg5
-// (this version: 5.74 ms), both bit-exact:
+// scoring at 9.6 lanes; DRAM traffic = 1.0 x the algorithmic bytes).  Three more designs measured and rejected on cfg5
+// (this version: 5.74 ms), all bit-exact:
 //  * the rectangle query split in two halves (bin cover + the four bin_start loads / the candidate walk) so that the
 //    loads of the up and the down query of a cluster are in flight together before either walk starts: 6.12 ms - the
 //    down query is then computed for the 15 % of the clusters whose up window turns out empty, and eight more live
 //    values per thread cost more than the overlapped latency (the kernel is issue-bound, 75 % of the slots busy);
 //  * the candidate lists keep (position, y, z) so that the scoring does not gather the candidates a second time
 //    (kCap 4 to keep 5 CTAs per SM): 7.77 ms - the second gather hits L1 anyway, while the lists' shared-memory
-//    traffic triples and windows with 5 - 8 candidates fall back to the re-walk.
+//    traffic triples and windows with 5 - 8 candidates fall back to the re-walk;
+//  * warp tiles: the warp finds, per target row, the one contiguous run of positions that holds all 32 windows (two
+//    bin_start loads), streams it through a 32-entry shared-memory tile with coalesced loads, and every lane tests every
+//    candidate of the tile against its own rectangle (broadcast reads, uniform control flow, no divergence): 13.7 ms.
+//    The run holds ~36 candidates for windows that accept ~1.5 each, and a test costs ~12 instructions: the uniform scan
+//    does ten times the comparisons the bin lookup does, which costs more than all the idle lanes it removes.
 #include "tpc_internal.cuh"
 
 namespace tpc {
