@@ -504,6 +504,13 @@ def run_ours(args):
     apex_ms = ev0.elapsed_time(ev1)
     n_apex = int((ax_buf["apex_partner"][:n_merged] >= 0).sum().item()) // 2
     del mg_buf, ax_buf
+    # ---- strategy-A hit removal: wall time of the convenience call minus the calls timed above
+    torch.cuda.synchronize(dev)
+    t0 = time.perf_counter()
+    cls_, rem_ = trk.removable(out)
+    removable_all_ms = (time.perf_counter() - t0) * 1e3
+    removed_frac = float(rem_.float().mean().item()) if tf.n else 0.0
+    del cls_, rem_
     # ---- cluster protection for hit removal, strategy B (separate call), 1 cm road
     keep = trk.protect(out, 1.0, 1.0)
     ev0.record(stream)
@@ -613,6 +620,9 @@ def run_ours(args):
                           "borders and long holes, upward + merged downward refit", "ms": merge_ms, "n_merged": n_merged},
         "apex": {"what": "tpc_tracker_apex (separate call after the merge, not in the step): looper legs paired through their "
                          "circles, returning leg labelled", "ms": apex_ms, "pairs": n_apex},
+        "removable": {"what": "tpc_tracker_removable after refit + merge + apex (strategy A: class per cluster, protection by good "
+                              "tracks); wall ms of the whole sequence incl. its buffer allocations", "ms_sequence": removable_all_ms,
+                      "removed_fraction": removed_frac},
         "protect": {"what": "tpc_tracker_protect (separate call, not in the step): strategy-B keep flag per cluster, 1 cm road",
                     "ms": protect_ms, "kept_fraction": kept_frac},
         "roofline": roofline,

@@ -346,6 +346,28 @@ TPC_API int tpc_tracker_apex(tpc_tracker_t* t, const tpc_merged_t* merged, const
 TPC_API int tpc_tracker_protect(tpc_tracker_t* t, const int32_t* cluster_track, float road_y, float road_z, uint8_t* keep,
                                 void* cuda_stream);
 
+/* Cuts of the strategy-A hit removal. */
+typedef struct {
+  float min_pt;    /* GeV/c: merged tracks with |q/pT| * min_pt > 1 are "very low momentum" (0.05) */
+  float max_incl;  /* a track segment steeper than this |sin(phi)| at BOTH ends has "high inclination" (0.85) */
+  float road_y;    /* cm: road of the protection by good tracks, as in tpc_tracker_protect */
+  float road_z;    /* cm */
+} tpc_removal_cuts_t;
+
+/* Hit removal, "strategy A" ("positive identification of all hits that can safely
+ * be removed" - very low momentum, secondary legs of looping tracks, high inclination - while the good tracks "protect all
+ * hits in their vicinity from removal").  For the LAST tpc_track_timeframe / tpc_tracker_refit / tpc_tracker_merge /
+ * tpc_tracker_apex sequence on this handle (`cluster_track`, `fit`, `merged`, `apex` are their outputs, DEVICE):
+ * cls[i]    (DEVICE, [n] bytes) class of input cluster i: 0 not attached, 1 good track, 2 secondary leg of a looper,
+ *           3 very low momentum, 4 high inclination;
+ * remove[i] (DEVICE, [n] bytes) 1 iff cls[i] >= 2 and the cluster does not lie, in its own (sector, row), within the road
+ *           of a cluster owned by a good track.
+ * Enqueued on `cuda_stream`, ordered after those calls; does not synchronise.  The S1 record scratch of the workspace is
+ * reused (the next tpc_track_timeframe overwrites it anyway). */
+TPC_API int tpc_tracker_removable(tpc_tracker_t* t, const int32_t* cluster_track, const tpc_fit_t* fit, const tpc_merged_t* merged,
+                                  const tpc_apex_t* apex, const tpc_removal_cuts_t* cuts, uint8_t* cls, uint8_t* remove,
+                                  void* cuda_stream);
+
 /* Pipelined host path (tracker created with host_io = 2 or 3 = number of staging slots; BASELINE.json north_star: whole time frames arrive one
  * after the other).  `begin` enqueues the H2D copy of one frame's HOST (pinned) inputs and its
  * S1..S5 on streams the library owns and returns without waiting; `end` waits for that frame, copies exactly the

@@ -67,6 +67,8 @@ def _load():
         lib.orc_merge.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float]
         lib.orc_apex.restype = None
         lib.orc_apex.argtypes = [C.c_void_p, C.c_int] + [C.c_float] * 6
+        lib.orc_removable.restype = None
+        lib.orc_removable.argtypes = [C.c_void_p] + [C.c_float] * 4
         lib.orc_kf_rotate.restype = C.c_double
         lib.orc_kf_rotate.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double]
         lib.orc_search.restype = C.c_int
@@ -134,6 +136,11 @@ class Oracle:
              tol_t: float = 0.1, cut: float = 3.0) -> "Oracle":
         """DESIGN.md section 3.9.8 on the merged tracks of the last merge(): results under apx_*."""
         self._lib.orc_apex(self._h, int(max_k), float(min_s), float(dz_win), float(tol_c), float(tol_z), float(tol_t), float(cut))
+        return self
+
+    def removable(self, min_pt: float = 0.05, max_incl: float = 0.85, road_y: float = 1.0, road_z: float = 1.0) -> "Oracle":
+        """DESIGN.md section 3.8a (strategy A) on the results of the last merge() + apex(): rem_class, rem_good_track, rem_remove."""
+        self._lib.orc_removable(self._h, float(min_pt), float(max_incl), float(road_y), float(road_z))
         return self
 
     def kf_rotate(self, par, cov15, x, sa, ca, precision=64):

@@ -306,6 +306,8 @@ struct Oracle {
   // S9 apex links of loopers
   std::vector<int32_t> apx_best, apx_partner, apx_leg;             // [n_merged]
   std::vector<double> apx_score;                                   // [n_merged] score of apx_best or -1
+  // hit removal, strategy A
+  std::vector<int32_t> rem_class, rem_good_track, rem_remove;      // [n] by INPUT index
   int s4_prec = 32;
   std::vector<int32_t> trk_cl_start, trk_cl_idx, cluster_track;
   std::vector<double> stage_seconds;                              // [5]
@@ -976,6 +978,46 @@ struct Oracle {
     }
   }
 
+
+  // ---------------------------------------------------------------------------------------- S8a
+  // Hit removal, "strategy A": "positive identification of all hits that can
+  // safely be removed" - hits of "tracks of very low momentum", "secondary legs of looping tracks", "track segments with
+  // high inclination angle" - while "the online tracking identifies the good tracks used for physics and protects all hits
+  // in their vicinity from removal".  Class of an input cluster: 0 not attached; else, for its track k and merged track m:
+  // 2 if m is the secondary leg of a looper (3.9.8); else 3 if |q/pT| of the merged fit times min_pt exceeds 1 (low
+  // momentum); else 4 if both ends of the segment k are steeper than max_incl; else 1 (good).  Good tracks protect the
+  // clusters inside their road exactly as in section 3.8; a cluster is removable iff its class is >= 2 and it is not
+  // protected.
+  void stage11(float min_pt, float max_incl, float road_y, float road_z) {
+    const int nt = (int)trk_seed.size();
+    std::vector<int32_t> cls_of_track(nt, 1);
+    for (int k = 0; k < nt; ++k) {
+      const int m = mrg_of_track[k];
+      if (m >= 0 && apx_leg[m] == 1) cls_of_track[k] = 2;
+      else if (m >= 0 && std::fabs((float)mrg_par[(size_t)m * 5 + 4]) * min_pt > 1.0f) cls_of_track[k] = 3;
+      else if (std::fabs((float)fit_par[(size_t)k * 5 + 2]) > max_incl && std::fabs((float)up_par[(size_t)k * 5 + 2]) > max_incl) cls_of_track[k] = 4;
+    }
+    rem_class.assign(n, 0); rem_good_track.assign(n, -1); rem_remove.assign(n, 0);
+    for (int64_t i = 0; i < n; ++i) {
+      const int k = cluster_track[i];
+      if (k < 0) continue;
+      rem_class[i] = cls_of_track[k];
+      if (cls_of_track[k] == 1) rem_good_track[i] = k;
+    }
+    // protection by the good tracks only (the road of section 3.8 around every cluster a good track owns)
+    std::vector<int32_t> kept(n, 0);
+    for (int id = 0; id < nt; ++id) {
+      if (cls_of_track[id] != 1) continue;
+      for (int32_t q = trk_cl_start[id]; q < trk_cl_start[id + 1]; ++q) {
+        const int o = trk_cl_pos[q];
+        const float y = ys[o], z = zs[o];
+        for_each_in_rect(s_sector[o], s_row[o], y - road_y, y + road_y, z - road_z, z + road_z,
+                         [&](int j) { kept[perm[j]] = 1; });
+      }
+    }
+    for (int64_t i = 0; i < n; ++i) rem_remove[i] = rem_class[i] >= 2 && !kept[i];
+  }
+
   // ---------------------------------------------------------------------------------------- S8
   // Cluster protection for hit removal, "strategy B": "runs only the online tracking and removes all hits not in the
   // vicinity of good tracks".  A cluster is protected iff it is attached to a track or
@@ -1119,6 +1161,7 @@ int orc_get(void* h, const char* name, const void** ptr, int64_t* n, int* kind) 
   I32(fit_row); F64(up_par); F64(up_cov); F64(up_x_ref); F64(up_z_ref); F64(up_chi2); I32(up_row); I32(up_n);
   I32(mrg_best_b); I32(mrg_best_a); I32(mrg_next); I32(mrg_prev); I32(mrg_dir); F64(mrg_chi2_b);
   I32(mrg_of_track); I32(mrg_seg_start); I32(mrg_seg_idx);
+  I32(rem_class); I32(rem_good_track); I32(rem_remove);
   I32(apx_best); I32(apx_partner); I32(apx_leg); F64(apx_score);
   F64(mrg_par); F64(mrg_cov); F64(mrg_x_ref); F64(mrg_z_ref); F64(mrg_chi2); I32(mrg_n_fit); I32(mrg_ndf); I32(mrg_sector); I32(mrg_n_clusters);
   F32(up_dx); F32(up_ratio); F32(up_wy); F32(up_wz); F32(dn_dx); F32(dn_ratio); F32(dn_wy); F32(dn_wz);
@@ -1171,6 +1214,11 @@ void orc_apex(void* h, int max_k, float min_s, float dz_win, float tol_c, float 
   Oracle* o = reinterpret_cast<Oracle*>(h);
   const Oracle::ApexCuts ac{max_k, min_s, dz_win, tol_c, tol_z, tol_t, cut};
   if (o->s4_prec == 64) o->stage10<double>(ac); else o->stage10<float>(ac);
+}
+
+// strategy-A classification on the results of the last orc_merge + orc_apex
+void orc_removable(void* h, float min_pt, float max_incl, float road_y, float road_z) {
+  reinterpret_cast<Oracle*>(h)->stage11(min_pt, max_incl, road_y, road_z);
 }
 
 // one rotation of DESIGN.md section 3.9.2 (for the pins): par / cov15 in place, returns the new x or NaN on failure

@@ -75,6 +75,11 @@ class tpc_apex_t(C.Structure):
     _fields_ = [("max_tracks", C.c_int64), ("apex_partner", C.c_void_p), ("apex_leg", C.c_void_p)]
 
 
+class tpc_removal_cuts_t(C.Structure):
+    _fields_ = [("min_pt", C.c_float), ("max_incl", C.c_float), ("road_y", C.c_float), ("road_z", C.c_float)]
+
+
+REMOVAL_CUTS = dict(min_pt=0.05, max_incl=0.85, road_y=1.0, road_z=1.0)
 APEX_CUTS = dict(max_k=4, min_s=0.6, dz_win=150.0, tol_c=0.1, tol_z=4.0, tol_t=0.1, cut=3.0)
 MERGE_CUTS = dict(max_rows=30, back_rows=1, edge=6.0, dz_win=50.0, chi2_cut=100.0, road_z0=2.0, road_z1=0.3)
 
@@ -101,7 +106,7 @@ STATUS_BITS = {1: "BAD_CLUSTER", 2: "BINS_OVERFLOW", 4: "SEEDS_OVERFLOW", 8: "TR
 
 EXPORTS = [
     "tpc_tracker_workspace_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
-    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit", "tpc_tracker_merge", "tpc_tracker_apex", "tpc_tracker_protect",
+    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit", "tpc_tracker_merge", "tpc_tracker_apex", "tpc_tracker_removable", "tpc_tracker_protect",
     "tpc_tracker_counters", "tpc_tracker_enable_stage_timing", "tpc_tracker_stage_ms", "tpc_tracker_stage_view",
     "tpc_tracker_launches_per_call", "tpc_tracker_destroy", "tpc_error_string",
 ]
@@ -148,6 +153,9 @@ def load_library(build: bool = True) -> C.CDLL:
     lib.tpc_tracker_merge.argtypes = [C.c_void_p, P(tpc_fit_t), P(tpc_merge_cuts_t), P(tpc_merged_t), C.c_void_p]
     lib.tpc_tracker_apex.restype = C.c_int
     lib.tpc_tracker_apex.argtypes = [C.c_void_p, P(tpc_merged_t), P(tpc_apex_cuts_t), P(tpc_apex_t), C.c_void_p]
+    lib.tpc_tracker_removable.restype = C.c_int
+    lib.tpc_tracker_removable.argtypes = [C.c_void_p, C.c_void_p, P(tpc_fit_t), P(tpc_merged_t), P(tpc_apex_t), P(tpc_removal_cuts_t),
+                                          C.c_void_p, C.c_void_p, C.c_void_p]
     lib.tpc_tracker_protect.restype = C.c_int
     lib.tpc_tracker_protect.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
     lib.tpc_tracker_counters.restype = C.c_int
@@ -408,6 +416,30 @@ class Tracker:
         o.apex_partner = out["apex_partner"].data_ptr(); o.apex_leg = out["apex_leg"].data_ptr()
         _check(self.lib, self.lib.tpc_tracker_apex(self._h, C.byref(m), C.byref(c), C.byref(o), C.c_void_p(st.cuda_stream)),
                "tpc_tracker_apex")
+
+    def removable(self, out: "Tracks", cuts: dict | None = None, merge_cuts: dict | None = None, apex_cuts: dict | None = None):
+        """Convenience: refit + merge + apex + tpc_tracker_removable for the last track_timeframe call (outputs `out`);
+        returns (cls, remove) as uint8 device tensors [n]."""
+        st = torch.cuda.current_stream(self.device)
+        fit = self.new_fit(); mg = self.new_merged(); ax = self.new_apex()
+        self.refit_into(fit); self.merge_into(fit, mg, merge_cuts); self.apex_into(mg, ax, apex_cuts)
+        f = tpc_fit_t(); f.max_tracks = self.caps[3]
+        for k in ("par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit"):
+            setattr(f, k, fit[k].data_ptr())
+        m = tpc_merged_t(); m.max_tracks = self.caps[3]
+        for k in _MERGED_FIELDS:
+            setattr(m, k, mg[k].data_ptr())
+        a = tpc_apex_t(); a.max_tracks = self.caps[3]
+        a.apex_partner = ax["apex_partner"].data_ptr(); a.apex_leg = ax["apex_leg"].data_ptr()
+        kw = dict(REMOVAL_CUTS); kw.update(cuts or {})
+        c = tpc_removal_cuts_t(float(kw["min_pt"]), float(kw["max_incl"]), float(kw["road_y"]), float(kw["road_z"]))
+        n = max(1, out.n_in)
+        cls = torch.zeros(n, dtype=torch.uint8, device=self.device); rem = torch.zeros(n, dtype=torch.uint8, device=self.device)
+        _check(self.lib, self.lib.tpc_tracker_removable(self._h, out.cluster_track.data_ptr(), C.byref(f), C.byref(m), C.byref(a),
+                                                         C.byref(c), cls.data_ptr(), rem.data_ptr(), C.c_void_p(st.cuda_stream)),
+               "tpc_tracker_removable")
+        torch.cuda.synchronize(self.device)
+        return cls[: out.n_in], rem[: out.n_in]
 
     def new_apex(self) -> dict:
         mt, dev = self.caps[3], self.device

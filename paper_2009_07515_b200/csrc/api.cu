@@ -489,6 +489,23 @@ int tpc_tracker_apex(tpc_tracker_t* t, const tpc_merged_t* merged, const tpc_ape
   return launch_apex(t->ctx, m, o, st) ? TPC_ERR_CUDA : TPC_OK;
 }
 
+int tpc_tracker_removable(tpc_tracker_t* t, const int32_t* cluster_track, const tpc_fit_t* fit, const tpc_merged_t* merged,
+                          const tpc_apex_t* apex, const tpc_removal_cuts_t* cuts, uint8_t* cls, uint8_t* remove, void* cuda_stream) {
+  if (!t || !cluster_track || !fit || !merged || !apex || !cuts || !cls || !remove) return TPC_ERR_INVALID_ARG;
+  if (!fit->par || !merged->merged_of_track || !merged->par || !apex->apex_leg) return TPC_ERR_INVALID_ARG;
+  if (!(cuts->min_pt >= 0.f) || !(cuts->max_incl >= 0.f) || !(cuts->road_y >= 0.f) || !(cuts->road_z >= 0.f)) return TPC_ERR_INVALID_ARG;
+  if (fit->max_tracks > t->max_tracks || merged->max_tracks > t->max_tracks || fit->max_tracks < 1 || merged->max_tracks < 1)
+    return TPC_ERR_CAPACITY;
+  RemovePtrs o{};
+  o.min_pt = cuts->min_pt; o.max_incl = cuts->max_incl; o.road_y = cuts->road_y; o.road_z = cuts->road_z;
+  o.cluster_track = cluster_track; o.merged_of_track = merged->merged_of_track; o.apex_leg = apex->apex_leg;
+  o.mrg_par = merged->par; o.mrg_stride = (int)merged->max_tracks; o.fit_par = fit->par; o.fit_stride = (int)fit->max_tracks;
+  o.cls = cls; o.remove = remove;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  t->last_stream = st;
+  return launch_removable(t->ctx, o, st) ? TPC_ERR_CUDA : TPC_OK;
+}
+
 int tpc_tracker_protect(tpc_tracker_t* t, const int32_t* cluster_track, float road_y, float road_z, uint8_t* keep,
                         void* cuda_stream) {
   if (!t || !keep || !cluster_track || !(road_y >= 0.f) || !(road_z >= 0.f)) return TPC_ERR_INVALID_ARG;

@@ -38,7 +38,59 @@ __global__ void __launch_bounds__(kThreads) k_out(Ctx c, const unsigned char* __
     keep[c.perm[o]] = mark[o];
 }
 
+// ---- hit removal, "strategy A": class of every track, then of every input cluster
+__global__ void __launch_bounds__(kThreads) k_track_class(Ctx c, RemovePtrs o) {
+  const int nt = c.cnt->status ? 0 : min(c.cnt->n_tracks, c.max_tracks);
+  const size_t mt = (size_t)c.max_tracks, ft = (size_t)o.fit_stride, gt = (size_t)o.mrg_stride;
+  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nt; k += gridDim.x * blockDim.x) {
+    const int m = o.merged_of_track[k];
+    int cls = 1;
+    if (m >= 0 && o.apex_leg[m] == 1) cls = 2;
+    else if (m >= 0 && fabsf(o.mrg_par[4 * gt + m]) * o.min_pt > 1.0f) cls = 3;
+    else if (fabsf(o.fit_par[2 * ft + k]) > o.max_incl && fabsf(c.up_par[2 * mt + k]) > o.max_incl) cls = 4;
+    c.m_bin_of[k] = cls;                                  // per-track scratch of the merger, free by now
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_cluster_class(Ctx c, RemovePtrs o, int* __restrict__ good_track) {
+  const long long n = c.n;
+  const bool dead = c.cnt->status != 0;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const int k = dead ? -1 : o.cluster_track[i];
+    const int cls = k >= 0 ? c.m_bin_of[k] : 0;
+    o.cls[i] = (unsigned char)cls;
+    good_track[i] = cls == 1 ? k : -1;
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_removable(Ctx c, RemovePtrs o, const unsigned char* __restrict__ keep) {
+  const long long n = c.n;
+  const bool dead = c.cnt->status != 0;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+    o.remove[i] = (!dead && o.cls[i] >= 2 && !keep[i]) ? 1 : 0;
+}
+
 }  // namespace
+
+int launch_protect(const Ctx& c, const int* cluster_track, float road_y, float road_z, unsigned char* keep, cudaStream_t st);
+
+int launch_removable(const Ctx& c, const RemovePtrs& o, cudaStream_t st) {
+  if (c.n == 0) return 0;
+  // scratch: the S1 record buffer (16 bytes per cluster) is dead after S1: the good-track map and the keep flags live there
+  int* good_track = reinterpret_cast<int*>(c.rec);
+  unsigned char* keep = reinterpret_cast<unsigned char*>(good_track + c.n);
+  long long g = ((long long)c.n + kThreads - 1) / kThreads;
+  const long long cap = (long long)c.n_sms * 256;
+  if (g > cap) g = cap;
+  long long gk = ((long long)c.max_tracks + kThreads - 1) / kThreads;
+  if (gk > cap) gk = cap;
+  k_track_class<<<(unsigned)gk, kThreads, 0, st>>>(c, o);
+  k_cluster_class<<<(unsigned)g, kThreads, 0, st>>>(c, o, good_track);
+  if (cudaMemsetAsync(keep, 0, (size_t)c.n, st) != cudaSuccess) return -1;   // a dead run marks nothing
+  if (launch_protect(c, good_track, o.road_y, o.road_z, keep, st)) return -1;
+  k_removable<<<(unsigned)g, kThreads, 0, st>>>(c, o, keep);
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
 
 int launch_protect(const Ctx& c, const int* cluster_track, float road_y, float road_z, unsigned char* keep, cudaStream_t st) {
   unsigned char* mark = reinterpret_cast<unsigned char*>(c.flag_scan);      // scratch, free after S3

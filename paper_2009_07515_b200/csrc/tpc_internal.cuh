@@ -152,6 +152,13 @@ struct ApexPtrs {                     // apex links: c
 int launch_apex(const Ctx& c, const MergePtrs& m, const ApexPtrs& o, cudaStream_t st);
 int launches_apex();
 int launch_protect(const Ctx& c, const int* cluster_track, float road_y, float road_z, unsigned char* keep, cudaStream_t st);   // S8
+struct RemovePtrs {                   // hit removal, strategy A
+  float min_pt, max_incl, road_y, road_z;
+  const int* cluster_track; const int* merged_of_track; const int* apex_leg;
+  const float* mrg_par; int mrg_stride; const float* fit_par; int fit_stride;
+  unsigned char* cls; unsigned char* remove;
+};
+int launch_removable(const Ctx& c, const RemovePtrs& o, cudaStream_t st);
 
 // In-place inclusive scan of data[0 .. *n_ptr + n_add) (int32), length known only on the device.
 // max_n bounds the grid; tile_sums needs ceil(max_n / kScanTile) + 1 ints.  total_out (nullable)

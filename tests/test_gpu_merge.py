@@ -220,3 +220,33 @@ def test_merge_in_odd_geometries(S, cfg1):
     mm = trk.merge(out.numpy()["n_tracks"], apex=kw)
     oo = run_oracle(tf, P, last_stage=6).merge(**CUTS).apex(**kw)
     assert np.array_equal(mm["apex_partner"], oo.get("apx_partner"))
+
+
+# ------------------------------------------------------------------------------------------------ strategy-A removal (3.8a)
+@pytest.mark.parametrize("cuts", [dict(min_pt=0.05, max_incl=0.85, road_y=1.0, road_z=1.0),
+                                  dict(min_pt=0.14, max_incl=0.6, road_y=3.0, road_z=0.5),
+                                  dict(min_pt=0.0, max_incl=0.0, road_y=0.0, road_z=0.0)])
+def test_strategy_a_removal_bit_exact(cuts):
+    tf = generate_config("cfg3", n_collisions=3, loopers=True)
+    P, trk, out = run_gpu(tf)
+    cls, rem = trk.removable(out, cuts)
+    o = run_oracle(tf, P, last_stage=6).merge(**CUTS).apex(**APEX).removable(**cuts)
+    assert np.array_equal(cls.cpu().numpy().astype(np.int32), o.get("rem_class"))
+    assert np.array_equal(rem.cpu().numpy().astype(np.int32), o.get("rem_remove"))
+    assert (o.get("rem_class") == 2).sum() > 50000
+
+
+def test_strategy_a_removal_rejects_bad_arguments_and_handles_empty_frames(cfg1):
+    import paper_2009_07515_b200 as tpc
+    P, trk, out = run_gpu(cfg1)
+    for bad in (dict(min_pt=-1.0), dict(road_y=float("nan")), dict(max_incl=-0.1)):
+        with pytest.raises(RuntimeError):
+            trk.removable(out, bad)
+    cls, rem = trk.removable(out)
+    assert int(rem.sum().item()) == 0 and int((cls == 1).sum().item()) == int((out.cluster_track[: cfg1.n] >= 0).sum().item())
+    trk2 = tpc.Tracker(default_params(cfg1), 1024, 4096, 64, 64, 1024)
+    e = [torch.empty(0, dtype=dt, device="cuda") for dt in (torch.uint8, torch.uint8, torch.float32, torch.float32)]
+    o2 = trk2.new_tracks(0)
+    trk2.track_timeframe(*e, o2)
+    cls, rem = trk2.removable(o2)
+    assert cls.numel() == 0 and rem.numel() == 0
