@@ -467,6 +467,21 @@ def run_ours(args):
     torch.cuda.synchronize(dev)
     per_step = np.array([evs[i].elapsed_time(evs[i + 1]) for i in range(reps)])
 
+    # ---- the same step replayed from the cached CUDA graph (tpc_tracker_enable_graph; needs a non-default stream)
+    gs = torch.cuda.Stream(device=dev)
+    trk.enable_graph(True)
+    with torch.cuda.stream(gs):
+        for _ in range(2):
+            trk.track_timeframe(*d_in, out, stream=gs)
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record(gs)
+        for _ in range(args.steps):
+            trk.track_timeframe(*d_in, out, stream=gs)
+        g1.record(gs)
+        gs.synchronize()
+    graph_ms = g0.elapsed_time(g1) / args.steps
+    trk.enable_graph(False)
+
     # ---- per-stage device times (events recorded inside the library, separate untimed-by-value runs)
     trk.enable_stage_timing(True)
     stage = np.zeros(5)
@@ -605,7 +620,7 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "ms_per_step_median": float(np.median(per_step)), "ms_per_step_best": float(per_step.min()),
-        "repeats": int(per_step.size), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "repeats": int(per_step.size), "ms_per_step_cuda_graph": graph_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": tf.name, "n_clusters_per_gpu": tf.n, "n_clusters_total": n_total,
                    "parallelism": "replicas (one time frame per GPU, no collective)" if world > 1 else "single GPU",

@@ -107,7 +107,7 @@ STATUS_BITS = {1: "BAD_CLUSTER", 2: "BINS_OVERFLOW", 4: "SEEDS_OVERFLOW", 8: "TR
 EXPORTS = [
     "tpc_tracker_workspace_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
     "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit", "tpc_tracker_merge", "tpc_tracker_apex", "tpc_tracker_removable", "tpc_tracker_protect",
-    "tpc_tracker_counters", "tpc_tracker_enable_stage_timing", "tpc_tracker_stage_ms", "tpc_tracker_stage_view",
+    "tpc_tracker_counters", "tpc_tracker_enable_graph", "tpc_tracker_enable_stage_timing", "tpc_tracker_stage_ms", "tpc_tracker_stage_view",
     "tpc_tracker_launches_per_call", "tpc_tracker_destroy", "tpc_error_string",
 ]
 
@@ -160,6 +160,8 @@ def load_library(build: bool = True) -> C.CDLL:
     lib.tpc_tracker_protect.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
     lib.tpc_tracker_counters.restype = C.c_int
     lib.tpc_tracker_counters.argtypes = [C.c_void_p, P(tpc_counters_t)]
+    lib.tpc_tracker_enable_graph.restype = C.c_int
+    lib.tpc_tracker_enable_graph.argtypes = [C.c_void_p, C.c_int32]
     lib.tpc_tracker_enable_stage_timing.restype = C.c_int
     lib.tpc_tracker_enable_stage_timing.argtypes = [C.c_void_p, C.c_int32]
     lib.tpc_tracker_stage_ms.restype = C.c_int
@@ -481,6 +483,10 @@ class Tracker:
 
     def enable_stage_timing(self, on: bool = True):
         _check(self.lib, self.lib.tpc_tracker_enable_stage_timing(self._h, int(on)), "tpc_tracker_enable_stage_timing")
+
+    def enable_graph(self, on: bool = True):
+        """Replay a cached CUDA graph of S1..S5 while the arguments of track_timeframe stay the same (non-default stream)."""
+        _check(self.lib, self.lib.tpc_tracker_enable_graph(self._h, int(on)), "tpc_tracker_enable_graph")
 
     def stage_ms(self) -> list[float]:
         ms = (C.c_float * 5)()

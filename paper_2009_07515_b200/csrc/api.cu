@@ -30,6 +30,12 @@ struct tpc_tracker {
   cudaStream_t s_in, s_compute, s_out;                // pipelined path only (host_io >= 2)
   int* h_counts;                                      // pinned host: [slot][4] = n_tracks, status, n_track_clusters, -
   cudaStream_t last_stream;
+  // optional CUDA graph of the S1..S5 launch sequence (tpc_tracker_enable_graph): one cached executable, replayed while the
+  // call's arguments (n and every pointer) stay the same, re-captured when they change
+  bool use_graph;
+  cudaGraphExec_t graph_exec;
+  tpc_clusters_t graph_in;
+  OutPtrs graph_out;
   bool timing;
   cudaEvent_t ev[6];
   int64_t last_n;
@@ -323,7 +329,34 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tr
   if (in->n > t->max_clusters || out->max_tracks > t->max_tracks || out->max_track_clusters > t->max_track_clusters)
     return TPC_ERR_CAPACITY;
   if (!aligned(in->sector, 4) || !aligned(in->row, 4) || !aligned(in->z, 16) || !aligned(in->y, 16)) return TPC_ERR_INVALID_ARG;
-  return run_device(t, in, to_out(out), static_cast<cudaStream_t>(cuda_stream));
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const OutPtrs o = to_out(out);
+  if (!t->use_graph || t->timing || st == nullptr) return run_device(t, in, o, st);   // (the legacy default stream cannot capture)
+  const bool same = t->graph_exec && t->graph_in.n == in->n && t->graph_in.sector == in->sector && t->graph_in.row == in->row &&
+                    t->graph_in.y == in->y && t->graph_in.z == in->z && std::memcmp(&t->graph_out, &o, sizeof(OutPtrs)) == 0;
+  if (!same) {
+    if (t->graph_exec) { cudaGraphExecDestroy(t->graph_exec); t->graph_exec = nullptr; }
+    cudaGraph_t g = nullptr;
+    if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) return TPC_ERR_CUDA;
+    const int rc = run_device(t, in, o, st);
+    const cudaError_t ce = cudaStreamEndCapture(st, &g);
+    if (rc != TPC_OK || ce != cudaSuccess || !g) { if (g) cudaGraphDestroy(g); cudaGetLastError(); return rc != TPC_OK ? rc : TPC_ERR_CUDA; }
+    const cudaError_t ie = cudaGraphInstantiate(&t->graph_exec, g, 0);
+    cudaGraphDestroy(g);
+    if (ie != cudaSuccess) { t->graph_exec = nullptr; return TPC_ERR_CUDA; }
+    t->graph_in = *in; t->graph_out = o;
+  }
+  t->last_stream = st; t->last_n = in->n;
+  t->ctx.n = (int)in->n;
+  t->ctx.in_sector = in->sector; t->ctx.in_row = in->row; t->ctx.in_y = in->y; t->ctx.in_z = in->z;
+  return cudaGraphLaunch(t->graph_exec, st) == cudaSuccess ? TPC_OK : TPC_ERR_CUDA;
+}
+
+int tpc_tracker_enable_graph(tpc_tracker_t* t, int32_t enable) {
+  if (!t) return TPC_ERR_INVALID_ARG;
+  t->use_graph = enable != 0;
+  if (!t->use_graph && t->graph_exec) { cudaGraphExecDestroy(t->graph_exec); t->graph_exec = nullptr; }
+  return TPC_OK;
 }
 
 int tpc_track_timeframe_host(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tracks_t* out, void* cuda_stream) {
@@ -612,6 +645,7 @@ int tpc_tracker_destroy(tpc_tracker_t* t) {
   for (cudaStream_t st : {t->s_in, t->s_compute, t->s_out})
     if (st) cudaStreamDestroy(st);
   if (t->h_counts) cudaFreeHost(t->h_counts);
+  if (t->graph_exec) cudaGraphExecDestroy(t->graph_exec);
   delete t;
   return TPC_OK;
 }
