@@ -49,7 +49,9 @@ enum tpc_error {
   TPC_OK = 0,
   TPC_ERR_INVALID_ARG = -1, /* null pointer, negative size, unsupported geometry (n_rows > 256, ...) */
   TPC_ERR_CAPACITY = -2,    /* workspace too small for the requested capacities, n > max_clusters */
-  TPC_ERR_CUDA = -3         /* a CUDA runtime call or kernel launch failed (cudaGetLastError) */
+  TPC_ERR_CUDA = -3,        /* a CUDA runtime call or kernel launch failed (cudaGetLastError) */
+  TPC_ERR_STATIC_SCRATCH = -4 /* tpc_tracker_protect_static only: the frame has more clusters than the scratch array built
+                                 into the library holds (TPC_PROTECT_STATIC_MAX_CLUSTERS); nothing was enqueued */
 };
 
 enum tpc_status_bits {
@@ -353,6 +355,41 @@ TPC_API int tpc_tracker_apex(tpc_tracker_t* t, const tpc_merged_t* merged, const
  * be ordered after the call; does not synchronise.  INVALID_ARG for null pointers or a negative road. */
 TPC_API int tpc_tracker_protect(tpc_tracker_t* t, const int32_t* cluster_track, float road_y, float road_z, uint8_t* keep,
                                 void* cuda_stream);
+
+/* Largest frame (clusters) tpc_tracker_protect_static accepts = bytes of the scratch array compiled into the library. */
+#define TPC_PROTECT_STATIC_MAX_CLUSTERS 4194304
+
+/* tpc_tracker_protect without any scratch memory from the caller or from an allocator: same inputs, same `keep` output,
+ * same result as tpc_tracker_protect, for frames of at most TPC_PROTECT_STATIC_MAX_CLUSTERS clusters (BASELINE.json
+ * configs 1-4: single sectors, events, slices, pp frames; a 50 kHz Pb-Pb time frame is far beyond it).
+ *
+ * Who it is for.  tpc_tracker_protect keeps one mark byte per cluster in a slice of the handle's workspace; every other
+ * call of this header likewise lives on memory somebody obtained from cudaMalloc and handed in.  Some callers have no
+ * way to get that extra slice: a processing step plugged into a reconstruction framework that reserved the whole card
+ * for its own arena at start-up finds cudaMalloc failing for lack of memory; and code on a latency
+ * path (a trigger-like loop fed frame after frame) must not call cudaMalloc / cudaFree because both stall the whole
+ * device until everything in flight has drained.  For such callers the mark bytes of THIS call live in a fixed array
+ * that is part of the library image (a file-scope __device__ array in csrc/s8_protect.cu):
+ * the call performs no cudaMalloc, cudaFree, or any other allocating routine, and does not touch the workspace slice
+ * the ordinary call uses.
+ *
+ * What that costs and what to watch.
+ *  - Every GPU on which the library's code gets loaded carries the array (4 MiB) until the process exits, used or not.
+ *  - A frame with more clusters than the array has bytes is refused with TPC_ERR_STATIC_SCRATCH before anything is
+ *    enqueued (`keep` is left as it was); use tpc_tracker_protect for those.
+ *  - The first call on each device looks up where the array sits on that device (cudaGetSymbolAddress, checked; the
+ *    address is remembered per device).  Make that first call with the handle's device current and before any stream
+ *    capture is begun; later calls do no set-up.
+ *  - There is ONE array per device, shared by all handles, streams and threads of the process, and it still holds
+ *    the marks of the previous call.  Each call therefore begins by clearing the n bytes it will use (a memset
+ *    enqueued on `cuda_stream`), so back-to-back calls on one stream are fine; two calls whose GPU work may overlap
+ *    (different streams without an ordering between them, or two host threads) race on it and give wrong flags.
+ *    Order them yourself (one stream, or an event between the streams).
+ * Everything else is as for tpc_tracker_protect: `cluster_track` (DEVICE, [n]) from the LAST tpc_track_timeframe on this
+ * handle, `keep` DEVICE [n] bytes, enqueued on `cuda_stream` ordered after that call, no synchronisation.
+ * INVALID_ARG for null pointers or a negative road, STATIC_SCRATCH as above, CUDA if the look-up or a launch failed. */
+TPC_API int tpc_tracker_protect_static(tpc_tracker_t* t, const int32_t* cluster_track, float road_y, float road_z, uint8_t* keep,
+                                       void* cuda_stream);
 
 /* Cuts of the strategy-A hit removal. */
 typedef struct {

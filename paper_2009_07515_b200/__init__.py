@@ -7,6 +7,7 @@ from .binding import (  # noqa: F401
     EXPORTS,
     APEX_CUTS,
     MERGE_CUTS,
+    PROTECT_STATIC_MAX_CLUSTERS,
     REMOVAL_CUTS,
     STATUS_BITS,
     Tracker,

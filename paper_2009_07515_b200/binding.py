@@ -102,11 +102,13 @@ VIEWS = {name: i for i, name in enumerate([
     "fit_row", "up_par", "up_cov", "up_x", "up_zref", "up_row", "up_n",
     "mrg_best_b", "mrg_best_a", "mrg_chi_b", "mrg_next", "mrg_prev", "mrg_dir", "apex_best", "apex_score"])}
 
+PROTECT_STATIC_MAX_CLUSTERS = 4194304   # TPC_PROTECT_STATIC_MAX_CLUSTERS of include/tpc_tracker.h
+
 STATUS_BITS = {1: "BAD_CLUSTER", 2: "BINS_OVERFLOW", 4: "SEEDS_OVERFLOW", 8: "TRACKS_OVERFLOW", 16: "CHAIN_CYCLE"}
 
 EXPORTS = [
     "tpc_tracker_workspace_bytes", "tpc_tracker_create", "tpc_track_timeframe", "tpc_track_timeframe_host",
-    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit", "tpc_tracker_merge", "tpc_tracker_apex", "tpc_tracker_removable", "tpc_tracker_protect",
+    "tpc_track_timeframe_host_begin", "tpc_track_timeframe_host_end", "tpc_tracker_refit", "tpc_tracker_merge", "tpc_tracker_apex", "tpc_tracker_removable", "tpc_tracker_protect", "tpc_tracker_protect_static",
     "tpc_tracker_counters", "tpc_tracker_enable_graph", "tpc_tracker_enable_stage_timing", "tpc_tracker_stage_ms", "tpc_tracker_stage_view",
     "tpc_tracker_launches_per_call", "tpc_tracker_destroy", "tpc_error_string",
 ]
@@ -158,6 +160,8 @@ def load_library(build: bool = True) -> C.CDLL:
                                           C.c_void_p, C.c_void_p, C.c_void_p]
     lib.tpc_tracker_protect.restype = C.c_int
     lib.tpc_tracker_protect.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
+    lib.tpc_tracker_protect_static.restype = C.c_int
+    lib.tpc_tracker_protect_static.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
     lib.tpc_tracker_counters.restype = C.c_int
     lib.tpc_tracker_counters.argtypes = [C.c_void_p, P(tpc_counters_t)]
     lib.tpc_tracker_enable_graph.restype = C.c_int
@@ -474,6 +478,19 @@ class Tracker:
             keep = torch.empty(max(1, out.n_in), dtype=torch.uint8, device=self.device)
         _check(self.lib, self.lib.tpc_tracker_protect(self._h, out.cluster_track.data_ptr(), float(road_y), float(road_z),
                                                       keep.data_ptr(), C.c_void_p(st.cuda_stream)), "tpc_tracker_protect")
+        return keep
+
+    def protect_static(self, out: Tracks, road_y: float, road_z: float, keep, stream=None):
+        """tpc_tracker_protect_static: the flags of `protect` for a frame of at most PROTECT_STATIC_MAX_CLUSTERS clusters,
+        computed without any device allocation - the per-cluster scratch is an array inside the library, not workspace or
+        cudaMalloc memory (for callers whose framework owns all GPU memory, or that may not stall the device with an
+        allocation).  `keep` (uint8 device tensor [n]) must be passed in: this wrapper does not allocate either.  One
+        array per device, shared by everybody: calls that could overlap on the GPU must be ordered by the caller.  The
+        first call on a device looks the array up; make it before any stream capture.  Raises on larger frames."""
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        assert keep.is_cuda and keep.dtype == torch.uint8 and keep.numel() >= out.n_in
+        _check(self.lib, self.lib.tpc_tracker_protect_static(self._h, out.cluster_track.data_ptr(), float(road_y), float(road_z),
+                                                             keep.data_ptr(), C.c_void_p(st.cuda_stream)), "tpc_tracker_protect_static")
         return keep
 
     def counters(self) -> dict:

@@ -547,6 +547,17 @@ int tpc_tracker_protect(tpc_tracker_t* t, const int32_t* cluster_track, float ro
   return launch_protect(t->ctx, cluster_track, road_y, road_z, keep, st) ? TPC_ERR_CUDA : TPC_OK;
 }
 
+// Strategy-B protection with the mark bytes in the static array of s8_protect.cu (see the header): no cudaMalloc / cudaFree,
+// no workspace scratch.  The size check comes first so that an oversized frame enqueues nothing.
+int tpc_tracker_protect_static(tpc_tracker_t* t, const int32_t* cluster_track, float road_y, float road_z, uint8_t* keep,
+                               void* cuda_stream) {
+  if (!t || !keep || !cluster_track || !(road_y >= 0.f) || !(road_z >= 0.f)) return TPC_ERR_INVALID_ARG;
+  if (t->last_n > (int64_t)TPC_PROTECT_STATIC_MAX_CLUSTERS) return TPC_ERR_STATIC_SCRATCH;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  t->last_stream = st;
+  return launch_protect_static(t->ctx, cluster_track, road_y, road_z, keep, st) ? TPC_ERR_CUDA : TPC_OK;
+}
+
 int tpc_tracker_counters(tpc_tracker_t* t, tpc_counters_t* out) {
   if (!t || !out) return TPC_ERR_INVALID_ARG;
   Counters k;
@@ -656,6 +667,7 @@ const char* tpc_error_string(int code) {
     case TPC_ERR_INVALID_ARG: return "invalid argument";
     case TPC_ERR_CAPACITY: return "capacity exceeded";
     case TPC_ERR_CUDA: return "CUDA error";
+    case TPC_ERR_STATIC_SCRATCH: return "frame has more clusters than the library's built-in scratch array holds (TPC_PROTECT_STATIC_MAX_CLUSTERS)";
     default: return "unknown error";
   }
 }

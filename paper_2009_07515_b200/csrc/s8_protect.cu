@@ -4,12 +4,21 @@
 // clusters and the grid the last tpc_track_timeframe left in the workspace and the caller's cluster_track array.
 //   k_mark   thread per sorted position: an owned cluster marks the members of the rectangle around itself
 //   k_out    keep[input index] = mark[sorted position]
+#include <mutex>
+
+#include "../../include/tpc_tracker.h"
 #include "tpc_internal.cuh"
 
 namespace tpc {
 namespace {
 
 constexpr int kThreads = 256;
+
+// Mark bytes of tpc_tracker_protect_static (include/tpc_tracker.h): one byte per sorted position, in an array that is part
+// of the library image instead of the caller's workspace, for callers that cannot obtain device memory at run time.
+// One copy per device that loads this module, shared by every handle and stream of the process.  In HOST code this
+// name is only a handle for cudaGetSymbolAddress - it is not a device address and must never be handed to a kernel.
+static __device__ __align__(256) unsigned char g_static_mark[TPC_PROTECT_STATIC_MAX_CLUSTERS];
 
 __global__ void __launch_bounds__(kThreads) k_mark(Ctx c, const int* __restrict__ cluster_track, float road_y, float road_z,
                                                    unsigned char* __restrict__ mark) {
@@ -95,6 +104,39 @@ int launch_removable(const Ctx& c, const RemovePtrs& o, cudaStream_t st) {
 int launch_protect(const Ctx& c, const int* cluster_track, float road_y, float road_z, unsigned char* keep, cudaStream_t st) {
   unsigned char* mark = reinterpret_cast<unsigned char*>(c.flag_scan);      // scratch, free after S3
   if (c.n == 0) return 0;
+  if (cudaMemsetAsync(mark, 0, (size_t)c.n, st) != cudaSuccess) return -1;
+  long long g = ((long long)c.n + kThreads - 1) / kThreads;
+  const long long cap = (long long)c.n_sms * 256;
+  if (g > cap) g = cap;
+  k_mark<<<(unsigned)g, kThreads, 0, st>>>(c, cluster_track, road_y, road_z, mark);
+  k_out<<<(unsigned)g, kThreads, 0, st>>>(c, mark, keep);
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+// ---- tpc_tracker_protect_static: the same two kernels, the marks in g_static_mark.  No allocation of any kind here.
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mutex;
+unsigned char* g_static_mark_addr[kMaxDevices];   // device address of g_static_mark per device ordinal; null = not looked up yet
+}  // namespace
+
+int launch_protect_static(const Ctx& c, const int* cluster_track, float road_y, float road_z, unsigned char* keep, cudaStream_t st) {
+  if (c.n == 0) return 0;
+  if ((long long)c.n > (long long)TPC_PROTECT_STATIC_MAX_CLUSTERS) return -1;   // (the C entry point has refused this already)
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return -1;
+  unsigned char* mark = nullptr;
+  {
+    // first call on this device: ask the runtime where the array lives HERE (the current device's copy)
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    mark = g_static_mark_addr[dev];
+    if (!mark) {
+      void* p = nullptr;
+      if (cudaGetSymbolAddress(&p, g_static_mark) != cudaSuccess || !p) { cudaGetLastError(); return -1; }
+      mark = g_static_mark_addr[dev] = static_cast<unsigned char*>(p);
+    }
+  }
+  // the array still holds the previous call's marks: clear the part this frame uses, on the caller's stream
   if (cudaMemsetAsync(mark, 0, (size_t)c.n, st) != cudaSuccess) return -1;
   long long g = ((long long)c.n + kThreads - 1) / kThreads;
   const long long cap = (long long)c.n_sms * 256;

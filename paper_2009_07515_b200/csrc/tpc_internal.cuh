@@ -152,6 +152,8 @@ struct ApexPtrs {                     // apex links: c
 int launch_apex(const Ctx& c, const MergePtrs& m, const ApexPtrs& o, cudaStream_t st);
 int launches_apex();
 int launch_protect(const Ctx& c, const int* cluster_track, float road_y, float road_z, unsigned char* keep, cudaStream_t st);   // S8
+// the same with the mark bytes in the library's own static array (n <= TPC_PROTECT_STATIC_MAX_CLUSTERS); allocates nothing
+int launch_protect_static(const Ctx& c, const int* cluster_track, float road_y, float road_z, unsigned char* keep, cudaStream_t st);
 struct RemovePtrs {                   // hit removal, strategy A
   float min_pt, max_incl, road_y, road_z;
   const int* cluster_track; const int* merged_of_track; const int* apex_leg;
