@@ -379,11 +379,12 @@ class Tracker:
                     z_ref=out["z_ref"][:T].copy(), chi2=out["chi2"][:T].copy(), ndf=out["ndf"][:T].copy(),
                     n_fit=out["n_fit"][:T].copy())
 
-    def new_merged(self) -> dict:
-        """Device buffers for tpc_tracker_merge (layouts as in tpc_merged_t)."""
+    def new_merged(self, fill: int = 0) -> dict:
+        """Device buffers for tpc_tracker_merge (layouts as in tpc_merged_t); the integer ones pre-filled with `fill`
+        (tests pass a poison value to see that every entry the header promises is really written)."""
         mt, dev = self.caps[3], self.device
         f32 = lambda *s: torch.empty(*s, dtype=torch.float32, device=dev)   # noqa: E731
-        i32 = lambda *s: torch.zeros(*s, dtype=torch.int32, device=dev)     # noqa: E731
+        i32 = lambda *s: torch.full(s, int(fill), dtype=torch.int32, device=dev)     # noqa: E731
         return dict(n_merged=i32(1), merged_of_track=i32(mt), seg_start=i32(mt + 1), seg_idx=i32(mt), par=f32(5, mt),
                     cov=f32(15, mt), x_ref=f32(mt), z_ref=f32(mt), chi2=f32(mt), ndf=i32(mt), n_fit=i32(mt), sector=i32(mt),
                     n_clusters=i32(mt))
@@ -423,11 +424,12 @@ class Tracker:
         _check(self.lib, self.lib.tpc_tracker_apex(self._h, C.byref(m), C.byref(c), C.byref(o), C.c_void_p(st.cuda_stream)),
                "tpc_tracker_apex")
 
-    def removable(self, out: "Tracks", cuts: dict | None = None, merge_cuts: dict | None = None, apex_cuts: dict | None = None):
+    def removable(self, out: "Tracks", cuts: dict | None = None, merge_cuts: dict | None = None, apex_cuts: dict | None = None,
+                  fill: int = 0):
         """Convenience: refit + merge + apex + tpc_tracker_removable for the last track_timeframe call (outputs `out`);
-        returns (cls, remove) as uint8 device tensors [n]."""
+        returns (cls, remove) as uint8 device tensors [n].  `fill`: see new_merged."""
         st = torch.cuda.current_stream(self.device)
-        fit = self.new_fit(); mg = self.new_merged(); ax = self.new_apex()
+        fit = self.new_fit(); mg = self.new_merged(fill); ax = self.new_apex()
         self.refit_into(fit); self.merge_into(fit, mg, merge_cuts); self.apex_into(mg, ax, apex_cuts)
         f = tpc_fit_t(); f.max_tracks = self.caps[3]
         for k in ("par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit"):
@@ -451,10 +453,10 @@ class Tracker:
         mt, dev = self.caps[3], self.device
         return dict(apex_partner=torch.zeros(mt, dtype=torch.int32, device=dev), apex_leg=torch.zeros(mt, dtype=torch.int32, device=dev))
 
-    def merge(self, n_tracks: int, cuts: dict | None = None, apex: dict | bool | None = None) -> dict:
+    def merge(self, n_tracks: int, cuts: dict | None = None, apex: dict | bool | None = None, fill: int = 0) -> dict:
         """Convenience: refit + merge (+ apex links when `apex` is True or a dict of cuts) + host copies trimmed to the
-        tracks / merged tracks found."""
-        fit = self.new_fit(); mg = self.new_merged()
+        tracks / merged tracks found.  `fill`: see new_merged."""
+        fit = self.new_fit(); mg = self.new_merged(fill)
         self.refit_into(fit)
         self.merge_into(fit, mg, cuts)
         extra = {}

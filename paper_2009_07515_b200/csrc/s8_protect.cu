@@ -52,7 +52,10 @@ __global__ void __launch_bounds__(kThreads) k_track_class(Ctx c, RemovePtrs o) {
   const int nt = c.cnt->status ? 0 : min(c.cnt->n_tracks, c.max_tracks);
   const size_t mt = (size_t)c.max_tracks, ft = (size_t)o.fit_stride, gt = (size_t)o.mrg_stride;
   for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nt; k += gridDim.x * blockDim.x) {
-    const int m = o.merged_of_track[k];
+    // a track outside every merged track (-1: link cycle), a merge that did not run (status bit) or an id
+    // that cannot be one is classified from its own segment only - and never used as an index
+    int m = o.merged_of_track[k];
+    if (c.mcnt->status || m >= c.mcnt->n_merged) m = -1;
     int cls = 1;
     if (m >= 0 && o.apex_leg[m] == 1) cls = 2;
     else if (m >= 0 && fabsf(o.mrg_par[4 * gt + m]) * o.min_pt > 1.0f) cls = 3;

@@ -150,6 +150,9 @@ __global__ void __launch_bounds__(kThreads) k_merge_clear(Ctx c, MergePtrs o) {
     c.m_best_b[i] = -1; c.m_chi_b[i] = -1.0f; c.m_dir_b[i] = 0;
     c.m_best_a[i] = ~0ull;
     c.m_next[i] = -1; c.m_prev[i] = -1; c.m_dir[i] = 0;
+    // -1 = in no merged track: what a track keeps when no chain head reaches it (a cycle of links) and
+    // what every track has when the run was aborted by a status bit - never the previous content of the caller's buffer
+    o.merged_of_track[i] = -1;
   }
 }
 

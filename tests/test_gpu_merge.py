@@ -204,6 +204,44 @@ def test_merge_and_apex_on_an_empty_frame_and_after_a_status_bit(cfg1):
     assert m2["n_merged"] == 0
 
 
+POISON = 0x7F7F7F7F
+WILD = dict(max_rows=150, back_rows=150, edge=1000.0, dz_win=200.0, chi2_cut=1e30, road_z0=1e3, road_z1=1e3)
+
+
+def test_link_cycles_get_minus_one_and_never_the_callers_garbage():
+    """With cuts this loose (any row distance, any chi2) mutual links close into cycles: no chain head reaches those
+    tracks, the oracle leaves them at -1 (DESIGN.md 3.9.6) and so must the kernel, whatever the caller's buffer held;
+    the hit removal then classifies them from their own segment (no index taken from a -1)."""
+    tf = generate_config("cfg3", n_collisions=3, loopers=True)
+    P, trk, out = run_gpu(tf)
+    T = out.numpy()["n_tracks"]
+    m = trk.merge(T, WILD, fill=POISON)
+    o = run_oracle(tf, P, last_stage=6).merge(**WILD)
+    want = o.get("mrg_of_track")
+    assert int((want < 0).sum()) >= 50                     # the case is really there
+    assert np.array_equal(m["merged_of_track"], want)
+    assert m["n_merged"] == o.get("mrg_seg_start").size - 1
+    assert np.array_equal(m["seg_start"], o.get("mrg_seg_start"))
+    assert np.array_equal(m["seg_idx"][: int(m["seg_start"][-1])], o.get("mrg_seg_idx"))
+    assert np.array_equal(m["par"], o.get("mrg_par").astype(np.float32).reshape(-1, 5))
+    cuts = dict(min_pt=0.05, max_incl=0.85, road_y=1.0, road_z=1.0)
+    cls, rem = trk.removable(out, cuts, merge_cuts=WILD, fill=POISON)
+    oo = o.apex(**APEX).removable(**cuts)
+    assert np.array_equal(cls.cpu().numpy().astype(np.int32), oo.get("rem_class"))
+    assert np.array_equal(rem.cpu().numpy().astype(np.int32), oo.get("rem_remove"))
+
+
+def test_merge_and_removal_after_a_status_bit_write_defined_values_into_poisoned_buffers(cfg1):
+    """A frame aborted by a status bit has no tracks: the merger reports none and the hit removal marks every cluster as
+    not attached and not removable, also when the caller's buffers were full of garbage."""
+    _, trk, out = run_gpu(cfg1, caps=dict(max_seeds=4))
+    assert out.numpy()["status"] & 4 and out.numpy()["n_tracks"] == 0
+    m = trk.merge(0, apex=True, fill=POISON)
+    assert m["n_merged"] == 0 and m["seg_start"].tolist() == [0]
+    cls, rem = trk.removable(out, fill=POISON)
+    assert int(cls.max().item()) == 0 and int(rem.max().item()) == 0
+
+
 @pytest.mark.parametrize("S", [1, 2, 5])
 def test_merge_in_odd_geometries(S, cfg1):
     """One sector (no neighbour), two sectors, an odd count: same results as the oracle, no neighbour arithmetic blows up."""
