@@ -280,7 +280,9 @@ typedef struct {
 /* Refit of every track of the LAST tpc_track_timeframe call on this handle over the clusters it owns after the
  * selector, top row downwards (the first slice of "Track Fit").  Enqueued on
  * `cuda_stream`, which must be ordered after that call; does not synchronise; entries [0, n_tracks) are written.
- * Not part of tpc_track_timeframe (and not of the timed hot path).  CAPACITY if out->max_tracks exceeds the tracker's. */
+ * Not part of tpc_track_timeframe (and not of the timed hot path).  CAPACITY if out->max_tracks exceeds the tracker's or
+ * is smaller than the max_tracks of that tpc_track_timeframe call (every track it may have found must fit: this call and
+ * the four below never cut a result off silently; the same rule holds for every max_tracks they are given). */
 TPC_API int tpc_tracker_refit(tpc_tracker_t* t, const tpc_fit_t* out, void* cuda_stream);
 
 /* Cuts of the track merger. */
@@ -319,7 +321,8 @@ typedef struct {
  * downward pass through all segments with the frame turned at sector changes).  `fit` is the output of the
  * tpc_tracker_refit call that followed that tpc_track_timeframe (DEVICE; its residual fields are not used).  Enqueued on
  * `cuda_stream`, which must be ordered after both; does not synchronise; entries [0, n_merged) / [0, n_tracks) are written.
- * INVALID_ARG for null pointers or cuts out of range, CAPACITY if a max_tracks exceeds the tracker's. */
+ * INVALID_ARG for null pointers or cuts out of range, CAPACITY if a max_tracks (fit, out) exceeds the tracker's or is smaller
+ * than the max_tracks of that tpc_track_timeframe call. */
 TPC_API int tpc_tracker_merge(tpc_tracker_t* t, const tpc_fit_t* fit, const tpc_merge_cuts_t* cuts, const tpc_merged_t* out,
                               void* cuda_stream);
 
@@ -344,7 +347,8 @@ typedef struct {
  * of looping tracks"): pairs the merged tracks of the LAST tpc_tracker_merge call on this handle that are the outgoing
  * and the returning leg of one track curling up inside the TPC, by comparing the circles of their outermost states, and
  * labels the returning leg.  `merged` is that call's output (DEVICE; seg_start / seg_idx are read).  Enqueued on
- * `cuda_stream`, ordered after the merge; does not synchronise; entries [0, n_merged) are written. */
+ * `cuda_stream`, ordered after the merge; does not synchronise; entries [0, n_merged) are written.  CAPACITY as for
+ * tpc_tracker_merge (merged, out). */
 TPC_API int tpc_tracker_apex(tpc_tracker_t* t, const tpc_merged_t* merged, const tpc_apex_cuts_t* cuts, const tpc_apex_t* out,
                              void* cuda_stream);
 
@@ -408,7 +412,7 @@ typedef struct {
  * remove[i] (DEVICE, [n] bytes) 1 iff cls[i] >= 2 and the cluster does not lie, in its own (sector, row), within the road
  *           of a cluster owned by a good track.
  * Enqueued on `cuda_stream`, ordered after those calls; does not synchronise.  The S1 record scratch of the workspace is
- * reused (the next tpc_track_timeframe overwrites it anyway). */
+ * reused (the next tpc_track_timeframe overwrites it anyway).  CAPACITY as for tpc_tracker_merge (fit, merged, apex). */
 TPC_API int tpc_tracker_removable(tpc_tracker_t* t, const int32_t* cluster_track, const tpc_fit_t* fit, const tpc_merged_t* merged,
                                   const tpc_apex_t* apex, const tpc_removal_cuts_t* cuts, uint8_t* cls, uint8_t* remove,
                                   void* cuda_stream);

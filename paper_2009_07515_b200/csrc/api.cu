@@ -39,6 +39,7 @@ struct tpc_tracker {
   bool timing;
   cudaEvent_t ev[6];
   int64_t last_n;
+  int64_t last_max_tracks;        // out->max_tracks of the last track call: n_tracks <= it (S5 raises TRACKS_OVERFLOW otherwise)
 };
 
 namespace {
@@ -201,6 +202,7 @@ int run_device(tpc_tracker* t, const tpc_clusters_t* in, const OutPtrs& o, cudaS
   c.in_sector = in->sector; c.in_row = in->row; c.in_y = in->y; c.in_z = in->z;
   t->last_stream = st;
   t->last_n = in->n;
+  t->last_max_tracks = o.max_tracks;
   const bool tm = t->timing;
   if (tm) cudaEventRecord(t->ev[0], st);
   if (launch_reset(c, st)) return TPC_ERR_CUDA;
@@ -346,7 +348,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tr
     if (ie != cudaSuccess) { t->graph_exec = nullptr; return TPC_ERR_CUDA; }
     t->graph_in = *in; t->graph_out = o;
   }
-  t->last_stream = st; t->last_n = in->n;
+  t->last_stream = st; t->last_n = in->n; t->last_max_tracks = o.max_tracks;
   t->ctx.n = (int)in->n;
   t->ctx.in_sector = in->sector; t->ctx.in_row = in->row; t->ctx.in_y = in->y; t->ctx.in_z = in->z;
   return cudaGraphLaunch(t->graph_exec, st) == cudaSuccess ? TPC_OK : TPC_ERR_CUDA;
@@ -458,7 +460,8 @@ int tpc_track_timeframe_host_end(tpc_tracker_t* t, const tpc_tracks_t* out, int3
 int tpc_tracker_refit(tpc_tracker_t* t, const tpc_fit_t* out, void* cuda_stream) {
   if (!t || !out || !out->par || !out->cov || !out->x_ref || !out->z_ref || !out->chi2 || !out->ndf || !out->n_fit)
     return TPC_ERR_INVALID_ARG;
-  if (out->max_tracks < 1 || out->max_tracks > t->max_tracks) return TPC_ERR_CAPACITY;
+  // room for every track the last frame can have found (its out->max_tracks): nothing is ever cut off silently
+  if (out->max_tracks < 1 || out->max_tracks > t->max_tracks || out->max_tracks < t->last_max_tracks) return TPC_ERR_CAPACITY;
   FitPtrs o;
   o.par = out->par; o.cov = out->cov; o.x_ref = out->x_ref; o.z_ref = out->z_ref; o.chi2 = out->chi2; o.ndf = out->ndf;
   o.n_fit = out->n_fit; o.max_tracks = (int)out->max_tracks;
@@ -482,6 +485,8 @@ int tpc_tracker_merge(tpc_tracker_t* t, const tpc_fit_t* fit, const tpc_merge_cu
     return TPC_ERR_INVALID_ARG;
   if (fit->max_tracks < 1 || fit->max_tracks > t->max_tracks || out->max_tracks < 1 || out->max_tracks > t->max_tracks)
     return TPC_ERR_CAPACITY;
+  // the kernels index `fit` and `out` by track id up to n_tracks: both must hold every track of the last frame
+  if (fit->max_tracks < t->last_max_tracks || out->max_tracks < t->last_max_tracks) return TPC_ERR_CAPACITY;
   FitPtrs f{};
   f.par = fit->par; f.cov = fit->cov; f.x_ref = fit->x_ref; f.z_ref = fit->z_ref; f.chi2 = fit->chi2; f.ndf = fit->ndf;
   f.n_fit = fit->n_fit; f.max_tracks = (int)fit->max_tracks;
@@ -507,7 +512,10 @@ int tpc_tracker_apex(tpc_tracker_t* t, const tpc_merged_t* merged, const tpc_ape
   if (cuts->max_k < 0 || !(cuts->min_s >= 0.f) || !(cuts->dz_win > 0.f) || !(cuts->dz_win < INFINITY) || !(cuts->tol_c > 0.f) ||
       !(cuts->tol_z > 0.f) || !(cuts->tol_t > 0.f) || !(cuts->cut >= 0.f))
     return TPC_ERR_INVALID_ARG;
-  if (out->max_tracks < 1 || out->max_tracks > t->max_tracks || merged->max_tracks > t->max_tracks) return TPC_ERR_CAPACITY;
+  if (out->max_tracks < 1 || out->max_tracks > t->max_tracks || merged->max_tracks < 1 || merged->max_tracks > t->max_tracks)
+    return TPC_ERR_CAPACITY;
+  // entries [0, n_merged) are read / written and n_merged <= n_tracks <= the last frame's max_tracks
+  if (out->max_tracks < t->last_max_tracks || merged->max_tracks < t->last_max_tracks) return TPC_ERR_CAPACITY;
   MergePtrs m{};
   const float th = t->params.tan_half_sector;
   const float den = 1.0f + th * th;
@@ -527,7 +535,10 @@ int tpc_tracker_removable(tpc_tracker_t* t, const int32_t* cluster_track, const 
   if (!t || !cluster_track || !fit || !merged || !apex || !cuts || !cls || !remove) return TPC_ERR_INVALID_ARG;
   if (!fit->par || !merged->merged_of_track || !merged->par || !apex->apex_leg) return TPC_ERR_INVALID_ARG;
   if (!(cuts->min_pt >= 0.f) || !(cuts->max_incl >= 0.f) || !(cuts->road_y >= 0.f) || !(cuts->road_z >= 0.f)) return TPC_ERR_INVALID_ARG;
-  if (fit->max_tracks > t->max_tracks || merged->max_tracks > t->max_tracks || fit->max_tracks < 1 || merged->max_tracks < 1)
+  if (fit->max_tracks > t->max_tracks || merged->max_tracks > t->max_tracks || fit->max_tracks < 1 || merged->max_tracks < 1 ||
+      apex->max_tracks < 1 || apex->max_tracks > t->max_tracks)
+    return TPC_ERR_CAPACITY;
+  if (fit->max_tracks < t->last_max_tracks || merged->max_tracks < t->last_max_tracks || apex->max_tracks < t->last_max_tracks)
     return TPC_ERR_CAPACITY;
   RemovePtrs o{};
   o.min_pt = cuts->min_pt; o.max_incl = cuts->max_incl; o.road_y = cuts->road_y; o.road_z = cuts->road_z;

@@ -141,6 +141,62 @@ def test_merge_rejects_bad_arguments(cfg1):
     assert int(mg["n_merged"].item()) >= 1
 
 
+def test_buffers_smaller_than_the_frames_max_tracks_are_refused(cfg1):
+    """refit / merge / apex / removable index their per-track buffers by track id up to n_tracks <= the max_tracks of the
+    tpc_track_timeframe call: any buffer declared smaller than that is CAPACITY (-2) - no out-of-bounds access, no
+    silently shortened result."""
+    import ctypes as C
+    import paper_2009_07515_b200 as tpc
+    from paper_2009_07515_b200.binding import (_MERGED_FIELDS, tpc_apex_cuts_t, tpc_apex_t, tpc_fit_t, tpc_merge_cuts_t,
+                                               tpc_merged_t, tpc_removal_cuts_t)
+    P, trk, out = run_gpu(cfg1)
+    lib, h, mt = trk.lib, trk._h, trk.caps[3]
+    st = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    fit = trk.new_fit(); mg = trk.new_merged(); ax = trk.new_apex()
+
+    def fit_s(n):
+        f = tpc_fit_t(); f.max_tracks = n
+        for k in ("par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit"):
+            setattr(f, k, fit[k].data_ptr())
+        return f
+
+    def mrg_s(n):
+        m = tpc_merged_t(); m.max_tracks = n
+        for k in _MERGED_FIELDS:
+            setattr(m, k, mg[k].data_ptr())
+        return m
+
+    def apx_s(n):
+        a = tpc_apex_t(); a.max_tracks = n
+        a.apex_partner = ax["apex_partner"].data_ptr(); a.apex_leg = ax["apex_leg"].data_ptr()
+        return a
+    mc = tpc_merge_cuts_t(30, 1, 6.0, 50.0, 100.0, 2.0, 0.3)
+    ac = tpc_apex_cuts_t(4, 0.6, 150.0, 0.1, 4.0, 0.1, 3.0)
+    rc = tpc_removal_cuts_t(0.05, 0.85, 1.0, 1.0)
+    cls = torch.zeros(cfg1.n, dtype=torch.uint8, device="cuda"); rem = torch.zeros_like(cls)
+    small = mt - 1
+    assert lib.tpc_tracker_refit(h, C.byref(fit_s(small)), st) == -2
+    assert lib.tpc_tracker_refit(h, C.byref(fit_s(mt)), st) == 0
+    assert lib.tpc_tracker_merge(h, C.byref(fit_s(small)), C.byref(mc), C.byref(mrg_s(mt)), st) == -2
+    assert lib.tpc_tracker_merge(h, C.byref(fit_s(mt)), C.byref(mc), C.byref(mrg_s(small)), st) == -2
+    assert lib.tpc_tracker_merge(h, C.byref(fit_s(mt)), C.byref(mc), C.byref(mrg_s(mt)), st) == 0
+    assert lib.tpc_tracker_apex(h, C.byref(mrg_s(small)), C.byref(ac), C.byref(apx_s(mt)), st) == -2
+    assert lib.tpc_tracker_apex(h, C.byref(mrg_s(mt)), C.byref(ac), C.byref(apx_s(small)), st) == -2
+    assert lib.tpc_tracker_apex(h, C.byref(mrg_s(mt)), C.byref(ac), C.byref(apx_s(mt)), st) == 0
+    ct = out.cluster_track.data_ptr()
+    for f_n, m_n, a_n, want in ((small, mt, mt, -2), (mt, small, mt, -2), (mt, mt, small, -2), (mt, mt, mt + 1, -2), (mt, mt, mt, 0)):
+        got = lib.tpc_tracker_removable(h, ct, C.byref(fit_s(f_n)), C.byref(mrg_s(m_n)), C.byref(apx_s(a_n)), C.byref(rc),
+                                        cls.data_ptr(), rem.data_ptr(), st)
+        assert got == want, (f_n, m_n, a_n, got)
+    torch.cuda.synchronize()
+    # a frame tracked with a smaller max_tracks lowers the bar accordingly
+    out_small = tpc.Tracks(cfg1.n, 64, trk.caps[4], trk.device)
+    ins = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (cfg1.sector, cfg1.row, cfg1.y, cfg1.z)]
+    trk.track_timeframe(*ins, out_small)
+    assert lib.tpc_tracker_refit(h, C.byref(fit_s(64)), st) == 0 and lib.tpc_tracker_refit(h, C.byref(fit_s(63)), st) == -2
+    torch.cuda.synchronize()
+
+
 # ------------------------------------------------------------------------------------------------ apex links (3.9.8)
 APEX = dict(max_k=4, min_s=0.6, dz_win=150.0, tol_c=0.1, tol_z=4.0, tol_t=0.1, cut=3.0)
 
