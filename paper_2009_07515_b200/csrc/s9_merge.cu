@@ -216,12 +216,13 @@ __global__ void __launch_bounds__(kThreads) k_refit_up(Ctx c, FitPtrs f, MergePt
     const float z_in = f.z_ref[id] + f.par[1 * ft + id];
     c.m_zin[id] = z_in;
     c.m_zout[id] = zref + k.p[1];
-    // the inner end goes into its (sector, z) bin (every track: those that take no part are skipped when read)
-    const int b = merge_bin(c, sector, z_in, inv_w);
+    // the inner end goes into its (sector, z) bin (every track: those that take no part are skipped when read) - unless
+    // its sector has no grid (a track without an owned row is filed under sector 0, which may be empty): no bin then
+    const int b = c.m_nzb[sector] > 0 ? merge_bin(c, sector, z_in, inv_w) : -1;
     c.m_bin_of[id] = b;
     // the record the candidate scan reads: z_in, the row of the inner state (-1: takes no part), the id, x of the inner state
     c.m_rec[id] = make_float4(z_in, __int_as_float(nfit >= 2 && f.n_fit[id] >= 2 ? c.fit_row[id] : -1), __int_as_float(id), f.x_ref[id]);
-    atomicAdd(c.m_bin_start + b + 1, 1);              // counts at b + 1: the inclusive scan leaves the CSR starts in place
+    if (b >= 0) atomicAdd(c.m_bin_start + b + 1, 1);  // counts at b + 1: the inclusive scan leaves the CSR starts in place
   }
 }
 
@@ -230,6 +231,7 @@ __global__ void __launch_bounds__(kThreads) k_merge_fill(Ctx c, MergePtrs o) {
   const int nt = n_tracks_of(c, o);
   for (int id = blockIdx.x * blockDim.x + threadIdx.x; id < nt; id += gridDim.x * blockDim.x) {
     const int b = c.m_bin_of[id];
+    if (b < 0) continue;
     const int pos = c.m_bin_start[b] + atomicAdd(c.m_bin_fill + b, 1);
     c.m_srec[pos] = c.m_rec[id];
   }
@@ -309,7 +311,7 @@ __global__ void __launch_bounds__(kThreads) k_merge_match(Ctx c, FitPtrs f, Merg
         if (bb < 0 || chi < best || (chi == best && b < bb)) { best = chi; bb = b; bdir = dir; }
         // high word: order-preserving unsigned key of chi (fp32 variances can come out slightly negative, and then so
         // does chi); low word = id -> ties go to the lowest a
-        const unsigned cb = __float_as_uint(chi);
+        const unsigned cb = __float_as_uint(chi + 0.0f);   // -0 -> +0: the oracle's `chi == best` makes no difference between them
         const unsigned ck = (cb & 0x80000000u) ? ~cb : (cb | 0x80000000u);
         atomicMin(c.m_best_a + b, ((unsigned long long)ck << 32) | (unsigned)a);
       }
