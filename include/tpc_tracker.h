@@ -24,6 +24,10 @@
  * from different threads or streams concurrently.  tpc_error_string and tpc_tracker_workspace_bytes
  * touch no handle and are thread-safe.
  *
+ * Call order: tpc_tracker_refit, _merge, _apex and _removable work on the frame of the LAST track call on the handle
+ * and read what their predecessors left in the workspace, so each returns INVALID_ARG unless its predecessors ran after
+ * that track call: refit needs a tracked frame, merge the refit, apex the merge, removable the merge and the apex.
+ *
  * Error behaviour: functions return 0 (TPC_OK) or a negative tpc_error code; device-detected
  * conditions (bad sector/row value, capacity overflow) are reported through the 32-bit status word
  * (tpc_tracks_t.status, tpc_counters_t.status) as a bit set of TPC_STATUS_*; when a status bit is
@@ -248,7 +252,8 @@ TPC_API int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, cons
  * CUDA graph the first time and replays the cached executable while n and every pointer of `in` / `out` stay the same; a
  * call with other arguments re-captures.  Worth 0.05 - 0.07 ms per call (5 - 7 % of the small configurations, whose floor
  * is the serial depth of one tracklet; nothing on a full time frame).  Not used while stage timing is on, on the default
- * stream, or by the host paths.  The handle owns the graph executable (released by tpc_tracker_destroy). */
+ * stream, by the host paths, or when `cuda_stream` is already being captured by the caller (the launches then go into
+ * the caller's capture as they are).  The handle owns the graph executable (released by tpc_tracker_destroy). */
 TPC_API int tpc_tracker_enable_graph(tpc_tracker_t* t, int32_t enable);
 
 /* Same from/to HOST buffers (tracker created with host_io != 0): copies the SoA input to the device,

@@ -40,6 +40,10 @@ struct tpc_tracker {
   cudaEvent_t ev[6];
   int64_t last_n;
   int64_t last_max_tracks;        // out->max_tracks of the last track call: n_tracks <= it (S5 raises TRACKS_OVERFLOW otherwise)
+  // call order of the optional calls: frame_seq counts the track calls; the others remember the frame they ran on
+  // (0 = never).  refit -> merge -> apex -> removable each need their predecessors to have run on the CURRENT frame,
+  // because they read what those left in the workspace (fit_row, up_*, MergeCounters).
+  uint64_t frame_seq, refit_seq, merge_seq, apex_seq;
 };
 
 namespace {
@@ -203,6 +207,7 @@ int run_device(tpc_tracker* t, const tpc_clusters_t* in, const OutPtrs& o, cudaS
   t->last_stream = st;
   t->last_n = in->n;
   t->last_max_tracks = o.max_tracks;
+  ++t->frame_seq;
   const bool tm = t->timing;
   if (tm) cudaEventRecord(t->ev[0], st);
   if (launch_reset(c, st)) return TPC_ERR_CUDA;
@@ -305,7 +310,7 @@ int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t
   c.n_sms = sms;
   if (init_s1()) { delete t; return TPC_ERR_CUDA; }
   if (cudaMemcpy(const_cast<RowTab*>(c.rowtab), tab.data(), tab.size() * sizeof(RowTab), cudaMemcpyHostToDevice) != cudaSuccess ||
-      cudaMemset(c.cnt, 0, sizeof(Counters)) != cudaSuccess) {
+      cudaMemset(c.cnt, 0, sizeof(Counters)) != cudaSuccess || cudaMemset(c.mcnt, 0, sizeof(MergeCounters)) != cudaSuccess) {
     delete t; return TPC_ERR_CUDA;
   }
   // from here on a failure goes through tpc_tracker_destroy, which releases whatever was created so far
@@ -334,6 +339,11 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tr
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const OutPtrs o = to_out(out);
   if (!t->use_graph || t->timing || st == nullptr) return run_device(t, in, o, st);   // (the legacy default stream cannot capture)
+  // a stream the caller is already capturing (the framework around the tracker records its own graph): a second
+  // BeginCapture would fail and could invalidate that capture - enqueue the plain launches into the caller's graph instead
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cudaGetLastError(); return TPC_ERR_CUDA; }
+  if (cap != cudaStreamCaptureStatusNone) return run_device(t, in, o, st);
   const bool same = t->graph_exec && t->graph_in.n == in->n && t->graph_in.sector == in->sector && t->graph_in.row == in->row &&
                     t->graph_in.y == in->y && t->graph_in.z == in->z && std::memcmp(&t->graph_out, &o, sizeof(OutPtrs)) == 0;
   if (!same) {
@@ -349,6 +359,7 @@ int tpc_track_timeframe(tpc_tracker_t* t, const tpc_clusters_t* in, const tpc_tr
     t->graph_in = *in; t->graph_out = o;
   }
   t->last_stream = st; t->last_n = in->n; t->last_max_tracks = o.max_tracks;
+  ++t->frame_seq;
   t->ctx.n = (int)in->n;
   t->ctx.in_sector = in->sector; t->ctx.in_row = in->row; t->ctx.in_y = in->y; t->ctx.in_z = in->z;
   return cudaGraphLaunch(t->graph_exec, st) == cudaSuccess ? TPC_OK : TPC_ERR_CUDA;
@@ -468,9 +479,12 @@ int tpc_tracker_refit(tpc_tracker_t* t, const tpc_fit_t* out, void* cuda_stream)
   const int nres = (out->trk_cl_start != nullptr) + (out->res_y != nullptr) + (out->res_z != nullptr);
   if (nres != 0 && nres != 3) return TPC_ERR_INVALID_ARG;
   o.trk_cl_start = out->trk_cl_start; o.res_y = out->res_y; o.res_z = out->res_z;
+  if (!t->frame_seq) return TPC_ERR_INVALID_ARG;      // no frame tracked yet
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   t->last_stream = st;
-  return launch_refit(t->ctx, o, st) ? TPC_ERR_CUDA : TPC_OK;
+  if (launch_refit(t->ctx, o, st)) return TPC_ERR_CUDA;
+  t->refit_seq = t->frame_seq;
+  return TPC_OK;
 }
 
 int tpc_tracker_merge(tpc_tracker_t* t, const tpc_fit_t* fit, const tpc_merge_cuts_t* cuts, const tpc_merged_t* out,
@@ -500,9 +514,12 @@ int tpc_tracker_merge(tpc_tracker_t* t, const tpc_fit_t* fit, const tpc_merge_cu
   o.n_merged = out->n_merged; o.merged_of_track = out->merged_of_track; o.seg_start = out->seg_start; o.seg_idx = out->seg_idx;
   o.par = out->par; o.cov = out->cov; o.x_ref = out->x_ref; o.z_ref = out->z_ref; o.chi2 = out->chi2; o.ndf = out->ndf;
   o.n_fit = out->n_fit; o.sector = out->sector; o.n_clusters = out->n_clusters; o.max_tracks = (int)out->max_tracks;
+  if (!t->frame_seq || t->refit_seq != t->frame_seq) return TPC_ERR_INVALID_ARG;   // needs the refit of THIS frame
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   t->last_stream = st;
-  return launch_merge(t->ctx, f, o, st) ? TPC_ERR_CUDA : TPC_OK;
+  if (launch_merge(t->ctx, f, o, st)) return TPC_ERR_CUDA;
+  t->merge_seq = t->frame_seq;
+  return TPC_OK;
 }
 
 int tpc_tracker_apex(tpc_tracker_t* t, const tpc_merged_t* merged, const tpc_apex_cuts_t* cuts, const tpc_apex_t* out,
@@ -525,9 +542,12 @@ int tpc_tracker_apex(tpc_tracker_t* t, const tpc_merged_t* merged, const tpc_ape
   o.max_k = cuts->max_k; o.min_s = cuts->min_s; o.dz_win = cuts->dz_win; o.tol_c = cuts->tol_c; o.tol_z = cuts->tol_z;
   o.tol_t = cuts->tol_t; o.cut = cuts->cut;
   o.apex_partner = out->apex_partner; o.apex_leg = out->apex_leg; o.max_tracks = (int)out->max_tracks;
+  if (!t->frame_seq || t->merge_seq != t->frame_seq) return TPC_ERR_INVALID_ARG;   // needs the merge of THIS frame
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   t->last_stream = st;
-  return launch_apex(t->ctx, m, o, st) ? TPC_ERR_CUDA : TPC_OK;
+  if (launch_apex(t->ctx, m, o, st)) return TPC_ERR_CUDA;
+  t->apex_seq = t->frame_seq;
+  return TPC_OK;
 }
 
 int tpc_tracker_removable(tpc_tracker_t* t, const int32_t* cluster_track, const tpc_fit_t* fit, const tpc_merged_t* merged,
@@ -545,6 +565,7 @@ int tpc_tracker_removable(tpc_tracker_t* t, const int32_t* cluster_track, const 
   o.cluster_track = cluster_track; o.merged_of_track = merged->merged_of_track; o.apex_leg = apex->apex_leg;
   o.mrg_par = merged->par; o.mrg_stride = (int)merged->max_tracks; o.fit_par = fit->par; o.fit_stride = (int)fit->max_tracks;
   o.cls = cls; o.remove = remove;
+  if (!t->frame_seq || t->merge_seq != t->frame_seq || t->apex_seq != t->frame_seq) return TPC_ERR_INVALID_ARG;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   t->last_stream = st;
   return launch_removable(t->ctx, o, st) ? TPC_ERR_CUDA : TPC_OK;

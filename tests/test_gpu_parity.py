@@ -197,6 +197,36 @@ def test_cuda_graph_path_gives_the_same_result_and_recaptures_on_new_arguments(m
     assert np.array_equal(trk.stage_view("perm"), run_oracle(tf, P, last_stage=1).get("perm"))
 
 
+def test_graph_mode_inside_a_capture_of_the_callers_own(mini_event):
+    """A framework that records its own CUDA graph around the tracker: with graph mode on, tpc_track_timeframe must not
+    begin a second capture on that stream (it would fail and break the caller's) - its launches go into the caller's
+    graph, and replaying that graph gives the result of the direct launches."""
+    tf = mini_event
+    P, trk, out = run_gpu(tf)
+    ref = out.numpy()
+    trk.enable_graph(True)
+    ins = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (tf.sector, tf.row, tf.y, tf.z)]
+    o1 = trk.new_tracks(tf.n)
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        trk.track_timeframe(*ins, o1, stream=torch.cuda.current_stream())
+    o1.n_tracks.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    a = o1.numpy()
+    assert a["n_tracks"] == ref["n_tracks"] > 0
+    for k in ref:
+        if isinstance(ref[k], np.ndarray):
+            assert np.array_equal(ref[k], a[k]), k
+    # and the handle's own graph path still works afterwards on an ordinary stream
+    with torch.cuda.stream(s):
+        trk.track_timeframe(*ins, o1, stream=s); trk.track_timeframe(*ins, o1, stream=s)
+        s.synchronize()
+    assert np.array_equal(o1.numpy()["cluster_track"], ref["cluster_track"])
+
+
 def test_repeatable_and_reusable(mini_event):
     """Two calls on one handle give identical results (ids come from scans, not from atomics)."""
     import paper_2009_07515_b200 as tpc
