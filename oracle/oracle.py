@@ -25,10 +25,11 @@ class _Params(C.Structure):
         ("pick_chi2_cut", C.c_float), ("max_sinphi", C.c_float), ("y_margin", C.c_float),
         ("init_c_ss", C.c_float), ("init_c_tt", C.c_float), ("init_c_qq", C.c_float),
         ("z_is_time", C.c_int32), ("cm_per_time_unit", C.c_float), ("drift_length", C.c_float),
+        ("y_is_pad", C.c_int32), ("n_pads", C.c_int32 * _MAX_ROWS), ("pad_pitch", C.c_float * _MAX_ROWS),
     ]
 
 
-_DEFAULTS = {"z_is_time": 0, "cm_per_time_unit": 0.0, "drift_length": 0.0}
+_DEFAULTS = {"z_is_time": 0, "cm_per_time_unit": 0.0, "drift_length": 0.0, "y_is_pad": 0}
 
 
 _KINDS = {0: np.int32, 1: np.float32, 2: np.float64, 3: np.uint64, 4: np.int64}
@@ -88,6 +89,12 @@ def _pack(params: dict) -> _Params:
         if name == "row_x":
             for i, v in enumerate(rx):
                 p.row_x[i] = float(v)
+        elif name in ("n_pads", "pad_pitch"):              # per-row tables of the native pad input (only with y_is_pad)
+            if params.get("y_is_pad", 0):
+                tab = np.asarray(params[name])
+                assert tab.shape[0] == params["n_rows"]
+                for i, v in enumerate(tab):
+                    getattr(p, name)[i] = v.item()
         else:
             v = params[name] if name in params else _DEFAULTS[name]
             setattr(p, name, v.item() if hasattr(v, "item") else v)

@@ -55,6 +55,9 @@ struct Params {             // mirrors the ctypes Structure in oracle/oracle.py 
   int32_t min_chain_len, max_gap, min_tracklet_hits, min_track_hits;
   float pick_chi2_cut, max_sinphi, y_margin, init_c_ss, init_c_tt, init_c_qq;
   int32_t z_is_time; float cm_per_time_unit, drift_length;   // native time input, DESIGN.md section 3.0a
+  int32_t y_is_pad;                                          // native pad input, DESIGN.md section 3.0b
+  int32_t n_pads[kMaxRows];                                  //   pads of row r
+  float pad_pitch[kMaxRows];                                 //   pad width of row r, cm
 };
 
 // floor(v) clamped to [0, hi]; defined for every v (NaN and negatives -> 0), DESIGN.md section 3.1 (3)
@@ -262,6 +265,7 @@ struct Oracle {
   const uint8_t* in_sector = nullptr; const uint8_t* in_row = nullptr;
   const float* in_y = nullptr; const float* in_z = nullptr;
   std::vector<float> z_from_time;      // pseudo-z computed from the native time, when z_is_time
+  std::vector<float> y_from_pad;       // sector-local y computed from the native pad coordinate (section 3.0b), when y_is_pad
 
   // S1
   std::vector<float> zmin, zmax; std::vector<int32_t> nz;         // per sector
@@ -1045,6 +1049,22 @@ struct Oracle {
         z_from_time[i] = (int)sec[i] < P.n_sectors / 2 ? zc : 0.0f - zc;
       }
       in_z = z_from_time.data();
+    }
+    if (P.y_is_pad) {
+      // DESIGN.md section 3.0b (hits arrive in "native pad, row, and time coordinates"): the input holds
+      // the pad coordinate p of the cluster (centre of pad 0 = 0, centre of the last pad = n_pads_r - 1, fractional for a
+      // centroid).  The pads of a row lie symmetric about the sector axis, so y = (p - (n_pads_r - 1) / 2) * pitch_r.
+      // fp32: the half pad count is exact, the difference and the product are rounded separately.  A row out of
+      // range is rejected by stage 1 below; its y is left as given.
+      y_from_pad.resize(n);
+      for (int64_t i = 0; i < n; ++i) {
+        const int r = row[i];
+        if (r >= P.n_rows) { y_from_pad[i] = y[i]; continue; }
+        const float centre = 0.5f * (float)(P.n_pads[r] - 1);
+        const float d = y[i] - centre;
+        y_from_pad[i] = d * P.pad_pitch[r];
+      }
+      in_y = y_from_pad.data();
     }
     stage_seconds.assign(5, 0.0);
     auto now = [] { return std::chrono::steady_clock::now(); };

@@ -17,5 +17,6 @@ from .generator import (  # noqa: F401
     choose_cell,
     default_params,
     select_sectors,
+    to_native_pad,
     to_native_time,
 )

@@ -369,6 +369,22 @@ def to_native_time(tf: TimeFrame, time_unit_us: float = 0.2) -> tuple[TimeFrame,
                      drift_length=np.float32(g.drift_length))
 
 
+def to_native_pad(tf: TimeFrame, pitch_inner: float = 0.4375, pitch_outer: float = 0.625, n_inner: int = 63) -> tuple[TimeFrame, dict]:
+    """The same time frame with the NATIVE pad coordinate in place of the sector-local y: row r has
+    n_pads_r pads of width pitch_r (narrow pads on the first `n_inner` rows, wide ones outside - the ALICE read-out chambers
+    have 4-6 mm pads), symmetric about the sector axis and enough of them to cover +-ymax_r; a cluster at y has the
+    pad coordinate p = y / pitch_r + (n_pads_r - 1) / 2 (pad centres at the integers), evaluated in double from the
+    frame's own y, cast to fp32 last.  Returns (frame whose `y` holds p, the three tpc_params_t entries that describe it)."""
+    g = tf.geometry
+    rx = g.row_x()
+    pitch = np.where(np.arange(g.n_rows) < n_inner, float(pitch_inner), float(pitch_outer))
+    n_pads = (2 * np.ceil(rx * g.tan_half_sector / pitch)).astype(np.int32)
+    p = tf.y.astype(np.float64) / pitch[tf.row] + 0.5 * (n_pads[tf.row] - 1)
+    out = TimeFrame(sector=tf.sector, row=tf.row, x=tf.x, y=p.astype(np.float32), z=tf.z, track_id=tf.track_id,
+                    truth=tf.truth, geometry=g, tf_length_us=tf.tf_length_us, sigma=tf.sigma, name=tf.name + "+pad", leg=tf.leg)
+    return out, dict(y_is_pad=1, n_pads=n_pads, pad_pitch=pitch.astype(np.float32))
+
+
 def select_sectors(tf: TimeFrame, sectors) -> tuple[TimeFrame, np.ndarray]:
     """Sub-frame holding only the clusters of ``sectors`` (order kept) + their input indices."""
     keep = np.isin(tf.sector, np.asarray(list(sectors), dtype=np.uint8))
