@@ -62,6 +62,10 @@ def _load():
         lib.orc_kf_fit.restype = C.c_int
         lib.orc_kf_fit.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                    C.c_void_p, C.c_void_p]
+        lib.orc_quantise_residuals.restype = None
+        lib.orc_quantise_residuals.argtypes = [C.c_void_p, C.c_float, C.c_float]
+        lib.orc_quantise_values.restype = None
+        lib.orc_quantise_values.argtypes = [C.c_void_p, C.c_int64, C.c_float, C.c_void_p]
         lib.orc_protect.restype = None
         lib.orc_protect.argtypes = [C.c_void_p, C.c_float, C.c_float]
         lib.orc_merge.restype = None
@@ -126,6 +130,19 @@ class Oracle:
         if rc != 0:
             raise ValueError(f"oracle rejected the input (rc={rc})")
         return self
+
+    def quantise_residuals(self, step_y: float, step_z: float) -> "Oracle":
+        """DESIGN.md section 3.7a on the residuals of the last run (last_stage = 6): fit_qres_y / fit_qres_z."""
+        self._lib.orc_quantise_residuals(self._h, float(step_y), float(step_z))
+        return self
+
+    @staticmethod
+    def quantise_values(res, step: float) -> np.ndarray:
+        """The scalar rule of section 3.7a applied to given residuals (test entry)."""
+        res = np.ascontiguousarray(res, dtype=np.float32)
+        out = np.empty(res.shape[0], np.int32)
+        _load().orc_quantise_values(res.ctypes.data, res.shape[0], float(step), out.ctypes.data)
+        return out
 
     def protect(self, road_y: float, road_z: float) -> np.ndarray:
         """DESIGN.md section 3.8 on the tracks of the last run: keep flag per INPUT cluster."""

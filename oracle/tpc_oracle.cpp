@@ -60,6 +60,18 @@ struct Params {             // mirrors the ctypes Structure in oracle/oracle.py 
   float pad_pitch[kMaxRows];                                 //   pad width of row r, cm
 };
 
+// DESIGN.md section 3.7a ("tailored custom fixed ... point data formats using only exactly as many bits as
+// needed", "stored as residuals to the extrapolated track position"): a residual as a signed 16-bit count
+// of steps.  fp32: one product with the reciprocal step, round to nearest with ties to even, saturation at +-32767
+// (-32768 is never produced; a NaN - no residual is one - counts as below the range).
+inline int32_t quantise_residual(float res, float inv_step) {
+  const float v = res * inv_step;
+  const float r = std::nearbyint(v);                    // default rounding mode: to nearest, ties to even
+  if (!(r > -32767.0f)) return -32767;
+  if (r >= 32767.0f) return 32767;
+  return (int32_t)r;
+}
+
 // floor(v) clamped to [0, hi]; defined for every v (NaN and negatives -> 0), DESIGN.md section 3.1 (3)
 inline int floor_clamp(float v, int hi) {
   const float f = std::floor(v);
@@ -296,6 +308,7 @@ struct Oracle {
   std::vector<double> fit_par, fit_cov, fit_x_ref, fit_z_ref, fit_chi2;
   std::vector<int32_t> fit_ndf, fit_n;
   std::vector<double> fit_res_y, fit_res_z;                        // parallel to trk_cl_idx: residual to the extrapolated track
+  std::vector<int32_t> fit_qres_y, fit_qres_z;                     // the same as counts of steps
   // S8 cluster protection, "strategy B"
   std::vector<int32_t> keep;                                       // [n] by INPUT index: 1 protected, 0 removable
   // S9 track merger
@@ -692,6 +705,17 @@ struct Oracle {
     }
   }
 
+
+  // the residuals of the last stage6 as 16-bit counts of `step_y` / `step_z` (cm).  The residual is
+  // the fp32 one (in the double instance: the double residual cast to fp32 first); inv_step = 1 / step, one fp32 division.
+  void quantise_residuals(float step_y, float step_z) {
+    const float iy = 1.0f / step_y, iz = 1.0f / step_z;
+    fit_qres_y.resize(fit_res_y.size()); fit_qres_z.resize(fit_res_z.size());
+    for (size_t i = 0; i < fit_res_y.size(); ++i) {
+      fit_qres_y[i] = quantise_residual((float)fit_res_y[i], iy);
+      fit_qres_z[i] = quantise_residual((float)fit_res_z[i], iz);
+    }
+  }
 
   // ---------------------------------------------------------------------------------------- S9
   // Track merger ("Track Fit" of PAPER.md:99, 131, 138: the segments a track was found in - one per
@@ -1177,6 +1201,7 @@ int orc_get(void* h, const char* name, const void** ptr, int64_t* n, int* kind) 
   I32(trk_seed); I32(trk_sector); I32(trk_first_row); I32(trk_last_row); I32(trk_n_clusters); I32(trk_ndf);
   F64(trk_par); F64(trk_cov); F64(trk_x_ref); F64(trk_z_ref); F64(trk_chi2); F64(trk_z_beam);
   I32(trk_cl_start); I32(trk_cl_idx); I32(trk_cl_pos); I32(cluster_track); F64(stage_seconds);
+  I32(fit_qres_y); I32(fit_qres_z);
   I32(keep); F64(fit_res_y); F64(fit_res_z); F64(fit_par); F64(fit_cov); F64(fit_x_ref); F64(fit_z_ref); F64(fit_chi2); I32(fit_ndf); I32(fit_n);
   I32(fit_row); F64(up_par); F64(up_cov); F64(up_x_ref); F64(up_z_ref); F64(up_chi2); I32(up_row); I32(up_n);
   I32(mrg_best_b); I32(mrg_best_a); I32(mrg_next); I32(mrg_prev); I32(mrg_dir); F64(mrg_chi2_b);
@@ -1220,6 +1245,13 @@ int orc_kf_fit(const void* params, int prec, int npt, const double* x, const dou
 }
 
 // S8 on the tracks of the last orc_run (last_stage >= 5)
+void orc_quantise_residuals(void* h, float step_y, float step_z) { reinterpret_cast<Oracle*>(h)->quantise_residuals(step_y, step_z); }
+// test entry: the scalar rule on caller-given values
+void orc_quantise_values(const float* res, int64_t n, float step, int32_t* out) {
+  const float inv = 1.0f / step;
+  for (int64_t i = 0; i < n; ++i) out[i] = quantise_residual(res[i], inv);
+}
+
 void orc_protect(void* h, float road_y, float road_z) { reinterpret_cast<Oracle*>(h)->stage7_protect(road_y, road_z); }
 
 // S9 on the tracks and the refit of the last orc_run (last_stage >= 6)
