@@ -99,6 +99,15 @@ typedef struct {
   int32_t z_is_time;
   float cm_per_time_unit;
   float drift_length;       /* cm, full drift length of one side (250) */
+  /* Native pad input (same passage of the paper).  y_is_pad = 0: tpc_clusters_t.y is the
+   * sector-local y in cm and the two tables below are ignored (may be NULL).  y_is_pad != 0: tpc_clusters_t.y holds the PAD
+   * coordinate p of the cluster in its row (pad centres at 0 .. n_pads[row] - 1, fractional for a centroid) and S1 computes
+   * y itself, in fp32, while it reads the input (no extra pass): y = (p - 0.5 * (n_pads[row] - 1)) * pad_pitch[row], the
+   * difference and the product rounded separately (pads symmetric about the sector axis, y growing with the pad number).
+   * Together with z_is_time this is the detector's (pad, row, time) input. */
+  int32_t y_is_pad;
+  const int32_t* n_pads;    /* HOST, n_rows values >= 1: pads of each row (copied at create) */
+  const float* pad_pitch;   /* HOST, n_rows values > 0, finite: pad width of each row, cm (copied at create) */
 } tpc_params_t;
 
 /* Input clusters of one time frame, SoA.  DEVICE pointers for tpc_track_timeframe, HOST pointers
@@ -114,7 +123,7 @@ typedef struct {
   const uint8_t* sector; /* [n] */
   const uint8_t* row;    /* [n] */
   const float* x;        /* [n] or NULL (unused) */
-  const float* y;        /* [n] sector-local y, cm */
+  const float* y;        /* [n] sector-local y, cm (y_is_pad = 0) or pad coordinate (y_is_pad != 0) */
   const float* z;        /* [n] pseudo-z, cm (z_is_time = 0) or time, time units (z_is_time != 0) */
 } tpc_clusters_t;
 
@@ -280,6 +289,12 @@ typedef struct {
   const int32_t* trk_cl_start; /* [n_tracks+1] the call's tpc_tracks_t.trk_cl_start (DEVICE) */
   float* res_y;      /* [max_track_clusters of the call] cm */
   float* res_z;      /* [max_track_clusters of the call] cm */
+  /* optional (both NULL to skip; need the three fields above): the same residuals as signed 16-bit counts of steps
+   * (DESIGN.md section 3.7a): q = rint(res * (1 / step)) in fp32, ties to even, saturated at +-32767;
+   * decoding q * step is within step / 2 of the residual.  res_step_y / res_step_z: cm, finite, > 0 (0.01 = 0.1 mm). */
+  int16_t* qres_y;   /* [max_track_clusters of the call] */
+  int16_t* qres_z;   /* [max_track_clusters of the call] */
+  float res_step_y, res_step_z;
 } tpc_fit_t;
 
 /* Refit of every track of the LAST tpc_track_timeframe call on this handle over the clusters it owns after the

@@ -29,10 +29,12 @@ class tpc_params_t(C.Structure):
         ("pick_chi2_cut", C.c_float), ("max_sinphi", C.c_float), ("y_margin", C.c_float),
         ("init_c_ss", C.c_float), ("init_c_tt", C.c_float), ("init_c_qq", C.c_float),
         ("z_is_time", C.c_int32), ("cm_per_time_unit", C.c_float), ("drift_length", C.c_float),
+        ("y_is_pad", C.c_int32), ("n_pads", C.c_void_p), ("pad_pitch", C.c_void_p),
     ]
 
 
-_PARAM_DEFAULTS = {"z_is_time": 0, "cm_per_time_unit": 0.0, "drift_length": 0.0}   # pseudo-z input unless asked otherwise
+# pseudo-z and y in cm unless asked otherwise
+_PARAM_DEFAULTS = {"z_is_time": 0, "cm_per_time_unit": 0.0, "drift_length": 0.0, "y_is_pad": 0}
 
 
 class tpc_clusters_t(C.Structure):
@@ -50,7 +52,8 @@ class tpc_tracks_t(C.Structure):
 
 class tpc_fit_t(C.Structure):
     _fields_ = [("max_tracks", C.c_int64)] + [(f, C.c_void_p) for f in ("par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit",
-                                                                       "trk_cl_start", "res_y", "res_z")]
+                                                                       "trk_cl_start", "res_y", "res_z", "qres_y", "qres_z")] + \
+               [("res_step_y", C.c_float), ("res_step_z", C.c_float)]
 
 
 class tpc_merge_cuts_t(C.Structure):
@@ -188,16 +191,23 @@ def _check(lib, rc: int, what: str):
 
 
 def pack_params(params: dict):
-    """dict (tpc_synth.default_params) -> (tpc_params_t, keep-alive row_x array)."""
+    """dict (tpc_synth.default_params) -> (tpc_params_t, keep-alive host tables: row_x and, with y_is_pad, the pad plane)."""
     rx = np.ascontiguousarray(params["row_x"], dtype=np.float32)
+    keep = [rx]
     p = tpc_params_t()
     for name, _ in tpc_params_t._fields_:
         if name == "row_x":
             p.row_x = rx.ctypes.data
+        elif name in ("n_pads", "pad_pitch"):
+            if params.get("y_is_pad", 0):
+                tab = np.ascontiguousarray(params[name], dtype=np.int32 if name == "n_pads" else np.float32)
+                assert tab.shape[0] == params["n_rows"]
+                keep.append(tab)
+                setattr(p, name, tab.ctypes.data)
         else:
             v = params[name] if name in params else _PARAM_DEFAULTS[name]
             setattr(p, name, v.item() if hasattr(v, "item") else v)
-    return p, rx
+    return p, keep
 
 
 class Tracks:
@@ -342,14 +352,19 @@ class Tracker:
         s = out.struct()
         _check(self.lib, self.lib.tpc_track_timeframe_host_end(self._h, C.byref(s), int(slot)), "tpc_track_timeframe_host_end")
 
-    def new_fit(self, residuals: bool = False) -> dict:
-        """Device buffers for tpc_tracker_refit (layouts as in tpc_fit_t); with `residuals` also res_y / res_z."""
+    def new_fit(self, residuals: bool = False, steps: "tuple[float, float] | None" = None) -> dict:
+        """Device buffers for tpc_tracker_refit (layouts as in tpc_fit_t); with `residuals` also res_y / res_z; with
+        `steps` = (step_y, step_z) in cm also the 16-bit residual codes qres_y / qres_z (implies the residuals)."""
         mt, dev = self.caps[3], self.device
         f32 = lambda *s: torch.empty(*s, dtype=torch.float32, device=dev)   # noqa: E731
         i32 = lambda *s: torch.empty(*s, dtype=torch.int32, device=dev)     # noqa: E731
         d = dict(par=f32(5, mt), cov=f32(15, mt), x_ref=f32(mt), z_ref=f32(mt), chi2=f32(mt), ndf=i32(mt), n_fit=i32(mt))
-        if residuals:
+        if residuals or steps is not None:
             d.update(res_y=f32(self.caps[4]), res_z=f32(self.caps[4]))
+        if steps is not None:
+            d.update(qres_y=torch.empty(self.caps[4], dtype=torch.int16, device=dev),
+                     qres_z=torch.empty(self.caps[4], dtype=torch.int16, device=dev),
+                     res_step_y=float(steps[0]), res_step_z=float(steps[1]))
         return d
 
     def refit_into(self, fit: dict, stream=None, out: "Tracks | None" = None):
@@ -359,22 +374,25 @@ class Tracker:
         f = tpc_fit_t()
         f.max_tracks = self.caps[3]
         for k, v in fit.items():
-            setattr(f, k, v.data_ptr())
+            setattr(f, k, v.data_ptr() if torch.is_tensor(v) else v)
         if "res_y" in fit:
             f.trk_cl_start = out.trk_cl_start.data_ptr()
         _check(self.lib, self.lib.tpc_tracker_refit(self._h, C.byref(f), C.c_void_p(st.cuda_stream)), "tpc_tracker_refit")
 
-    def refit(self, n_tracks: int, stream=None, tracks: "Tracks | None" = None) -> dict:
-        """Convenience: refit + host copies trimmed to n_tracks (with `tracks`, the call's outputs, also the residuals)."""
-        buf = self.new_fit(residuals=tracks is not None)
+    def refit(self, n_tracks: int, stream=None, tracks: "Tracks | None" = None, steps=None) -> dict:
+        """Convenience: refit + host copies trimmed to n_tracks (with `tracks`, the call's outputs, also the residuals;
+        with `steps` = (step_y, step_z) also their 16-bit codes)."""
+        buf = self.new_fit(residuals=tracks is not None, steps=steps if tracks is not None else None)
         self.refit_into(buf, stream, out=tracks)
         torch.cuda.synchronize(self.device)
         T = int(n_tracks)
-        out = {k: v.cpu().numpy() for k, v in buf.items()}
+        out = {k: v.cpu().numpy() for k, v in buf.items() if torch.is_tensor(v)}
         extra = {}
         if tracks is not None:
             ntc = int(tracks.trk_cl_start[T].item()) if T else 0
             extra = dict(res_y=out["res_y"][:ntc].copy(), res_z=out["res_z"][:ntc].copy())
+            if steps is not None:
+                extra.update(qres_y=out["qres_y"][:ntc].copy(), qres_z=out["qres_z"][:ntc].copy())
         return dict(**extra, par=out["par"][:, :T].T.copy(), cov=out["cov"][:, :T].T.copy(), x_ref=out["x_ref"][:T].copy(),
                     z_ref=out["z_ref"][:T].copy(), chi2=out["chi2"][:T].copy(), ndf=out["ndf"][:T].copy(),
                     n_fit=out["n_fit"][:T].copy())
@@ -428,9 +446,18 @@ class Tracker:
                   fill: int = 0):
         """Convenience: refit + merge + apex + tpc_tracker_removable for the last track_timeframe call (outputs `out`);
         returns (cls, remove) as uint8 device tensors [n].  `fill`: see new_merged."""
-        st = torch.cuda.current_stream(self.device)
         fit = self.new_fit(); mg = self.new_merged(fill); ax = self.new_apex()
         self.refit_into(fit); self.merge_into(fit, mg, merge_cuts); self.apex_into(mg, ax, apex_cuts)
+        n = max(1, out.n_in)
+        cls = torch.zeros(n, dtype=torch.uint8, device=self.device); rem = torch.zeros(n, dtype=torch.uint8, device=self.device)
+        self.removable_into(out, fit, mg, ax, cls, rem, cuts)
+        torch.cuda.synchronize(self.device)
+        return cls[: out.n_in], rem[: out.n_in]
+
+    def removable_into(self, out: "Tracks", fit: dict, mg: dict, ax: dict, cls, rem, cuts: dict | None = None, stream=None):
+        """Enqueues tpc_tracker_removable alone (does not synchronise, allocates nothing): `fit`, `mg`, `ax` are the buffers
+        the refit_into / merge_into / apex_into calls of this frame wrote; cls / rem uint8 device tensors [n]."""
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
         f = tpc_fit_t(); f.max_tracks = self.caps[3]
         for k in ("par", "cov", "x_ref", "z_ref", "chi2", "ndf", "n_fit"):
             setattr(f, k, fit[k].data_ptr())
@@ -441,13 +468,9 @@ class Tracker:
         a.apex_partner = ax["apex_partner"].data_ptr(); a.apex_leg = ax["apex_leg"].data_ptr()
         kw = dict(REMOVAL_CUTS); kw.update(cuts or {})
         c = tpc_removal_cuts_t(float(kw["min_pt"]), float(kw["max_incl"]), float(kw["road_y"]), float(kw["road_z"]))
-        n = max(1, out.n_in)
-        cls = torch.zeros(n, dtype=torch.uint8, device=self.device); rem = torch.zeros(n, dtype=torch.uint8, device=self.device)
         _check(self.lib, self.lib.tpc_tracker_removable(self._h, out.cluster_track.data_ptr(), C.byref(f), C.byref(m), C.byref(a),
                                                          C.byref(c), cls.data_ptr(), rem.data_ptr(), C.c_void_p(st.cuda_stream)),
                "tpc_tracker_removable")
-        torch.cuda.synchronize(self.device)
-        return cls[: out.n_in], rem[: out.n_in]
 
     def new_apex(self) -> dict:
         mt, dev = self.caps[3], self.device

@@ -69,6 +69,11 @@ bool params_ok(const tpc_params_t* p) {
   if (p->min_chain_len < 2 || p->max_gap < 0) return false;
   if (p->z_is_time && (!(p->cm_per_time_unit > 0.f) || !(p->cm_per_time_unit < INFINITY) || !(std::fabs(p->drift_length) < INFINITY)))
     return false;
+  if (p->y_is_pad) {
+    if (!p->n_pads || !p->pad_pitch) return false;
+    for (int r = 0; r < p->n_rows; ++r)
+      if (p->n_pads[r] < 1 || !(p->pad_pitch[r] > 0.f) || !(p->pad_pitch[r] < INFINITY)) return false;
+  }
   for (int r = 0; r < p->n_rows; ++r) {
     if (!(p->row_x[r] > 0.f)) return false;
     if (r && !(p->row_x[r] > p->row_x[r - 1])) return false;
@@ -83,6 +88,7 @@ void layout(tpc_tracker* t, char* base, size_t* total) {
   const int S = t->params.n_sectors, R = t->params.n_rows, SR = S * R;
   c.cnt = cv.take<Counters>(1);
   c.rowtab = cv.take<RowTab>(R);
+  c.padtab = cv.take<float2>(R);
   c.zmin_key = cv.take<int>(S); c.zmax_key = cv.take<int>(S);
   c.zmin = cv.take<float>(S); c.zmax = cv.take<float>(S); c.nz = cv.take<int>(S);
   c.bin_base = cv.take<int>(SR + 1); c.row_start = cv.take<int>(SR + 1);
@@ -299,7 +305,12 @@ int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t
   if (total > workspace_bytes) { delete t; return TPC_ERR_CAPACITY; }   // nothing but the host struct exists yet
   std::vector<RowTab> tab;
   fill_ctx_constants(t, tab);
-  t->params.row_x = nullptr;
+  // native pad input: per row the half pad count (exact in fp32) and the pitch
+  std::vector<float2> padtab((size_t)params->n_rows, make_float2(0.f, 1.f));
+  t->ctx.y_is_pad = params->y_is_pad != 0;
+  if (params->y_is_pad)
+    for (int r = 0; r < params->n_rows; ++r) padtab[r] = make_float2(0.5f * (float)(params->n_pads[r] - 1), params->pad_pitch[r]);
+  t->params.row_x = nullptr; t->params.n_pads = nullptr; t->params.pad_pitch = nullptr;   // the caller's tables are not kept
   Ctx& c = t->ctx;
   c.max_clusters = (int)max_clusters; c.max_bins = (int)max_bins; c.max_seeds = (int)max_seeds;
   c.max_tracks = (int)max_tracks; c.max_track_clusters = (int)max_track_clusters;
@@ -310,6 +321,7 @@ int tpc_tracker_create(const tpc_params_t* params, int64_t max_clusters, int64_t
   c.n_sms = sms;
   if (init_s1()) { delete t; return TPC_ERR_CUDA; }
   if (cudaMemcpy(const_cast<RowTab*>(c.rowtab), tab.data(), tab.size() * sizeof(RowTab), cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(const_cast<float2*>(c.padtab), padtab.data(), padtab.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemset(c.cnt, 0, sizeof(Counters)) != cudaSuccess || cudaMemset(c.mcnt, 0, sizeof(MergeCounters)) != cudaSuccess) {
     delete t; return TPC_ERR_CUDA;
   }
@@ -479,6 +491,16 @@ int tpc_tracker_refit(tpc_tracker_t* t, const tpc_fit_t* out, void* cuda_stream)
   const int nres = (out->trk_cl_start != nullptr) + (out->res_y != nullptr) + (out->res_z != nullptr);
   if (nres != 0 && nres != 3) return TPC_ERR_INVALID_ARG;
   o.trk_cl_start = out->trk_cl_start; o.res_y = out->res_y; o.res_z = out->res_z;
+  // residual codes: both or none, only next to the residuals, steps finite and > 0
+  const int nq = (out->qres_y != nullptr) + (out->qres_z != nullptr);
+  if (nq == 1 || (nq == 2 && nres != 3)) return TPC_ERR_INVALID_ARG;
+  o.qres_y = nullptr; o.qres_z = nullptr; o.inv_step_y = 0.f; o.inv_step_z = 0.f;
+  if (nq == 2) {
+    if (!(out->res_step_y > 0.f) || !(out->res_step_y < INFINITY) || !(out->res_step_z > 0.f) || !(out->res_step_z < INFINITY))
+      return TPC_ERR_INVALID_ARG;
+    o.qres_y = out->qres_y; o.qres_z = out->qres_z;
+    o.inv_step_y = 1.0f / out->res_step_y; o.inv_step_z = 1.0f / out->res_step_z;   // one fp32 division each
+  }
   if (!t->frame_seq) return TPC_ERR_INVALID_ARG;      // no frame tracked yet
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   t->last_stream = st;

@@ -183,8 +183,9 @@ __global__ void __launch_bounds__(kThreads) k_partition(Ctx c) {
   if (c.cnt->status) return;
   const long long n = c.n;
   bool bad = false;
-  auto one = [&](int s, int r, float y, float zin, long long i) {
+  auto one = [&](int s, int r, float yin, float zin, long long i) {
     const float z = input_z(c, s, zin);
+    const float y = input_y(c, r, yin);                 // cm as given, or converted from the pad coordinate (section 3.0b)
     if (!(fabsf(y) < INFINITY)) bad = true;             // precondition: finite coordinates (z was checked by k_zrange_count)
     const int pos = atomicAdd(c.sr_cursor + s * c.R + r, 1);
     c.rec[pos] = make_float4(y, z, __int_as_float((int)i), 0.0f);

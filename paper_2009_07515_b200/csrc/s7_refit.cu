@@ -34,6 +34,16 @@ struct OwnedRows {
   }
 };
 
+// a residual as a signed 16-bit count of steps - one fp32 product, round to nearest with ties
+// to even (rintf), saturation at +-32767 with the comparisons written out (a NaN counts as below the range)
+__device__ __forceinline__ short quantise_residual(float res, float inv_step) {
+  const float v = res * inv_step;
+  const float r = rintf(v);
+  if (!(r > -32767.0f)) return (short)-32767;
+  if (r >= 32767.0f) return (short)32767;
+  return (short)(int)r;
+}
+
 __global__ void __launch_bounds__(kThreads) k_refit(Ctx c, FitPtrs o) {
   extern __shared__ float tx[];                         // row_x[r]
   for (int i = threadIdx.x; i < c.R; i += blockDim.x) tx[i] = c.rowtab[i].x;
@@ -52,7 +62,7 @@ __global__ void __launch_bounds__(kThreads) k_refit(Ctx c, FitPtrs o) {
     OwnedRows rows2 = rows;                              // positioned after the top cluster
     const int r_nxt = rows.next();
     // residual slots: the owned clusters of track id sit at trk_cl_start[id] .. in ASCENDING row, the walk is descending
-    const bool want_res = o.res_y != nullptr;
+    const bool want_res = o.res_y != nullptr, want_q = o.qres_y != nullptr;
     int slot = want_res ? o.trk_cl_start[id + 1] - 1 : 0;
     const int slot0 = want_res ? o.trk_cl_start[id] : 0;
     KF k;
@@ -72,17 +82,29 @@ __global__ void __launch_bounds__(kThreads) k_refit(Ctx c, FitPtrs o) {
       k.p[0] = pt.x; k.p[1] = 0.0f; k.p[2] = dy / dl; k.p[3] = dz / dl; k.p[4] = c.t_par[(size_t)sd * 5 + 4];
       kf_reset_cov(k, c);
       nfit = 1;
-      if (want_res) { o.res_y[slot] = 0.0f; o.res_z[slot] = 0.0f; --slot; }
+      if (want_res) {
+        o.res_y[slot] = 0.0f; o.res_z[slot] = 0.0f;
+        if (want_q) { o.qres_y[slot] = 0; o.qres_z[slot] = 0; }
+        --slot;
+      }
       for (int r = rows2.next(); r >= 0; r = rows2.next()) {
         if (!kf_propagate(k, c.kb, tx[r] - tx[cur], c.max_sinphi)) break;
         const float2 v = __ldg(yz + hit[r]);
-        if (want_res) { o.res_y[slot] = v.x - k.p[0]; o.res_z[slot] = (v.y - zref) - k.p[1]; --slot; }
+        if (want_res) {
+          const float ry = v.x - k.p[0], rz = (v.y - zref) - k.p[1];
+          o.res_y[slot] = ry; o.res_z[slot] = rz;
+          if (want_q) { o.qres_y[slot] = quantise_residual(ry, o.inv_step_y); o.qres_z[slot] = quantise_residual(rz, o.inv_step_z); }
+          --slot;
+        }
         kf_update(k, v.x, v.y - zref, c.err_y2, c.err_z2);
         cur = r; ++nfit;
       }
     }
     if (want_res)
-      for (; slot >= slot0; --slot) { o.res_y[slot] = 0.0f; o.res_z[slot] = 0.0f; }   // clusters that did not enter the fit
+      for (; slot >= slot0; --slot) {                                                   // clusters that did not enter the fit
+        o.res_y[slot] = 0.0f; o.res_z[slot] = 0.0f;
+        if (want_q) { o.qres_y[slot] = 0; o.qres_z[slot] = 0; }
+      }
 #pragma unroll
     for (int i = 0; i < 5; ++i) o.par[i * mt + id] = k.p[i];
 #pragma unroll

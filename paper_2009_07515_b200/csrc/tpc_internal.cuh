@@ -63,6 +63,7 @@ struct Ctx {
   int min_chain_len, max_gap, min_tracklet_hits, min_track_hits;
   float pick_chi2_cut, max_sinphi, y_margin, init_c_ss, init_c_tt, init_c_qq;
   int z_is_time; float cm_per_time_unit, drift_length;   // native time input
+  int y_is_pad; const float2* padtab; // native pad input: [R] (0.5 (n_pads_r - 1), pad_pitch_r)
   const RowTab* rowtab;               // [R]
   // capacities
   int max_clusters; int max_bins; int max_seeds; int max_tracks; int max_track_clusters;
@@ -132,6 +133,7 @@ int launch_reset(const Ctx& c, cudaStream_t st);
 struct FitPtrs {
   float* par; float* cov; float* x_ref; float* z_ref; float* chi2; int* ndf; int* n_fit;
   const int* trk_cl_start; float* res_y; float* res_z;   // optional (null: no residuals)
+  short* qres_y; short* qres_z; float inv_step_y, inv_step_z;   // optional residual codes
   int max_tracks;
 };
 int launch_refit(const Ctx& c, const FitPtrs& o, cudaStream_t st);   // S7, separate call
@@ -187,6 +189,15 @@ __device__ __forceinline__ float input_z(const Ctx& c, int s, float v) {
   if (!c.z_is_time) return v;
   const float zc = c.drift_length - v * c.cm_per_time_unit;
   return s < (c.S >> 1) ? zc : 0.0f - zc;
+}
+
+// the sector-local y of an input cluster of row r (< R) whose y entry is v (cm, or the pad
+// coordinate when y_is_pad).  -fmad=false: the difference and the product are rounded separately, like the oracle's.
+__device__ __forceinline__ float input_y(const Ctx& c, int r, float v) {
+  if (!c.y_is_pad) return v;
+  const float2 t = __ldg(c.padtab + r);
+  const float d = v - t.x;
+  return d * t.y;
 }
 
 // order-preserving float <-> int key (signed compare)

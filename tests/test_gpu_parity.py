@@ -113,6 +113,93 @@ def test_native_time_input_rejects_bad_parameters_and_flags_overflowing_times(cf
     assert out.numpy()["status"] & 3 and out.numpy()["n_tracks"] == 0 and trk.guards_intact()
 
 
+def test_residual_codes_bit_exact_and_bad_steps_rejected(mini_tf, mini_event):
+    """the optional 16-bit residual codes of tpc_tracker_refit equal the oracle's
+    code for code at two resolutions (0.1 mm: the working point; 1 um: most codes saturate), the float residuals beside
+    them are unchanged, entries of clusters that did not enter the fit are 0; half-given or non-positive arguments are
+    INVALID_ARG."""
+    for tf, steps in ((mini_tf, (0.01, 0.02)), (mini_event, (1e-4, 1e-4)), (mini_tf, (0.25, 7.0))):
+        P, trk, out = run_gpu(tf)
+        T = out.numpy()["n_tracks"]
+        o = run_oracle(tf, P, last_stage=6).quantise_residuals(*steps)
+        fit = trk.refit(T, tracks=out, steps=steps)
+        assert fit["qres_y"].dtype == np.int16 and fit["qres_y"].size == o.get("fit_qres_y").size > 10_000
+        assert np.array_equal(fit["qres_y"].astype(np.int32), o.get("fit_qres_y"))
+        assert np.array_equal(fit["qres_z"].astype(np.int32), o.get("fit_qres_z"))
+        assert np.array_equal(fit["res_y"], o.get("fit_res_y").astype(np.float32))
+        assert np.array_equal(fit["par"], o.get("fit_par").astype(np.float32).reshape(-1, 5))
+    assert (np.abs(fit["qres_y"]) <= 1).mean() > 0.99             # 2.5 mm steps: almost everything rounds to 0 or +-1
+    buf = trk.new_fit(steps=(0.01, 0.01))
+    for bad in (dict(res_step_y=0.0), dict(res_step_z=-1.0), dict(res_step_y=float("inf")), dict(res_step_z=float("nan")),
+                dict(qres_z=None)):
+        b = dict(buf); b.update(bad)
+        if b.get("qres_z", 0) is None:
+            del b["qres_z"]
+        with pytest.raises(RuntimeError, match="invalid argument"):
+            trk.refit_into(b, out=out)
+    b = {k: v for k, v in buf.items() if k not in ("res_y", "res_z")}   # codes without the residuals
+    with pytest.raises(RuntimeError, match="invalid argument"):
+        trk.refit_into(b)
+    trk.refit_into(buf, out=out)
+    torch.cuda.synchronize()
+
+
+def test_native_pad_and_time_input_bit_exact(mini_tf):
+    """the y array holds native pad coordinates; S1 converts while it reads.  Every
+    stage, the refit and the keep flags bit-exact against the oracle on the same pads - alone, and together with the native
+    time (the detector's (pad, row, time) input); the sorted y the tracker works on is the frame's own y within the fp32
+    rounding of the pad coordinate."""
+    from tpc_synth import to_native_pad, to_native_time
+    tfp, pp = to_native_pad(mini_tf)
+    tfpt, tp = to_native_time(tfp)
+    for frame, extra in ((tfp, pp), (tfpt, {**pp, **tp})):
+        P = default_params(mini_tf); P.update(extra)
+        _, trk, out = run_gpu(frame, params=P)
+        o = run_oracle(frame, P, last_stage=6)
+        assert trk.counters()["status"] == 0
+        assert not compare_integer_stages(trk, o)
+        t = compare_tracklets(trk, o)
+        assert t["hit_mismatch_seeds"] == 0 and t["par_bitexact"] and t["cov_bitexact"] and t["chi2_bitexact"], t
+        res = compare_tracks(out.numpy(), o, frame.n)
+        assert res["cluster_track_equal"] and res["csr_equal"] and res["n_tracks"][0] > 1000, res
+        g = out.numpy()
+        fit = trk.refit(g["n_tracks"], tracks=out)
+        assert np.array_equal(fit["par"], o.get("fit_par").astype(np.float32).reshape(-1, 5))
+        assert np.array_equal(fit["res_y"], o.get("fit_res_y").astype(np.float32))
+        keep = trk.protect(out, 1.0, 1.0)
+        torch.cuda.synchronize()
+        assert np.array_equal(keep.cpu().numpy()[: frame.n].astype(np.int32), o.protect(1.0, 1.0))
+        y_in = np.empty(frame.n, np.float32); y_in[trk.stage_view("perm")] = trk.stage_view("yz").reshape(-1, 2)[:, 0]
+        assert np.abs(y_in.astype(np.float64) - mini_tf.y).max() < 2e-5
+    # the host path converts the same way
+    _, trk_h, out_h = run_gpu(frame, params=P, host=True)
+    assert np.array_equal(out_h.numpy()["cluster_track"], g["cluster_track"])
+
+
+def test_native_pad_input_rejects_bad_tables_and_flags_non_finite_pads(cfg1):
+    import copy
+    import paper_2009_07515_b200 as tpc
+    from tpc_synth import to_native_pad
+    tfp, pp = to_native_pad(cfg1)
+    R = cfg1.geometry.n_rows
+    zero_pads = pp["n_pads"].copy(); zero_pads[7] = 0
+    for bad in (dict(n_pads=zero_pads), dict(pad_pitch=np.where(np.arange(R) == 3, 0.0, pp["pad_pitch"]).astype(np.float32)),
+                dict(pad_pitch=np.where(np.arange(R) == 3, np.inf, pp["pad_pitch"]).astype(np.float32)),
+                dict(pad_pitch=np.where(np.arange(R) == 150, np.nan, pp["pad_pitch"]).astype(np.float32))):
+        P = default_params(cfg1); P.update(pp); P.update(bad)
+        with pytest.raises((RuntimeError, ValueError)):
+            tpc.Tracker(P, 1024, 1024, 64, 64, 1024)
+    P = default_params(cfg1); P.update(pp)
+    for v in (np.inf, np.nan):
+        tfb = copy.copy(tfp); tfb.y = tfp.y.copy(); tfb.y[11] = np.float32(v)
+        _, trk, out = run_gpu(tfb, params=P, guard_bytes=1 << 20)
+        assert out.numpy()["status"] & 1 and out.numpy()["n_tracks"] == 0 and trk.guards_intact()
+    # a row id out of range with the pad flag on: rejected before the pad table is indexed
+    tfb = copy.copy(tfp); tfb.row = tfp.row.copy(); tfb.row[5] = 200
+    _, trk, out = run_gpu(tfb, params=P, guard_bytes=1 << 20)
+    assert out.numpy()["status"] & 1 and trk.guards_intact()
+
+
 def test_reports_bit_exactness(mini_event):
     """Not a requirement of north_star, but the design goal: identical op order => identical bits."""
     P, trk, out = run_gpu(mini_event)
