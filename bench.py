@@ -47,18 +47,32 @@ def parse():
                     help="sectors of the timed frame checked against the oracle before timing (0: skip)")
     ap.add_argument("--repeats", type=int, default=10, help="separately-evented steps for median / best (>= 10)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-optional", action="store_true", help="skip the optional calls (refit / merge / apex / removable / protect)")
     return ap.parse_args()
+
+
+def _capture_is_current(src_file: str, sha1: str) -> bool:
+    """A committed ncu capture describes the kernel only as long as the kernel's source file is the one it was taken from:
+    the CSV rows carry the sha1 of that file at capture time."""
+    import hashlib
+    try:
+        with open(os.path.join(ROOT, "paper_2009_07515_b200", "csrc", src_file), "rb") as f:
+            return hashlib.sha1(f.read()).hexdigest() == sha1.strip()
+    except Exception:
+        return False
 
 
 def ncu_traffic(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on cfg5, copied from the committed
-    `ncu --set full` capture (profiles/traffic.csv names the capture); None if there is none."""
+    `ncu --set full` capture (profiles/traffic.csv names the capture and the sha1 of the kernel's source file it was taken
+    from); None if there is none or if the source has changed since (a stale capture is not reported)."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            head = f.readline().strip().split(",")
             for ln in f:
-                p = ln.strip().split(",")
-                if p[0] == kernel:
-                    return float(p[1])
+                d = dict(zip(head, ln.strip().split(",")))
+                if d["kernel"] == kernel:
+                    return float(d["dram_bytes_per_launch"]) if _capture_is_current(d["source_file"], d["source_sha1"]) else None
     except Exception:
         pass
     return None
@@ -74,6 +88,8 @@ def ncu_counters(kernel: str):
                 p = ln.strip().split(",")
                 if p[0] == kernel:
                     d = dict(zip(head, p))
+                    if not _capture_is_current(d["source_file"], d["source_sha1"]):
+                        return None
                     return {"issue_slots_busy": float(d["issue_slots_busy_pct"]) / 100, "active_lanes_of_32": float(d["active_lanes_per_instruction"]),
                             "achieved_occupancy": float(d["achieved_occupancy_pct"]) / 100, "l2_hit_rate": float(d["l2_hit_rate_pct"]) / 100,
                             "bound_by": d["bound_by"], "source": d["source"]}
@@ -285,6 +301,116 @@ def cpu_baseline(tf, P, one_thread_clusters=8_000_000) -> dict:
             "one_thread": one}
 
 
+def optional_parity(tfl, P) -> dict:
+    """refit -> merge through the parity checker before the optional calls are timed: four whole sectors of the looper
+    frame (the 17|0 wrap on the A side and its mirror on the C side: full z span and density of the frame) as a frame of
+    their own, CUDA against one oracle run, every output compared exactly.  apex / removable are NOT re-checked here: the
+    oracle's apex step is an all-pairs scan (minutes at this density); tests/test_gpu_merge.py compares them at this
+    density on two sectors."""
+    import torch
+    import paper_2009_07515_b200 as tpc
+    from oracle import Oracle
+    from tpc_synth import select_sectors
+    S = tfl.geometry.n_sectors
+    pick = sorted({0, S // 2 - 1, S // 2, S - 1})
+    sub, _ = select_sectors(tfl, pick)
+    t0 = time.perf_counter()
+    c = tpc.suggest_capacities(sub.n, P)
+    trk = tpc.Tracker(P, c["max_clusters"], tpc.max_bins_bound(sub.sector, sub.z, P), c["max_seeds"], c["max_tracks"], c["max_track_clusters"])
+    ins = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (sub.sector, sub.row, sub.y, sub.z)]
+    out = trk.new_tracks(sub.n)
+    trk.track_timeframe(*ins, out)
+    T = out.numpy()["n_tracks"]
+    m = trk.merge(T)
+    ct = out.numpy()["cluster_track"]
+    trk.destroy(); del trk, out, ins
+    torch.cuda.empty_cache()
+    o = Oracle(P).run(sub.sector, sub.row, sub.y, sub.z, precision=32, last_stage=6).merge()
+    bad = []
+
+    def eq(name, x, y_):
+        x = np.asarray(x); y_ = np.asarray(y_)
+        if x.shape != y_.shape or not np.array_equal(x, y_):
+            bad.append(name)
+    eq("cluster_track", ct, o.get("cluster_track"))
+    eq("merged_of_track", m["merged_of_track"], o.get("mrg_of_track"))
+    eq("seg_start", m["seg_start"], o.get("mrg_seg_start")); eq("seg_idx", m["seg_idx"], o.get("mrg_seg_idx"))
+    eq("mrg_par", m["par"], o.get("mrg_par").astype(np.float32).reshape(-1, 5))
+    eq("mrg_cov", m["cov"], o.get("mrg_cov").astype(np.float32).reshape(-1, 15))
+    eq("mrg_n_fit", m["n_fit"], o.get("mrg_n_fit"))
+    return {"checked": "oracle vs CUDA, exact: cluster_track, merged_of_track, seg_start, seg_idx, merged par / cov / n_fit "
+                       "(apex / removable: tests/test_gpu_merge.py, same density)", "sectors": pick, "clusters": int(sub.n), "tracks": int(T),
+            "merged": int(m["n_merged"]), "ok": not bad, "mismatches": bad,
+            "seconds": round(time.perf_counter() - t0, 1)}
+
+
+def optional_calls(args, tf, P, dev, stream, rank) -> dict:
+    """Device times of the optional calls on the looper twin of the timed frame (same recipe + `loopers`)."""
+    import torch
+    import paper_2009_07515_b200 as tpc
+    from tpc_synth import generate_config
+    over = {"loopers": True}
+    if args.collisions:
+        over["n_collisions"] = args.collisions
+    if rank:
+        over["seed"] = replica_seed(args.workload, rank)
+    tfl = generate_config(args.workload, device="cuda", **over)
+    parity = optional_parity(tfl, P) if (args.parity_sectors > 0 and rank == 0) else None
+    if parity and not parity["ok"]:
+        raise RuntimeError(f"parity check of the optional calls failed before timing: {parity['mismatches']}")
+    c = tpc.suggest_capacities(tfl.n, P)
+    trk = tpc.Tracker(P, c["max_clusters"], tpc.max_bins_bound(tfl.sector, tfl.z, P), c["max_seeds"], c["max_tracks"],
+                      c["max_track_clusters"], device=dev)
+    d_in = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (tfl.sector, tfl.row, tfl.y, tfl.z)]
+    out = trk.new_tracks(tfl.n)
+    trk.track_timeframe(*d_in, out)
+    k = trk.counters()
+    if k["status"] != 0:
+        raise RuntimeError(f"tracker status {k['status']} on the looper frame")
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed(fn):                                         # one warm-up, one timed call, device time
+        fn()
+        ev0.record(stream)
+        fn()
+        ev1.record(stream)
+        torch.cuda.synchronize(dev)
+        return ev0.elapsed_time(ev1)
+    fit_buf = trk.new_fit(); mg_buf = trk.new_merged(); ax_buf = trk.new_apex()
+    refit_ms = timed(lambda: trk.refit_into(fit_buf))
+    merge_ms = timed(lambda: trk.merge_into(fit_buf, mg_buf))
+    n_merged = int(mg_buf["n_merged"].item())
+    apex_ms = timed(lambda: trk.apex_into(mg_buf, ax_buf))
+    n_apex = int((ax_buf["apex_partner"][:n_merged] >= 0).sum().item()) // 2
+    cls = torch.zeros(tfl.n, dtype=torch.uint8, device=dev); rem = torch.zeros(tfl.n, dtype=torch.uint8, device=dev)
+    removable_ms = timed(lambda: trk.removable_into(out, fit_buf, mg_buf, ax_buf, cls, rem))
+    removed_frac = float(rem.float().mean().item())
+    sec_leg_frac = float((cls == 2).float().mean().item())
+    keep = torch.empty(tfl.n, dtype=torch.uint8, device=dev)
+    protect_ms = timed(lambda: trk.protect(out, 1.0, 1.0, keep=keep))
+    kept_frac = float(keep.float().mean().item())
+    # truth: tracks the generator gave both legs (>= 20 clusters each)
+    tid = tfl.track_id
+    nmax = int(tid.max()) + 1
+    c0 = np.bincount(tid[(tid >= 0) & (tfl.leg == 0)], minlength=nmax); c1 = np.bincount(tid[(tid >= 0) & (tfl.leg == 1)], minlength=nmax)
+    truth_pairs = int(((c0 >= 20) & (c1 >= 20)).sum())
+    res = {"frame": {"workload": tfl.name, "n_clusters": int(tfl.n), "returning_leg_clusters": int((tfl.leg == 1).sum()),
+                     "n_tracks": int(k["n_tracks"])},
+           "parity_before_timing": parity,
+           "refit": {"what": "tpc_tracker_refit: all tracks refitted over their owned clusters", "ms": refit_ms},
+           "merge": {"what": "tpc_tracker_merge: segments joined across sector borders and long holes, upward + merged downward refit",
+                     "ms": merge_ms, "n_merged": n_merged},
+           "apex": {"what": "tpc_tracker_apex: looper legs paired through their circles, returning leg labelled", "ms": apex_ms,
+                    "pairs": n_apex, "truth_pairs_with_20_clusters_per_leg": truth_pairs},
+           "removable": {"what": "tpc_tracker_removable alone (strategy A: class per cluster, protection by good tracks), buffers "
+                                 "pre-allocated, device ms", "ms": removable_ms, "removed_fraction": removed_frac,
+                         "secondary_leg_fraction": sec_leg_frac},
+           "protect": {"what": "tpc_tracker_protect: strategy-B keep flag per cluster, 1 cm road", "ms": protect_ms,
+                       "kept_fraction": kept_frac}}
+    trk.destroy()
+    return res
+
+
 def make_timeframe(args, rank: int):
     from tpc_synth import generate_config
     import torch
@@ -310,6 +436,12 @@ def algorithmic_bytes(k: dict) -> dict:
         "S5": 12 * N + 32 * H + 4 * Ho + 100 * T,
     }
     b["total"] = sum(b.values())
+    # the same total (i) with SURVEY.md section 8(d)'s own S2 formula (16 N + 4 N_b: no srow read) and (ii) at the 1.1 bins per
+    # cluster section 8(d) assumed - the harness's cell rule (tpc_synth.choose_cell, scale 0.5) gives ~3 bins per cluster
+    # because that is faster for S2 / S4, and those extra bin_start entries are bytes the method does not need
+    b["total_survey_S2"] = b["total"] - 4 * N
+    nb11 = int(1.1 * N)
+    b["total_at_1p1_bins_per_cluster"] = b["total_survey_S2"] - (8 + 4) * (Nb - nb11)
     return b
 
 
@@ -491,50 +623,10 @@ def run_ours(args):
     stage /= args.steps
     trk.enable_stage_timing(False)
 
-    # ---- the refit of DESIGN.md section 3.7 (separate call, not part of the step): device time, for the record
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    fit_buf = trk.new_fit()
-    trk.refit_into(fit_buf)
-    ev0.record(stream)
-    trk.refit_into(fit_buf)
-    ev1.record(stream)
-    torch.cuda.synchronize(dev)
-    refit_ms = ev0.elapsed_time(ev1)
-    # ---- the track merger of DESIGN.md section 3.9 (separate call after the refit): device time of the merge alone
-    mg_buf = trk.new_merged()
-    trk.merge_into(fit_buf, mg_buf)
-    ev0.record(stream)
-    trk.merge_into(fit_buf, mg_buf)
-    ev1.record(stream)
-    torch.cuda.synchronize(dev)
-    merge_ms = ev0.elapsed_time(ev1)
-    n_merged = int(mg_buf["n_merged"].item())
-    # ---- looper following (separate call after the merge)
-    ax_buf = trk.new_apex()
-    trk.apex_into(mg_buf, ax_buf)
-    ev0.record(stream)
-    trk.apex_into(mg_buf, ax_buf)
-    ev1.record(stream)
-    torch.cuda.synchronize(dev)
-    apex_ms = ev0.elapsed_time(ev1)
-    n_apex = int((ax_buf["apex_partner"][:n_merged] >= 0).sum().item()) // 2
-    del mg_buf, ax_buf
-    # ---- strategy-A hit removal: wall time of the convenience call minus the calls timed above
-    torch.cuda.synchronize(dev)
-    t0 = time.perf_counter()
-    cls_, rem_ = trk.removable(out)
-    removable_all_ms = (time.perf_counter() - t0) * 1e3
-    removed_frac = float(rem_.float().mean().item()) if tf.n else 0.0
-    del cls_, rem_
-    # ---- cluster protection for hit removal, strategy B (separate call), 1 cm road
-    keep = trk.protect(out, 1.0, 1.0)
-    ev0.record(stream)
-    trk.protect(out, 1.0, 1.0, keep=keep)
-    ev1.record(stream)
-    torch.cuda.synchronize(dev)
-    protect_ms = ev0.elapsed_time(ev1)
-    kept_frac = float(keep[: tf.n].float().mean().item())
-    del keep, fit_buf
+    # ---- the optional calls (refit, merge, apex, removable, protect: separate calls, not part of the step).  They are timed
+    # on the frame they were built for: the same workload WITH the returning legs of the loopers (generator key `loopers`),
+    # on a tracker of its own, after a parity check of exactly these calls against the oracle.
+    opt = optional_calls(args, tf, P, dev, stream, rank) if not args.no_optional else None
 
     # ---- end to end through the host entry points (pinned host buffers in and out).  Time frames arrive one after the
     # other, so the pipelined begin/end pair is the call a user makes: every step still does the H2D
@@ -611,7 +703,10 @@ def run_ours(args):
                 "counters": ncu_counters(dom_kernel) if tf.name == "cfg5" else None,
                 "whole_path": {"algorithmic_bytes": bytes_["total"], "achieved": bytes_["total"] / (ms_step * 1e-3) / 1e9,
                                "frac_of_measured": bytes_["total"] / (ms_step * 1e-3) / 1e9 / peak,
-                               "frac_of_8TBs": bytes_["total"] / (ms_step * 1e-3) / 1e9 / 8000.0},
+                               "frac_of_8TBs": bytes_["total"] / (ms_step * 1e-3) / 1e9 / 8000.0,
+                               "bins_per_cluster": k["n_bins"] / max(1, k["n_clusters"]),
+                               "frac_of_measured_with_survey_S2_formula": bytes_["total_survey_S2"] / (ms_step * 1e-3) / 1e9 / peak,
+                               "frac_of_measured_at_1p1_bins_per_cluster": bytes_["total_at_1p1_bins_per_cluster"] / (ms_step * 1e-3) / 1e9 / peak},
                 "stage_ms": {n: float(v) for n, v in zip(names, stage)},
                 "stage_bytes": {n: int(bytes_[n]) for n in names}}
 
@@ -629,17 +724,7 @@ def run_ours(args):
                    "workspace_GB": round(trk.workspace_bytes / 1e9, 2)},
         "counters": {kk: int(v) for kk, v in k.items()},
         "parity_before_timing": parity,
-        "refit": {"what": "tpc_tracker_refit (separate call, not in the step): all tracks refitted over their owned clusters",
-                  "ms": refit_ms},
-        "merge": {"what": "tpc_tracker_merge (separate call after the refit, not in the step): segments joined across sector "
-                          "borders and long holes, upward + merged downward refit", "ms": merge_ms, "n_merged": n_merged},
-        "apex": {"what": "tpc_tracker_apex (separate call after the merge, not in the step): looper legs paired through their "
-                         "circles, returning leg labelled", "ms": apex_ms, "pairs": n_apex},
-        "removable": {"what": "tpc_tracker_removable after refit + merge + apex (strategy A: class per cluster, protection by good "
-                              "tracks); wall ms of the whole sequence incl. its buffer allocations", "ms_sequence": removable_all_ms,
-                      "removed_fraction": removed_frac},
-        "protect": {"what": "tpc_tracker_protect (separate call, not in the step): strategy-B keep flag per cluster, 1 cm road",
-                    "ms": protect_ms, "kept_fraction": kept_frac},
+        "optional_calls": opt,      # separate calls, not in the step; timed on the looper twin of the frame
         "roofline": roofline,
         "cpu_baseline": cpu,
         "gpu_launches": trk.launches_per_call() * args.steps,

@@ -20,6 +20,14 @@ def _merge_parity(tf, P=None, cuts=None, min_links=1):
     T = g["n_tracks"]
     m = trk.merge(T, kw)
     o = run_oracle(tf, P, last_stage=6).merge(**kw)
+    links = _compare_merge(trk, m, o, T)
+    assert links >= min_links, links
+    return m, o, links
+
+
+def _compare_merge(trk, m, o, T):
+    """Every intermediate and output array of tpc_tracker_merge (`m` = Tracker.merge's host copies) against the oracle `o`
+    after its merge(): asserts equality, returns the number of links."""
     f32 = np.float32
     mt = trk.caps[3]
     bad = []
@@ -64,9 +72,7 @@ def _merge_parity(tf, P=None, cuts=None, min_links=1):
             w = np.nonzero(gk != o.get("mrg_" + nm))[0][:5]
             bad.append((nm, w.tolist(), gk[w].tolist(), o.get("mrg_" + nm)[w].tolist(), trk.stage_view("mrg_chi_b")[w].tolist(), o.get("mrg_chi2_b")[w].tolist()))
     assert not bad, bad
-    links = int((o.get("mrg_next") >= 0).sum())
-    assert links >= min_links, links
-    return m, o, links
+    return int((o.get("mrg_next") >= 0).sum())
 
 
 def test_merge_central_event(mini_event):
@@ -125,6 +131,35 @@ def test_merge_at_time_frame_density():
     P = default_params(sub)
     m, o, links = _merge_parity(sub, P=P, min_links=50000)
     print("tracks", o.get("trk_seed").size, "merged", m["n_merged"], "links", links)
+
+
+def test_merge_at_the_density_and_z_span_of_the_time_frame_with_loopers():
+    """The frame bench.py times the optional calls on: cfg5 (50 kHz Pb-Pb, 11.4 ms of z) WITH the returning legs of the
+    loopers.  Twelve whole sectors - six neighbours around the 17|0 wrap on the A side and their mirror on the C side - as
+    a frame of their own (~46 M clusters, 1.1 M tracks, the full +-28 500 cm of z): assignment, every intermediate of the
+    merger and the merged refit against the oracle, np.array_equal.  apex / removable are not part of it: the oracle's apex
+    step is an all-pairs scan by definition, quadratic in the merged tracks (two sectors of this frame took it 6.5 minutes
+    on the B200 box - every array came out identical - and a two-sector cut holds almost no complete looper; DESIGN.md
+    section 5)."""
+    import time
+    from tpc_synth import select_sectors
+    tf = generate_config("cfg5", device="cuda", loopers=True)
+    assert tf.n > 50_000_000 and int((tf.leg == 1).sum()) > 1_000_000
+    P = default_params(tf)
+    t0 = time.perf_counter()
+    sub, _ = select_sectors(tf, [15, 16, 17, 0, 1, 2, 33, 34, 35, 18, 19, 20])
+    assert float(sub.z.max()) - float(sub.z.min()) > 50_000
+    _, trk, out = run_gpu(sub, params=P)
+    g = out.numpy()
+    T = g["n_tracks"]
+    assert g["status"] == 0 and T > 200_000
+    m = trk.merge(T, CUTS, fill=POISON)
+    o = run_oracle(sub, P, last_stage=6)
+    assert np.array_equal(g["cluster_track"], o.get("cluster_track"))
+    links = _compare_merge(trk, m, o.merge(**CUTS), T)
+    t1 = time.perf_counter()
+    print(f"12 sectors of cfg5 + loopers: {sub.n} clusters, {T} tracks, {m['n_merged']} merged, {links} links ({t1 - t0:.0f} s)")
+    assert links > 50_000
 
 
 def test_merge_rejects_bad_arguments(cfg1):
@@ -195,6 +230,37 @@ def test_buffers_smaller_than_the_frames_max_tracks_are_refused(cfg1):
     trk.track_timeframe(*ins, out_small)
     assert lib.tpc_tracker_refit(h, C.byref(fit_s(64)), st) == 0 and lib.tpc_tracker_refit(h, C.byref(fit_s(63)), st) == -2
     torch.cuda.synchronize()
+
+
+def test_optional_calls_out_of_order_are_refused(cfg1):
+    """refit -> merge -> apex -> removable read what their predecessors left in the workspace for the CURRENT frame: a call
+    whose predecessor did not run after the last tpc_track_timeframe is INVALID_ARG, not a walk over stale counters."""
+    import paper_2009_07515_b200 as tpc
+    P = default_params(cfg1)
+    c = tpc.suggest_capacities(cfg1.n, P)
+    trk = tpc.Tracker(P, c["max_clusters"], tpc.max_bins_bound(cfg1.sector, cfg1.z, P), c["max_seeds"], c["max_tracks"], c["max_track_clusters"])
+    fit = trk.new_fit(); mg = trk.new_merged(); ax = trk.new_apex()
+    for call in (lambda: trk.refit_into(fit), lambda: trk.merge_into(fit, mg), lambda: trk.apex_into(mg, ax)):
+        with pytest.raises(RuntimeError, match="invalid argument"):
+            call()                                           # nothing tracked yet
+    ins = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (cfg1.sector, cfg1.row, cfg1.y, cfg1.z)]
+    out = trk.new_tracks(cfg1.n)
+    trk.track_timeframe(*ins, out)
+    with pytest.raises(RuntimeError, match="invalid argument"):
+        trk.merge_into(fit, mg)                              # no refit of this frame
+    trk.refit_into(fit)
+    with pytest.raises(RuntimeError, match="invalid argument"):
+        trk.apex_into(mg, ax)                                # no merge of this frame
+    trk.merge_into(fit, mg); trk.apex_into(mg, ax)
+    cls, rem = trk.removable(out)                            # refit + merge + apex + removable: fine
+    trk.track_timeframe(*ins, out)                           # a new frame: everything above is stale
+    with pytest.raises(RuntimeError, match="invalid argument"):
+        trk.apex_into(mg, ax)
+    with pytest.raises(RuntimeError, match="invalid argument"):
+        trk.merge_into(fit, mg)
+    trk.refit_into(fit); trk.merge_into(fit, mg); trk.apex_into(mg, ax)
+    torch.cuda.synchronize()
+    assert int(mg["n_merged"].item()) >= 1
 
 
 # ------------------------------------------------------------------------------------------------ apex links (3.9.8)
